@@ -1,0 +1,205 @@
+"""ctypes wrapper around oracle/lbcnn_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this.  It never imports the CUDA package.  The search loop below follows PAPER.md:88,94 (section
+III, Cells 5/6): for every candidate kernel set, expand train and test sets, fit ELM0 on the train
+features, score the test set, keep best and lowest.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lbcnn_oracle.c")
+_LIB = os.path.join(_HERE, "liblbcnn_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp; rebuilt when the source is newer than the library."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-mavx2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c11",
+               "-Wall", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Layer(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("conv_type", "n_kernels", "ksize", "act", "pool_k", "pool_s", "pool_p", "pool_cover_all")]
+
+
+class _Arch(C.Structure):
+    _fields_ = [("in_h", C.c_int32), ("in_w", C.c_int32), ("in_c", C.c_int32), ("n_layers", C.c_int32),
+                ("layer", _Layer * 3)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.orc_pool_out_size.restype = C.c_int
+        for f in ("orc_feature_dim", "orc_param_bits", "orc_conv", "orc_maxpool", "orc_expand", "orc_elm_fit",
+                  "orc_elm_score"):
+            getattr(_lib, f).restype = C.c_int
+    return _lib
+
+
+def n_threads() -> int:
+    """threads the OpenMP runtime will use (OMP_NUM_THREADS or the cores visible to this process)."""
+    v = os.environ.get("OMP_NUM_THREADS")
+    if v:
+        return int(v.split(",")[0])
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def make_arch(in_h: int, in_w: int, in_c: int, layers: Sequence) -> _Arch:
+    """layers: objects/tuples with (conv_type, n_kernels, ksize, act, pool_k, pool_s, pool_p, pool_cover_all)."""
+    a = _Arch()
+    a.in_h, a.in_w, a.in_c, a.n_layers = in_h, in_w, in_c, len(layers)
+    for i, L in enumerate(layers):
+        t = tuple(L) if isinstance(L, (tuple, list)) else (
+            L.conv_type, L.n_kernels, L.ksize, L.act, L.pool_k, L.pool_s, L.pool_p, L.pool_cover_all)
+        for name, v in zip([f[0] for f in _Layer._fields_], t):
+            setattr(a.layer[i], name, int(v))
+    return a
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def pool_out_size(n, k, s, p, cover_all) -> int:
+    return _load().orc_pool_out_size(int(n), int(k), int(s), int(p), int(cover_all))
+
+
+def feature_dim(arch: _Arch) -> Tuple[int, Tuple[int, int, int]]:
+    F = C.c_int64()
+    hwc = (C.c_int32 * 3)()
+    rc = _load().orc_feature_dim(C.byref(arch), C.byref(F), hwc)
+    if rc:
+        raise ValueError("invalid architecture (status %d)" % rc)
+    return F.value, tuple(hwc)
+
+
+def param_bits(arch: _Arch, n_classes: int) -> Tuple[int, int]:
+    cb, eb = C.c_int64(), C.c_int64()
+    rc = _load().orc_param_bits(C.byref(arch), int(n_classes), C.byref(cb), C.byref(eb))
+    if rc:
+        raise ValueError("invalid architecture (status %d)" % rc)
+    return cb.value, eb.value
+
+
+def conv(conv_type, n_kernels, ksize, a: np.ndarray, w: np.ndarray, bias: Optional[np.ndarray] = None) -> np.ndarray:
+    """a: int64 [n][h][w][cin]; w: int8 [n_kernels][cin][k][k]; returns int64 [n][h][w][cout]."""
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    w = np.ascontiguousarray(w, dtype=np.int8)
+    n, h, ww, cin = a.shape
+    cout = n_kernels if conv_type == 0 else cin * n_kernels
+    assert w.size == n_kernels * cin * ksize * ksize
+    b = None if bias is None else np.ascontiguousarray(bias, dtype=np.int32)
+    z = np.empty((n, h, ww, cout), dtype=np.int64)
+    rc = _load().orc_conv(int(conv_type), int(n_kernels), int(ksize), _p(a), C.c_int64(n), h, ww, cin, _p(w), _p(b), _p(z))
+    if rc:
+        raise ValueError("orc_conv status %d" % rc)
+    return z
+
+
+def maxpool(z: np.ndarray, k, s, p, cover_all) -> np.ndarray:
+    z = np.ascontiguousarray(z, dtype=np.int64)
+    n, h, w, c = z.shape
+    ho, wo = pool_out_size(h, k, s, p, cover_all), pool_out_size(w, k, s, p, cover_all)
+    if ho < 1 or wo < 1:
+        raise ValueError("invalid pooling geometry")
+    u = np.empty((n, ho, wo, c), dtype=np.int64)
+    rc = _load().orc_maxpool(_p(z), C.c_int64(n), h, w, c, int(k), int(s), int(p), int(cover_all), _p(u))
+    if rc:
+        raise ValueError("orc_maxpool status %d" % rc)
+    return u
+
+
+def expand(arch: _Arch, images: np.ndarray, kernels: np.ndarray, bias: Optional[np.ndarray] = None) -> np.ndarray:
+    """images u8 [n][H][W][C]; kernels int8 [n_weights] of ONE candidate; returns int64 [n][F] (exact integers)."""
+    images = np.ascontiguousarray(images, dtype=np.uint8)
+    kernels = np.ascontiguousarray(kernels, dtype=np.int8)
+    assert images.shape[1:] == (arch.in_h, arch.in_w, arch.in_c), images.shape
+    F, _ = feature_dim(arch)
+    b = None if bias is None else np.ascontiguousarray(bias, dtype=np.int32)
+    u = np.empty((images.shape[0], F), dtype=np.int64)
+    rc = _load().orc_expand(C.byref(arch), _p(images), C.c_int64(images.shape[0]), _p(kernels), _p(b), _p(u))
+    if rc:
+        raise ValueError("orc_expand status %d" % rc)
+    return u
+
+
+def elm_fit(H: np.ndarray, labels: np.ndarray, n_classes: int, Creg: float, force_branch: int = 0):
+    """H fp64 [n][F]; returns (W fp64 [F][classes], info, branch) -- branch 1 primal ('LLL'), 2 dual ('MMM')."""
+    H = np.ascontiguousarray(H, dtype=np.float64)
+    labels = np.ascontiguousarray(labels, dtype=np.int32)
+    n, F = H.shape
+    W = np.zeros((F, n_classes), dtype=np.float64)
+    br = C.c_int32()
+    info = _load().orc_elm_fit(_p(H), C.c_int64(n), C.c_int64(F), _p(labels), int(n_classes), C.c_double(Creg),
+                               int(force_branch), _p(W), C.byref(br))
+    if info < 0:
+        raise ValueError("orc_elm_fit bad argument (%d)" % info)
+    return W, info, br.value
+
+
+def elm_score(H: np.ndarray, W: np.ndarray, labels: Optional[np.ndarray] = None, want_margin: bool = False):
+    """returns (pred int32 [n], correct or None, margin or None)."""
+    H = np.ascontiguousarray(H, dtype=np.float64)
+    W = np.ascontiguousarray(W, dtype=np.float64)
+    n, F = H.shape
+    assert W.shape[0] == F
+    classes = W.shape[1]
+    lab = None if labels is None else np.ascontiguousarray(labels, dtype=np.int32)
+    pred = np.empty(n, dtype=np.int32)
+    corr = C.c_int64(0)
+    mar = np.empty(n, dtype=np.float64) if want_margin else None
+    rc = _load().orc_elm_score(_p(H), C.c_int64(n), C.c_int64(F), _p(W), classes, _p(lab), _p(pred), C.byref(corr), _p(mar))
+    if rc:
+        raise ValueError("orc_elm_score status %d" % rc)
+    return pred, (corr.value if labels is not None else None), mar
+
+
+def search(arch: _Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: float, kernels: np.ndarray,
+           feature_scale: float = 1.0 / 255.0, bias: Optional[np.ndarray] = None, keep: bool = False):
+    """The paper's trial loop: one trial per candidate kernel set.
+    feature_scale is the fp32 number the library receives, widened to double (R6).
+    Returns dict(acc [K] float64, correct [K], info [K], best, worst, W_best, and per-candidate W/pred if keep)."""
+    K = kernels.shape[0]
+    s = float(np.float32(feature_scale))
+    acc = np.zeros(K)
+    correct = np.zeros(K, dtype=np.int64)
+    info = np.zeros(K, dtype=np.int32)
+    Ws, preds = [], []
+    for k in range(K):
+        b = None if bias is None else bias[k]
+        Htr = expand(arch, train_x, kernels[k], b).astype(np.float64) * s
+        Hte = expand(arch, test_x, kernels[k], b).astype(np.float64) * s
+        W, inf, _ = elm_fit(Htr, train_y, n_classes, Creg)
+        info[k] = inf
+        if inf:
+            acc[k], correct[k] = -1.0, 0
+            Ws.append(None); preds.append(None)
+            continue
+        pred, corr, _ = elm_score(Hte, W, test_y)
+        correct[k] = corr
+        acc[k] = corr / float(len(test_y))
+        Ws.append(W); preds.append(pred)
+    best = int(np.argmax(acc))          # first index of the maximum (R13)
+    worst = int(np.argmin(acc))
+    out = dict(acc=acc, correct=correct, info=info, best=best, worst=worst, W_best=Ws[best])
+    if keep:
+        out["W"], out["pred"] = Ws, preds
+    return out
