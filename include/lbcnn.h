@@ -1,0 +1,153 @@
+/*
+ * lbcnn.h -- C ABI of the B200-native LB-CNN kernel-selection inner loop (arXiv 2106.15350).
+ *
+ * The loop, in the paper's words (section III Cells 4-6): draw random binary
+ * convolution kernels, push the (reduced) training set through 1..3 "convolution + max-pool"
+ * macro-layers with those fixed kernels, flatten, fit the only
+ * trainable layer -- the linear output layer "ELM0" -- by regularised least squares
+ * (PAPER.md:64-74), evaluate test accuracy and keep the best kernels.
+ *
+ * Conventions (all entry points)
+ *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch allocations); pointers
+ *     named h_* and all struct / out-parameter pointers are HOST pointers.  The library never
+ *     allocates, frees or retains device memory; scratch comes from the caller-provided workspace
+ *     (lbcnn_set_workspace).  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - Every call returns an int status (LBCNN_OK = 0 ...) and only ENQUEUES work on `stream`; it
+ *     never synchronises.  Numerical failure is not a status: a non-positive Cholesky pivot j
+ *     writes d_info[k] = j + 1 (LAPACK convention) for candidate k and the batch continues.
+ *   - Layouts: images uint8 NHWC "channels last"; kernel sets int8 with entries
+ *     -1/+1, per candidate the layers concatenated, layer l = [n_kernels][Cin_l][k][k]; bias int32
+ *     per candidate, layers concatenated, layer l = [Cout_l]; H = features, row-major
+ *     [candidate][sample][F] with the C,H,W flatten order f = (o*Hout + i)*Wout + j; W = output
+ *     weights row-major [candidate][F][n_classes]; labels int32 in [0, n_classes).
+ *   - H here is samples x features, the transpose of the listing's H (features x samples,
+ *     PAPER.md:66); the listing's H.H^T is H^T H here.
+ *   - There is no CPU fallback: without a CUDA device lbcnn_create fails with LBCNN_ERR_CUDA.
+ *     The shape helpers (lbcnn_feature_dim, lbcnn_kernel_set_size, lbcnn_status_string,
+ *     lbcnn_version) are host-only and need no device.
+ *   - Thread safety: one handle per host thread / stream.
+ */
+#ifndef LBCNN_H_
+#define LBCNN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  LBCNN_OK = 0,
+  LBCNN_ERR_INVALID_ARG = 1,  /* null pointer, n < 1, C <= 0, n_classes < 2, n_cand < 1 */
+  LBCNN_ERR_INVALID_ARCH = 2, /* a spatial size < 1, even kernel size, pooling window with no real cell, too large for one SM's shared memory */
+  LBCNN_ERR_SHAPE = 3,        /* F / channel mismatch */
+  LBCNN_ERR_WORKSPACE = 4,    /* workspace absent or too small (never a hidden allocation) */
+  LBCNN_ERR_CUDA = 5          /* no device / launch or driver error */
+};
+
+enum { LBCNN_CONV_FULL = 0, LBCNN_CONV_DEPTHWISE = 1 };
+enum { LBCNN_ACT_NONE = 0, LBCNN_ACT_RELU = 1 };
+
+/* flags of lbcnn_elm_fit */
+#define LBCNN_H_INTEGER 1u /* stored H values are integers with abs < 2^24 (the expander's output with feature_scale = 1) */
+#define LBCNN_FORCE_PRIMAL 2u /* testing: take the F x F branch whatever F and n are */
+#define LBCNN_FORCE_DUAL 4u   /* testing: take the n x n branch */
+
+/* One macro-layer "convolution -> (activation) -> max-pool" (listing lines 27-31).
+ * Convolution: cross-correlation, stride 1, zero padding (ksize-1)/2 (pad=1 for 3x3):
+ *   FULL:      z[y,x,o]     = b[o]     + sum_{c,dy,dx} w[o,c,dy,dx] * a[y+dy-p, x+dx-p, c]
+ *   DEPTHWISE: z[y,x,c*M+m] = b[c*M+m] + sum_{dy,dx}   w[m,c,dy,dx] * a[y+dy-p, x+dx-p, c]
+ * Pool: max over the in-image cells of window rows i*s-p .. i*s-p+k-1 (same for columns); padding never
+ * wins; output size floor((n+2p-k)/s)+1, or ceil(...)+1 with cover_all (PAPER.md:54
+ * max_pooling_2d(ksize=4, stride=str, pad=1, cover_all=True)). */
+typedef struct {
+  int32_t conv_type; /* LBCNN_CONV_FULL: n_kernels kernels of k x k x Cin; LBCNN_CONV_DEPTHWISE: multiplier M = n_kernels */
+  int32_t n_kernels;
+  int32_t ksize;     /* odd (3, 5, ...) */
+  int32_t act;       /* LBCNN_ACT_NONE = the paper ("Nonlinearity achieved in Max-pool") */
+  int32_t pool_k, pool_s, pool_p, pool_cover_all; /* (4,2,1,1) = paper; (2,2,0,0), (4,4,0,0) = BASELINE configs; (1,1,0,0) = none */
+} lbcnn_layer_t;
+
+typedef struct {
+  int32_t in_h, in_w, in_c;
+  int32_t n_layers; /* 1..3, "Up to three full convolution macro-layers" */
+  lbcnn_layer_t layer[3];
+  float feature_scale; /* multiplies the exact integer feature once on store; 1.0f keeps H integer-valued */
+} lbcnn_arch_t;
+
+typedef struct lbcnn_handle_s* lbcnn_handle_t;
+
+const char* lbcnn_version(void);
+const char* lbcnn_status_string(int status);
+
+/* Create / destroy a handle bound to CUDA device `device`.  Fails with LBCNN_ERR_CUDA when no
+ * such device exists (there is no CPU path). */
+int lbcnn_create(lbcnn_handle_t* h, int device);
+int lbcnn_destroy(lbcnn_handle_t h);
+
+/* Host-only shape arithmetic ("feature vector with size 15680"; Tables II-V).
+ * F = Cout_last * Hout * Wout; out_hwc = {Hout, Wout, Cout} of the last layer (may be NULL). */
+int lbcnn_feature_dim(const lbcnn_arch_t* arch, int64_t* F, int32_t out_hwc[3]);
+/* Number of int8 weights and int32 biases in ONE candidate kernel set. */
+int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t* n_bias);
+
+/* Workspace.  lbcnn_workspace_bytes gives the size with which lbcnn_search_candidates processes
+ * min(n_cand, as many candidates as fit in `budget_bytes`) candidates per chunk (budget 0 = no cap)
+ * -- and which is also enough for lbcnn_elm_fit on n_train samples and n_cand candidates.
+ * min_bytes (may be NULL) = the size for one candidate per chunk.  The workspace stays owned by the
+ * caller and must outlive every call enqueued with it. */
+int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
+                          int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes);
+int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
+
+/* Expander: d_H[k][i][:] = feature_scale * flatten(layers(image i; kernel set k)).
+ * The integer feature is exact (signed adds of uint8 pixels, abs < 2^24); the only rounding is the
+ * one fp32 multiply by feature_scale.  d_bias may be NULL (= 0).  Needs no workspace. */
+int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_images /*[n][H][W][C]*/, int64_t n,
+                 const int8_t* d_kernels /*[n_cand][n_weights]*/, const int32_t* d_bias /*[n_cand][n_bias] or NULL*/,
+                 int32_t n_cand, float* d_H /*[n_cand][n][F]*/, void* stream);
+
+/* ELM0 fit: W = argmin ||h_scale*H W - T||^2 + ||W||^2 / C with T the one-hot
+ * ("categorical") coding of the labels, i.e.
+ *   F <  n ("LLL"):  W = solve(I/C + H^T H, H^T T)
+ *   F >= n ("MMM"):  W = H^T solve(I/C + H H^T, T)
+ * on the logical features h_scale * d_H.  The Gram matrix is accumulated in fp64 (exact for
+ * LBCNN_H_INTEGER data), the system is solved by a blocked fp64 Cholesky (no pivoting, no jitter)
+ * and W is rounded once to fp32.  Needs the workspace.  d_info[k] = 0 or failing pivot + 1. */
+int lbcnn_elm_fit(lbcnn_handle_t h, const float* d_H /*[n_cand][n][F]*/, int64_t n, int64_t F, float h_scale,
+                  uint32_t flags, const int32_t* d_labels /*[n]*/, int32_t n_classes, float C, int32_t n_cand,
+                  float* d_W /*[n_cand][F][n_classes]*/, int32_t* d_info /*[n_cand]*/, void* stream);
+
+/* Score ("applied the feature vector directly to the Adaline output layer"; accuracy =
+ * "fraction of correctly recognized samples in a test set"):
+ *   logits = h_scale * d_H[k] . d_W[k];  pred = FIRST index of the maximum;  correct = #(pred == label).
+ * d_labels, d_pred, d_correct may each be NULL.  Needs no workspace. */
+int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H /*[n_cand][n][F]*/, int64_t n, int64_t F, float h_scale,
+                    const float* d_W /*[n_cand][F][n_classes]*/, int32_t n_classes, const int32_t* d_labels /*[n] or NULL*/,
+                    int32_t n_cand, int32_t* d_pred /*[n_cand][n] or NULL*/, int32_t* d_correct /*[n_cand] or NULL*/,
+                    void* stream);
+
+/* The search loop (one trial per candidate kernel set, keep best and lowest):
+ * for every candidate k: expand train and test, fit on train, score on test;
+ *   d_acc[k] = correct / n_test, or -1 when the fit failed (d_info[k] != 0);
+ *   d_best[0] = first k attaining the maximum accuracy, d_best[1] = first k attaining the minimum
+ *   among candidates whose fit succeeded (all failed: 0, 0);
+ *   d_W_best (may be NULL) = W of candidate d_best[0], acting on arch->feature_scale * integer features.
+ * Candidates are processed in chunks sized by the workspace; nothing crosses to the host. */
+int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch,
+                            const uint8_t* d_train, const int32_t* d_train_labels, int64_t n_train,
+                            const uint8_t* d_test, const int32_t* d_test_labels, int64_t n_test,
+                            int32_t n_classes, float C,
+                            const int8_t* d_kernels, const int32_t* d_bias /*or NULL*/, int32_t n_cand,
+                            float* d_acc /*[n_cand]*/, int32_t* d_correct /*[n_cand]*/, int32_t* d_info /*[n_cand]*/,
+                            int32_t* d_best /*[2]*/, float* d_W_best /*[F][n_classes] or NULL*/, void* stream);
+
+/* Number of kernel launches the library has enqueued through this handle since creation (for
+ * bench.py's gpu_launches claim). */
+int lbcnn_launch_count(lbcnn_handle_t h, int64_t* count);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBCNN_H_ */

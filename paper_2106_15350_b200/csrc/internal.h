@@ -1,0 +1,65 @@
+// internal.h -- declarations shared by the translation units of liblbcnn (CUDA path only;
+// nothing here is used by, or shared with, oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/lbcnn.h"
+
+struct lbcnn_handle_s {
+  int device;
+  int n_sm;
+  int max_smem_optin;  // bytes of dynamic shared memory one CTA may opt in to
+  void* ws;
+  size_t ws_bytes;
+  int64_t launches;
+};
+
+#define LB_CUDA_OK(expr)                                  \
+  do {                                                    \
+    cudaError_t e__ = (expr);                             \
+    if (e__ != cudaSuccess) return LBCNN_ERR_CUDA;        \
+  } while (0)
+
+static inline int64_t lb_align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+// ---- host shape logic (api.cu) -------------------------------------------------------------
+struct LayerShape {
+  int conv_type, nk, k, act, pk, ps, pp, cover;
+  int cin, cout, hin, win, hout, wout;
+  int64_t w_off, b_off;   // offsets of this layer inside one candidate's kernel set / bias set
+};
+struct ArchShape {
+  int n_layers;
+  LayerShape L[3];
+  int64_t F, n_weights, n_bias;
+  int64_t max_abs;        // bound on |integer feature| (255 * prod k^2 Cin), saturated at 2^62
+};
+int lb_pool_out(int n, int k, int s, int p, int cover_all);
+int lb_arch_shape(const lbcnn_arch_t* a, ArchShape* s);
+
+// ---- expander (expand.cu) ------------------------------------------------------------------
+int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
+                     const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, cudaStream_t st);
+
+// ---- fit (fit.cu) --------------------------------------------------------------------------
+struct FitPlan {
+  int primal;            // 1: F x F system, 0: n x n system
+  int64_t dim;           // system dimension
+  int64_t rows;          // dim + n_classes (right-hand sides appended as rows)
+  size_t a_bytes;        // per candidate: rows * dim doubles
+  size_t perm_off, off_off, a_off, total; // offsets inside the fit workspace
+};
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p);
+int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_H, int64_t n, int64_t F, float h_scale,
+                  const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
+                  cudaStream_t st);
+
+// ---- score (score.cu) ----------------------------------------------------------------------
+int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
+                    int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
+                    cudaStream_t st);
+int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
+int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
+                     float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,
+                     cudaStream_t st);
