@@ -1,0 +1,356 @@
+// fit.cu -- ELM0 fit: Gram + ridge (F1), right-hand side (F2), SPD solve (F3).
+//
+// System solved per candidate, on the STORED features U (logical feature = s*U, s = h_scale):
+//   primal (F < n):  (U^T U + lam I) W' = U^T T,        W = W'/s
+//   dual  (F >= n):  (U U^T + lam I) Z  = T,  W' = U^T Z, W = W'/s        lam = 1/(C s^2)
+// which is the paper's (H^T H + I/C) W = H^T T with H = s*U divided through by s^2.
+// Storage: per candidate a (dim + c) x dim fp64 matrix, row-major, leading dimension dim: the lower
+// triangle of rows 0..dim-1 holds the system matrix, rows dim..dim+c-1 hold the right-hand sides
+// TRANSPOSED (row = class).  A right-looking blocked Cholesky over all dim + c rows then leaves
+// L in the triangle and Y^T = (L^-1 B)^T in the appended rows (forward substitution for free);
+// a blocked backward sweep turns Y^T into X^T.
+#include "internal.h"
+#include "gemm64.cuh"
+
+namespace {
+
+constexpr int NB = 64;   // Cholesky block size
+
+// ---------------------------------------------------------------------------------------------
+// generic batched GEMM, fp64 accumulate:  C[i][j] (+)= alpha * sum_k A(i,k) B(j,k) (+ diag on i == j)
+struct GemmP {
+  const void* A; long long sAr, sAk, bA;
+  const void* B; long long sBr, sBk, bB;
+  void* C; long long ldc, bC;
+  int M, N, K;
+  double alpha; int accumulate; int lower; double diag;
+};
+
+template <typename TA, typename TB, typename TC, bool AK, bool BK>
+__global__ void __launch_bounds__(g64::NT) gemm_kernel(const GemmP p) {
+  const int ti = blockIdx.y, tj = blockIdx.x;
+  if (p.lower && tj > ti) return;
+  __shared__ g64::Smem sm;
+  const long long z = blockIdx.z;
+  const TA* A = reinterpret_cast<const TA*>(p.A) + z * p.bA;
+  const TB* B = reinterpret_cast<const TB*>(p.B) + z * p.bB;
+  TC* C = reinterpret_cast<TC*>(p.C) + z * p.bC;
+  double acc[4][4];
+  g64::tile_mma<TA, TB, AK, BK>(sm, A, p.sAr, p.sAk, ti * 64, p.M, B, p.sBr, p.sBk, tj * 64, p.N, p.K, acc);
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    const int i = ti * 64 + ty + 16 * a;
+    if (i >= p.M) continue;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int j = tj * 64 + tx + 16 * b;
+      if (j >= p.N) continue;
+      double v = p.alpha * acc[a][b];
+      if (i == j) v += p.diag;
+      TC* c = C + (long long)i * p.ldc + j;
+      if (p.accumulate) v += (double)*c;
+      *c = (TC)v;
+    }
+  }
+}
+
+template <typename TA, typename TB, typename TC, bool AK, bool BK>
+int launch_gemm(lbcnn_handle_s* h, const GemmP& p, int batch, cudaStream_t st) {
+  if (p.M <= 0 || p.N <= 0 || batch <= 0) return LBCNN_OK;
+  dim3 grid((p.N + 63) / 64, (p.M + 63) / 64, batch);
+  gemm_kernel<TA, TB, TC, AK, BK><<<grid, g64::NT, 0, st>>>(p);
+  h->launches += 1;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// labels -> stable class-sorted sample permutation (one thread per class; deterministic)
+__global__ void label_perm_kernel(const int32_t* __restrict__ y, int n, int c, int32_t* __restrict__ perm,
+                                  int32_t* __restrict__ off) {
+  extern __shared__ int cnt[];
+  for (int t = threadIdx.x; t <= c; t += blockDim.x) cnt[t] = 0;
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += blockDim.x) atomicAdd(&cnt[y[i] + 1], 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int t = 1; t <= c; ++t) cnt[t] += cnt[t - 1];
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t <= c; t += blockDim.x) off[t] = cnt[t];
+  for (int cls = threadIdx.x; cls < c; cls += blockDim.x) {
+    int w = cnt[cls];
+    for (int i = 0; i < n; ++i)
+      if (y[i] == cls) perm[w++] = i;
+  }
+}
+
+// primal right-hand side (F2): Bt[cls][f] = sum_{n: y_n = cls} U[n][f]  (T one-hot)
+__global__ void __launch_bounds__(128) rhs_primal_kernel(const float* __restrict__ U, long long n, long long F,
+                                                         const int32_t* __restrict__ perm,
+                                                         const int32_t* __restrict__ off, double* __restrict__ A,
+                                                         long long a_stride, long long dim) {
+  const long long f = (long long)blockIdx.x * 128 + threadIdx.x;
+  const int cls = blockIdx.y;
+  const long long z = blockIdx.z;
+  if (f >= F) return;
+  const float* Uz = U + z * n * F + f;
+  const int lo = off[cls], hi = off[cls + 1];
+  double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+  int i = lo;
+  for (; i + 3 < hi; i += 4) {
+    const float v0 = Uz[(long long)perm[i] * F], v1 = Uz[(long long)perm[i + 1] * F];
+    const float v2 = Uz[(long long)perm[i + 2] * F], v3 = Uz[(long long)perm[i + 3] * F];
+    s0 += v0; s1 += v1; s2 += v2; s3 += v3;
+  }
+  for (; i < hi; ++i) s0 += Uz[(long long)perm[i] * F];
+  A[z * a_stride + (dim + cls) * dim + f] = (s0 + s1) + (s2 + s3);
+}
+
+// dual right-hand side: rows dim.. = T^T (c x n one-hot)
+__global__ void rhs_dual_kernel(const int32_t* __restrict__ y, long long n, int c, double* __restrict__ A,
+                                long long a_stride) {
+  const long long z = blockIdx.z;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n * c) return;
+  const int cls = (int)(t / n);
+  const long long i = t % n;
+  A[z * a_stride + (n + cls) * n + i] = (y[i] == cls) ? 1.0 : 0.0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// blocked Cholesky pieces (F3).  Matrix of candidate z at A + z*a_stride, leading dimension ld = dim.
+
+// factorise the nbj x nbj diagonal block at (j0, j0); a non-positive pivot records info = index + 1
+// (first failure wins) and continues with pivot 1 so that the candidate's data stays finite.
+__global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A, long long a_stride, long long ld,
+                                                         int j0, int nbj, int32_t* __restrict__ info) {
+  __shared__ double S[NB][NB + 1];
+  double* Az = A + blockIdx.x * a_stride + (long long)j0 * ld + j0;
+  for (int e = threadIdx.x; e < nbj * nbj; e += blockDim.x) {
+    const int i = e / nbj, c = e % nbj;
+    S[i][c] = (c <= i) ? Az[(long long)i * ld + c] : 0.0;
+  }
+  for (int j = 0; j < nbj; ++j) {
+    __syncthreads();
+    double piv = S[j][j];
+    if (!(piv > 0.0)) {
+      if (threadIdx.x == 0 && info[blockIdx.x] == 0) info[blockIdx.x] = j0 + j + 1;
+      piv = 1.0;
+    }
+    const double l = sqrt(piv);
+    const double inv = 1.0 / l;
+    __syncthreads();
+    for (int i = j + 1 + threadIdx.x; i < nbj; i += blockDim.x) S[i][j] *= inv;
+    if (threadIdx.x == 0) S[j][j] = l;
+    __syncthreads();
+    const int rem = nbj - j - 1;
+    for (int e = threadIdx.x; e < rem * rem; e += blockDim.x) {
+      const int i = j + 1 + e / rem, c = j + 1 + e % rem;
+      if (c <= i) S[i][c] -= S[i][j] * S[c][j];
+    }
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < nbj * nbj; e += blockDim.x) {
+    const int i = e / nbj, c = e % nbj;
+    if (c <= i) Az[(long long)i * ld + c] = S[i][c];
+  }
+}
+
+// rows below the diagonal block (including the appended right-hand-side rows): X = A21 * L11^-T.
+// One thread per row, the row and L11 in shared memory.
+__global__ void __launch_bounds__(64) trsm_panel_kernel(double* __restrict__ A, long long a_stride, long long ld,
+                                                        int j0, int nbj, long long rows) {
+  extern __shared__ double sh[];
+  double (*Ls)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh);
+  double (*Rs)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh + NB * (NB + 1));
+  double* Az = A + blockIdx.y * a_stride;
+  const double* L11 = Az + (long long)j0 * ld + j0;
+  const long long r0 = (long long)j0 + nbj + (long long)blockIdx.x * 64;
+  const int t = threadIdx.x;
+  for (int i = 0; i < nbj; ++i)
+    if (t < nbj) Ls[i][t] = L11[(long long)i * ld + t];
+  const int nr = (int)min((long long)64, rows - r0);
+  for (int i = 0; i < nr; ++i)
+    if (t < nbj) Rs[i][t] = Az[(r0 + i) * ld + j0 + t];
+  __syncthreads();
+  if (t < nr) {
+    for (int c = 0; c < nbj; ++c) {
+      const double x = Rs[t][c] / Ls[c][c];
+      Rs[t][c] = x;
+      for (int c2 = c + 1; c2 < nbj; ++c2) Rs[t][c2] -= x * Ls[c2][c];
+    }
+  }
+  __syncthreads();
+  for (int i = 0; i < nr; ++i)
+    if (t < nbj) Az[(r0 + i) * ld + j0 + t] = Rs[i][t];
+}
+
+// backward sweep, diagonal step: rows of Y^T (one per class) x * L_jj = y, solved from the last column.
+__global__ void __launch_bounds__(64) bs_diag_kernel(double* __restrict__ A, long long a_stride, long long ld,
+                                                     long long dim, int j0, int nbj, int c) {
+  extern __shared__ double sh[];
+  double (*Ls)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh);
+  double (*Rs)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh + NB * (NB + 1));
+  double* Az = A + blockIdx.y * a_stride;
+  const double* L11 = Az + (long long)j0 * ld + j0;
+  const int r0 = blockIdx.x * 64;
+  const int t = threadIdx.x;
+  for (int i = 0; i < nbj; ++i)
+    if (t < nbj) Ls[i][t] = (t <= i) ? L11[(long long)i * ld + t] : 0.0;
+  const int nr = min(64, c - r0);
+  for (int i = 0; i < nr; ++i)
+    if (t < nbj) Rs[i][t] = Az[(dim + r0 + i) * ld + j0 + t];
+  __syncthreads();
+  if (t < nr) {
+    for (int cc = nbj - 1; cc >= 0; --cc) {
+      const double x = Rs[t][cc] / Ls[cc][cc];
+      Rs[t][cc] = x;
+      for (int c2 = 0; c2 < cc; ++c2) Rs[t][c2] -= x * Ls[cc][c2];
+    }
+  }
+  __syncthreads();
+  for (int i = 0; i < nr; ++i)
+    if (t < nbj) Az[(dim + r0 + i) * ld + j0 + t] = Rs[i][t];
+}
+
+// primal: W[f][cls] = X^T[cls][f] / s, rounded once to fp32
+__global__ void w_from_xt_kernel(const double* __restrict__ A, long long a_stride, long long dim, int c, double inv_s,
+                                 float* __restrict__ W) {
+  const long long z = blockIdx.z;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= dim * c) return;
+  const long long f = t / c;
+  const int cls = (int)(t % c);
+  W[z * dim * c + t] = (float)(A[z * a_stride + (dim + cls) * dim + f] * inv_s);
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p) {
+  int primal = (F < n) ? 1 : 0;                       // PAPER.md:68 `if n_inputs<Ntr` ('LLL'), else 'MMM'
+  if (flags & LBCNN_FORCE_PRIMAL) primal = 1;
+  if (flags & LBCNN_FORCE_DUAL) primal = 0;
+  p->primal = primal;
+  p->dim = primal ? F : n;
+  p->rows = p->dim + n_classes;
+  p->a_bytes = (size_t)p->rows * (size_t)p->dim * sizeof(double);
+  size_t off = 0;
+  p->perm_off = off; off += (size_t)lb_align_up(n * 4, 256);
+  p->off_off = off;  off += (size_t)lb_align_up(((int64_t)n_classes + 1) * 4, 256);
+  p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
+  p->total = off;
+}
+
+int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d_H, int64_t n, int64_t F, float h_scale,
+                  const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
+                  cudaStream_t st) {
+  char* base = reinterpret_cast<char*>(ws);
+  int32_t* perm = reinterpret_cast<int32_t*>(base + pl.perm_off);
+  int32_t* off = reinterpret_cast<int32_t*>(base + pl.off_off);
+  double* A = reinterpret_cast<double*>(base + pl.a_off);
+  const long long dim = pl.dim, rows = pl.rows, ld = pl.dim;
+  const long long a_stride = rows * dim;
+  const double s = (double)h_scale;
+  const double lam = 1.0 / ((double)C * s * s);
+  const int c = n_classes;
+  int rc;
+
+  rc = lb_launch_zero_i32(h, d_info, n_cand, st);
+  if (rc) return rc;
+
+  if (pl.primal) {
+    // F1: A = U^T U + lam I (lower tiles), operands read with k = sample (slow) and i = feature (contiguous)
+    GemmP g{};
+    g.A = d_H; g.sAr = 1; g.sAk = F; g.bA = n * F;
+    g.B = d_H; g.sBr = 1; g.sBk = F; g.bB = n * F;
+    g.C = A; g.ldc = ld; g.bC = a_stride;
+    g.M = (int)F; g.N = (int)F; g.K = (int)n; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
+    rc = launch_gemm<float, float, double, false, false>(h, g, n_cand, st);
+    if (rc) return rc;
+    // F2: appended rows = (U^T T)^T
+    label_perm_kernel<<<1, 1024, (c + 1) * sizeof(int), st>>>(d_labels, (int)n, c, perm, off);
+    h->launches += 1;
+    dim3 gr((unsigned)((F + 127) / 128), (unsigned)c, (unsigned)n_cand);
+    rhs_primal_kernel<<<gr, 128, 0, st>>>(d_H, n, F, perm, off, A, a_stride, dim);
+    h->launches += 1;
+  } else {
+    GemmP g{};
+    g.A = d_H; g.sAr = F; g.sAk = 1; g.bA = n * F;
+    g.B = d_H; g.sBr = F; g.sBk = 1; g.bB = n * F;
+    g.C = A; g.ldc = ld; g.bC = a_stride;
+    g.M = (int)n; g.N = (int)n; g.K = (int)F; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
+    rc = launch_gemm<float, float, double, true, true>(h, g, n_cand, st);
+    if (rc) return rc;
+    dim3 gr((unsigned)((n * c + 255) / 256), 1, (unsigned)n_cand);
+    rhs_dual_kernel<<<gr, 256, 0, st>>>(d_labels, n, c, A, a_stride);
+    h->launches += 1;
+  }
+  LB_CUDA_OK(cudaGetLastError());
+
+  const size_t tr_smem = 2 * NB * (NB + 1) * sizeof(double);
+  LB_CUDA_OK(cudaFuncSetAttribute(trsm_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));
+  LB_CUDA_OK(cudaFuncSetAttribute(bs_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));
+
+  // F3: right-looking blocked Cholesky over dim + c rows
+  for (long long j0 = 0; j0 < dim; j0 += NB) {
+    const int nbj = (int)((dim - j0 < NB) ? dim - j0 : NB);
+    potrf_diag_kernel<<<n_cand, 256, 0, st>>>(A, a_stride, ld, (int)j0, nbj, d_info);
+    h->launches += 1;
+    const long long below = rows - (j0 + nbj);
+    if (below > 0) {
+      dim3 gt((unsigned)((below + 63) / 64), (unsigned)n_cand);
+      trsm_panel_kernel<<<gt, 64, tr_smem, st>>>(A, a_stride, ld, (int)j0, nbj, rows);
+      h->launches += 1;
+      const long long j1 = j0 + nbj;
+      if (dim - j1 > 0) {
+        GemmP g{};
+        g.A = A + j1 * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
+        g.B = A + j1 * ld + j0; g.sBr = ld; g.sBk = 1; g.bB = a_stride;
+        g.C = A + j1 * ld + j1; g.ldc = ld; g.bC = a_stride;
+        g.M = (int)(rows - j1); g.N = (int)(dim - j1); g.K = nbj; g.alpha = -1.0; g.accumulate = 1; g.lower = 1;
+        g.diag = 0.0;
+        rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
+        if (rc) return rc;
+      }
+    }
+  }
+  // backward sweep on the appended rows: X^T L = Y^T, block columns from the last to the first
+  const long long nblk = (dim + NB - 1) / NB;
+  for (long long jb = nblk - 1; jb >= 0; --jb) {
+    const long long j0 = jb * NB;
+    const int nbj = (int)((dim - j0 < NB) ? dim - j0 : NB);
+    dim3 gd((unsigned)((c + 63) / 64), (unsigned)n_cand);
+    bs_diag_kernel<<<gd, 64, tr_smem, st>>>(A, a_stride, ld, dim, (int)j0, nbj, c);
+    h->launches += 1;
+    if (j0 > 0) {
+      GemmP g{};
+      g.A = A + dim * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;      // X^T[:, block]  (c x nbj)
+      g.B = A + j0 * ld; g.sBr = 1; g.sBk = ld; g.bB = a_stride;            // L[block, 0:j0] as (j, k)
+      g.C = A + dim * ld; g.ldc = ld; g.bC = a_stride;
+      g.M = c; g.N = (int)j0; g.K = nbj; g.alpha = -1.0; g.accumulate = 1; g.lower = 0; g.diag = 0.0;
+      rc = launch_gemm<double, double, double, true, false>(h, g, n_cand, st);
+      if (rc) return rc;
+    }
+  }
+  LB_CUDA_OK(cudaGetLastError());
+
+  if (pl.primal) {
+    dim3 gw((unsigned)((dim * c + 255) / 256), 1, (unsigned)n_cand);
+    w_from_xt_kernel<<<gw, 256, 0, st>>>(A, a_stride, dim, c, 1.0 / s, d_W);
+    h->launches += 1;
+  } else {
+    // W[f][cls] = (1/s) sum_n U[n][f] Z^T[cls][n]
+    GemmP g{};
+    g.A = d_H; g.sAr = 1; g.sAk = F; g.bA = n * F;
+    g.B = A + dim * ld; g.sBr = ld; g.sBk = 1; g.bB = a_stride;
+    g.C = d_W; g.ldc = c; g.bC = F * c;
+    g.M = (int)F; g.N = c; g.K = (int)n; g.alpha = 1.0 / s; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
+    rc = launch_gemm<float, double, float, false, true>(h, g, n_cand, st);
+    if (rc) return rc;
+  }
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}
