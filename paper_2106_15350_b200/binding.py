@@ -1,0 +1,232 @@
+"""Thin Python binding of liblbcnn.so (include/lbcnn.h): argument marshalling only.
+
+Every step of the path runs in the CUDA library; torch supplies device memory and the current stream.
+There is no CPU fallback: a missing library raises at import of the symbols, and a missing CUDA device
+makes ``Handle()`` raise ``LbcnnError(LBCNN_ERR_CUDA)``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence, Tuple
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "liblbcnn.so")
+
+OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA = range(6)
+CONV_FULL, CONV_DEPTHWISE = 0, 1
+ACT_NONE, ACT_RELU = 0, 1
+H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
+
+EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
+           "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
+           "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_launch_count")
+
+
+class Layer(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("conv_type", "n_kernels", "ksize", "act", "pool_k", "pool_s", "pool_p", "pool_cover_all")]
+
+
+class Arch(C.Structure):
+    _fields_ = [("in_h", C.c_int32), ("in_w", C.c_int32), ("in_c", C.c_int32), ("n_layers", C.c_int32),
+                ("layer", Layer * 3), ("feature_scale", C.c_float)]
+
+
+class LbcnnError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s: status %d (%s)" % (where, status, status_string(status)))
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load liblbcnn.so (built in-tree by paper_2106_15350_b200.build).  Fails loudly when it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("liblbcnn.so is not built: run `python -m paper_2106_15350_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.lbcnn_version.restype = C.c_char_p
+        L.lbcnn_status_string.restype = C.c_char_p
+        L.lbcnn_status_string.argtypes = [C.c_int]
+        for name in EXPORTS[2:]:
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def version() -> str:
+    return lib().lbcnn_version().decode()
+
+
+def status_string(status: int) -> str:
+    return lib().lbcnn_status_string(int(status)).decode()
+
+
+def _check(rc: int, where: str):
+    if rc != OK:
+        raise LbcnnError(rc, where)
+
+
+def make_arch(in_h: int, in_w: int, in_c: int, layers: Sequence, feature_scale: float = 1.0) -> Arch:
+    """layers: objects or tuples (conv_type, n_kernels, ksize, act, pool_k, pool_s, pool_p, pool_cover_all)."""
+    a = Arch()
+    a.in_h, a.in_w, a.in_c, a.n_layers = int(in_h), int(in_w), int(in_c), len(layers)
+    a.feature_scale = float(feature_scale)
+    if len(layers) > 3:
+        raise LbcnnError(ERR_INVALID_ARCH, "make_arch")
+    for i, L in enumerate(layers):
+        t = tuple(L) if isinstance(L, (tuple, list)) else (
+            L.conv_type, L.n_kernels, L.ksize, L.act, L.pool_k, L.pool_s, L.pool_p, L.pool_cover_all)
+        for (name, _), v in zip(Layer._fields_, t):
+            setattr(a.layer[i], name, int(v))
+    return a
+
+
+def arch_of(workload, feature_scale: Optional[float] = None) -> Arch:
+    """Arch of a synth.Workload (plain data; synth.py holds no arithmetic of the method)."""
+    fs = workload.feature_scale if feature_scale is None else feature_scale
+    return make_arch(workload.in_h, workload.in_w, workload.in_c, workload.layers, fs)
+
+
+def feature_dim(arch: Arch) -> Tuple[int, Tuple[int, int, int]]:
+    F = C.c_int64()
+    hwc = (C.c_int32 * 3)()
+    _check(lib().lbcnn_feature_dim(C.byref(arch), C.byref(F), hwc), "lbcnn_feature_dim")
+    return F.value, tuple(hwc)
+
+
+def kernel_set_size(arch: Arch) -> Tuple[int, int]:
+    nw, nb = C.c_int64(), C.c_int64()
+    _check(lib().lbcnn_kernel_set_size(C.byref(arch), C.byref(nw), C.byref(nb)), "lbcnn_kernel_set_size")
+    return nw.value, nb.value
+
+
+def workspace_bytes(arch: Arch, n_train: int, n_test: int, n_classes: int, n_cand: int, budget_bytes: int = 0,
+                    handle: "Optional[Handle]" = None) -> Tuple[int, int]:
+    b, m = C.c_size_t(), C.c_size_t()
+    h = handle._h if handle is not None else C.c_void_p(None)
+    _check(lib().lbcnn_workspace_bytes(h, C.byref(arch), C.c_int64(n_train), C.c_int64(n_test), C.c_int32(n_classes),
+                                       C.c_int32(n_cand), C.c_size_t(budget_bytes), C.byref(b), C.byref(m)),
+           "lbcnn_workspace_bytes")
+    return b.value, m.value
+
+
+def _ptr(t, dtype=None, allow_none: bool = False):
+    """device pointer of a contiguous CUDA torch tensor (or NULL)."""
+    if t is None:
+        if allow_none:
+            return C.c_void_p(None)
+        raise LbcnnError(ERR_INVALID_ARG, "null tensor")
+    if not t.is_cuda or not t.is_contiguous() or (dtype is not None and t.dtype != dtype):
+        raise LbcnnError(ERR_INVALID_ARG, "tensor must be a contiguous CUDA tensor of dtype %s" % dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Handle:
+    """lbcnn_handle_t plus a caller-owned torch workspace buffer."""
+
+    def __init__(self, device: int = 0):
+        self._h = C.c_void_p(None)
+        _check(lib().lbcnn_create(C.byref(self._h), int(device)), "lbcnn_create")
+        self.device = int(device)
+        self._ws = None
+
+    def close(self):
+        if self._h:
+            lib().lbcnn_destroy(self._h)
+            self._h = C.c_void_p(None)
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_workspace(self, ws):
+        """ws: 1-D uint8 CUDA tensor (kept alive by the handle) or None."""
+        if ws is None:
+            _check(lib().lbcnn_set_workspace(self._h, C.c_void_p(None), C.c_size_t(0)), "lbcnn_set_workspace")
+        else:
+            _check(lib().lbcnn_set_workspace(self._h, _ptr(ws), C.c_size_t(ws.numel() * ws.element_size())),
+                   "lbcnn_set_workspace")
+        self._ws = ws
+
+    def ensure_workspace(self, nbytes: int):
+        import torch
+        if self._ws is None or self._ws.numel() < nbytes:
+            self._ws = None
+            self.set_workspace(torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % self.device))
+
+    def launch_count(self) -> int:
+        n = C.c_int64()
+        _check(lib().lbcnn_launch_count(self._h, C.byref(n)), "lbcnn_launch_count")
+        return n.value
+
+    # ---- the four calls of the path ----------------------------------------------------------
+    def expand(self, arch: Arch, images, kernels, bias=None, out=None):
+        """images u8 [n][H][W][C]; kernels i8 [K][n_weights]; returns H f32 [K][n][F]."""
+        import torch
+        F, _ = feature_dim(arch)
+        n, K = images.shape[0], kernels.shape[0]
+        if out is None:
+            out = torch.empty((K, n, F), dtype=torch.float32, device=images.device)
+        _check(lib().lbcnn_expand(self._h, C.byref(arch), _ptr(images, torch.uint8), C.c_int64(n),
+                                  _ptr(kernels, torch.int8), _ptr(bias, torch.int32, True), C.c_int32(K),
+                                  _ptr(out, torch.float32), _stream()), "lbcnn_expand")
+        return out
+
+    def elm_fit(self, H, labels, n_classes: int, Creg: float, h_scale: float = 1.0, flags: int = 0):
+        """H f32 [K][n][F]; returns (W f32 [K][F][c], info i32 [K])."""
+        import torch
+        K, n, F = H.shape
+        W = torch.empty((K, F, n_classes), dtype=torch.float32, device=H.device)
+        info = torch.empty((K,), dtype=torch.int32, device=H.device)
+        _check(lib().lbcnn_elm_fit(self._h, _ptr(H, torch.float32), C.c_int64(n), C.c_int64(F), C.c_float(h_scale),
+                                   C.c_uint32(flags), _ptr(labels, torch.int32), C.c_int32(n_classes), C.c_float(Creg),
+                                   C.c_int32(K), _ptr(W), _ptr(info), _stream()), "lbcnn_elm_fit")
+        return W, info
+
+    def elm_score(self, H, W, labels=None, h_scale: float = 1.0, want_pred: bool = True):
+        """returns (pred i32 [K][n] or None, correct i32 [K] or None)."""
+        import torch
+        K, n, F = H.shape
+        c = W.shape[2]
+        pred = torch.empty((K, n), dtype=torch.int32, device=H.device) if want_pred else None
+        corr = torch.empty((K,), dtype=torch.int32, device=H.device) if labels is not None else None
+        _check(lib().lbcnn_elm_score(self._h, _ptr(H, torch.float32), C.c_int64(n), C.c_int64(F), C.c_float(h_scale),
+                                     _ptr(W, torch.float32), C.c_int32(c), _ptr(labels, torch.int32, True), C.c_int32(K),
+                                     _ptr(pred, None, True), _ptr(corr, None, True), _stream()), "lbcnn_elm_score")
+        return pred, corr
+
+    def search_candidates(self, arch: Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: float, kernels,
+                          bias=None, want_W: bool = True, out=None):
+        """returns dict(acc f32 [K], correct i32 [K], info i32 [K], best i32 [2], W_best f32 [F][c] or None);
+        everything stays on the device."""
+        import torch
+        F, _ = feature_dim(arch)
+        K = kernels.shape[0]
+        dev = train_x.device
+        if out is None:
+            out = dict(acc=torch.empty(K, dtype=torch.float32, device=dev),
+                       correct=torch.empty(K, dtype=torch.int32, device=dev),
+                       info=torch.empty(K, dtype=torch.int32, device=dev),
+                       best=torch.empty(2, dtype=torch.int32, device=dev),
+                       W_best=torch.empty((F, n_classes), dtype=torch.float32, device=dev) if want_W else None)
+        _check(lib().lbcnn_search_candidates(
+            self._h, C.byref(arch), _ptr(train_x, torch.uint8), _ptr(train_y, torch.int32), C.c_int64(train_x.shape[0]),
+            _ptr(test_x, torch.uint8), _ptr(test_y, torch.int32), C.c_int64(test_x.shape[0]), C.c_int32(n_classes),
+            C.c_float(Creg), _ptr(kernels, torch.int8), _ptr(bias, torch.int32, True), C.c_int32(K),
+            _ptr(out["acc"]), _ptr(out["correct"]), _ptr(out["info"]), _ptr(out["best"]),
+            _ptr(out["W_best"], None, True), _stream()), "lbcnn_search_candidates")
+        return out

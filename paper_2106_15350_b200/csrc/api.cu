@@ -1,0 +1,262 @@
+// api.cu -- the C ABI of liblbcnn (include/lbcnn.h): argument checking, shape arithmetic, workspace
+// planning and the search driver.  All compute is in expand.cu / fit.cu / score.cu; there is no CPU path.
+#include "internal.h"
+#include <new>
+
+// ---- host shape logic -------------------------------------------------------------------------
+// pooling output size (PAPER.md:54 max_pooling_2d(ksize, stride, pad, cover_all=True); PAPER.md:104 28->14->7)
+int lb_pool_out(int n, int k, int s, int p, int cover_all) {
+  if (n < 1 || k < 1 || s < 1 || p < 0) return -1;
+  const int span = n + 2 * p - k;
+  if (span < 0) return -1;
+  const int out = (cover_all ? (span + s - 1) / s : span / s) + 1;
+  // first and last windows must hold a real cell (windows in between then do as well when s <= k; check all)
+  for (int i = 0; i < out; ++i) {
+    int lo = i * s - p, hi = lo + k;
+    if (lo < 0) lo = 0;
+    if (hi > n) hi = n;
+    if (hi <= lo) return -1;
+  }
+  return out;
+}
+
+int lb_arch_shape(const lbcnn_arch_t* a, ArchShape* s) {
+  if (!a || !s) return LBCNN_ERR_INVALID_ARG;
+  if (a->n_layers < 1 || a->n_layers > 3 || a->in_h < 1 || a->in_w < 1 || a->in_c < 1) return LBCNN_ERR_INVALID_ARCH;
+  int h = a->in_h, w = a->in_w, c = a->in_c;
+  int64_t w_off = 0, b_off = 0;
+  long double bound = 255.0L;
+  s->n_layers = a->n_layers;
+  for (int l = 0; l < a->n_layers; ++l) {
+    const lbcnn_layer_t& A = a->layer[l];
+    LayerShape& L = s->L[l];
+    if (A.n_kernels < 1 || A.ksize < 1 || (A.ksize % 2) == 0) return LBCNN_ERR_INVALID_ARCH;
+    if (A.conv_type != LBCNN_CONV_FULL && A.conv_type != LBCNN_CONV_DEPTHWISE) return LBCNN_ERR_INVALID_ARCH;
+    if (A.act != LBCNN_ACT_NONE && A.act != LBCNN_ACT_RELU) return LBCNN_ERR_INVALID_ARCH;
+    L.conv_type = A.conv_type; L.nk = A.n_kernels; L.k = A.ksize; L.act = A.act;
+    L.pk = A.pool_k; L.ps = A.pool_s; L.pp = A.pool_p; L.cover = A.pool_cover_all;
+    L.cin = c; L.hin = h; L.win = w;
+    L.cout = (A.conv_type == LBCNN_CONV_FULL) ? A.n_kernels : c * A.n_kernels;
+    L.hout = lb_pool_out(h, A.pool_k, A.pool_s, A.pool_p, A.pool_cover_all);
+    L.wout = lb_pool_out(w, A.pool_k, A.pool_s, A.pool_p, A.pool_cover_all);
+    if (L.hout < 1 || L.wout < 1) return LBCNN_ERR_INVALID_ARCH;
+    L.w_off = w_off; L.b_off = b_off;
+    w_off += (int64_t)A.n_kernels * c * A.ksize * A.ksize;
+    b_off += L.cout;
+    bound *= (long double)A.ksize * A.ksize * (A.conv_type == LBCNN_CONV_FULL ? c : 1);
+    h = L.hout; w = L.wout; c = L.cout;
+  }
+  s->F = (int64_t)c * h * w;
+  s->n_weights = w_off; s->n_bias = b_off;
+  s->max_abs = bound > 4.0e18L ? (int64_t)4000000000000000000LL : (int64_t)bound;
+  return LBCNN_OK;
+}
+
+// ---- plain entry points -------------------------------------------------------------------------
+extern "C" {
+
+const char* lbcnn_version(void) { return "lbcnn-b200 0.1 (sm_100a)"; }
+
+const char* lbcnn_status_string(int status) {
+  switch (status) {
+    case LBCNN_OK: return "ok";
+    case LBCNN_ERR_INVALID_ARG: return "invalid argument";
+    case LBCNN_ERR_INVALID_ARCH: return "invalid architecture";
+    case LBCNN_ERR_SHAPE: return "shape mismatch";
+    case LBCNN_ERR_WORKSPACE: return "workspace absent or too small";
+    case LBCNN_ERR_CUDA: return "CUDA error (no device, launch or driver failure)";
+    default: return "unknown status";
+  }
+}
+
+int lbcnn_create(lbcnn_handle_t* h, int device) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  *h = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return LBCNN_ERR_CUDA;
+  LB_CUDA_OK(cudaSetDevice(device));
+  lbcnn_handle_s* p = new (std::nothrow) lbcnn_handle_s();
+  if (!p) return LBCNN_ERR_INVALID_ARG;
+  p->device = device;
+  LB_CUDA_OK(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device));
+  LB_CUDA_OK(cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
+  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0;
+  *h = p;
+  return LBCNN_OK;
+}
+
+int lbcnn_destroy(lbcnn_handle_t h) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  delete h;
+  return LBCNN_OK;
+}
+
+int lbcnn_feature_dim(const lbcnn_arch_t* arch, int64_t* F, int32_t out_hwc[3]) {
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  if (F) *F = s.F;
+  if (out_hwc) {
+    const LayerShape& L = s.L[s.n_layers - 1];
+    out_hwc[0] = L.hout; out_hwc[1] = L.wout; out_hwc[2] = L.cout;
+  }
+  return LBCNN_OK;
+}
+
+int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t* n_bias) {
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  if (n_weights) *n_weights = s.n_weights;
+  if (n_bias) *n_bias = s.n_bias;
+  return LBCNN_OK;
+}
+
+int lbcnn_launch_count(lbcnn_handle_t h, int64_t* count) {
+  if (!h || !count) return LBCNN_ERR_INVALID_ARG;
+  *count = h->launches;
+  return LBCNN_OK;
+}
+
+int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  if ((d_ws == nullptr) != (bytes == 0)) return LBCNN_ERR_INVALID_ARG;
+  if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0) return LBCNN_ERR_INVALID_ARG;
+  h->ws = d_ws; h->ws_bytes = bytes;
+  return LBCNN_OK;
+}
+
+}  // extern "C"
+
+// ---- workspace planning for the search driver ---------------------------------------------------
+namespace {
+struct SearchPlan {
+  FitPlan fit;
+  size_t fit_off, htr_off, hte_off, w_off, total;
+};
+void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, SearchPlan* p) {
+  lb_fit_plan(n_train, F, c, kc, 0, &p->fit);
+  size_t off = 0;
+  p->fit_off = off; off += p->fit.total;
+  p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * n_train * F * 4, 256);
+  p->hte_off = off; off += (size_t)lb_align_up((int64_t)kc * n_test * F * 4, 256);
+  p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
+  p->total = off;
+}
+// largest chunk size whose plan fits in `bytes` (0 if none)
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, size_t bytes) {
+  SearchPlan p;
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, &p);
+  if (p.total <= bytes) return n_cand;
+  int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
+  while (hi - lo > 1) {
+    const int mid = lo + (hi - lo) / 2;
+    plan_search(F, n_train, n_test, c, n_cand, mid, &p);
+    if (p.total <= bytes) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+}  // namespace
+
+extern "C" {
+
+int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
+                          int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes) {
+  (void)h;   // pure host arithmetic: a NULL handle is accepted
+  if (!bytes || n_train < 1 || n_test < 0 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  SearchPlan p1;
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, &p1);
+  if (min_bytes) *min_bytes = p1.total;
+  int kc = n_cand;
+  if (budget_bytes) {
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, budget_bytes);
+    if (kc < 1) kc = 1;
+  }
+  SearchPlan p;
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, &p);
+  FitPlan fp;   // a stand-alone lbcnn_elm_fit over all n_cand candidates must fit as well
+  lb_fit_plan(n_train, s.F, n_classes, n_cand, 0, &fp);
+  *bytes = p.total > fp.total ? p.total : fp.total;
+  return LBCNN_OK;
+}
+
+int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_images, int64_t n, const int8_t* d_kernels,
+                 const int32_t* d_bias, int32_t n_cand, float* d_H, void* stream) {
+  if (!h || !arch || !d_images || !d_kernels || !d_H || n < 1 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, (cudaStream_t)stream);
+}
+
+int lbcnn_elm_fit(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, float h_scale, uint32_t flags,
+                  const int32_t* d_labels, int32_t n_classes, float C, int32_t n_cand, float* d_W, int32_t* d_info,
+                  void* stream) {
+  if (!h || !d_H || !d_labels || !d_W || !d_info || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  if (!(C > 0.0f) || !(h_scale > 0.0f)) return LBCNN_ERR_INVALID_ARG;
+  if (n > 2147483647LL || F > 2147483647LL) return LBCNN_ERR_INVALID_ARG;
+  FitPlan p;
+  lb_fit_plan(n, F, n_classes, n_cand, flags, &p);
+  if (!h->ws || h->ws_bytes < p.total) return LBCNN_ERR_WORKSPACE;
+  return lb_launch_fit(h, h->ws, p, d_H, n, F, h_scale, d_labels, n_classes, C, n_cand, d_W, d_info, (cudaStream_t)stream);
+}
+
+int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
+                    int32_t n_classes, const int32_t* d_labels, int32_t n_cand, int32_t* d_pred, int32_t* d_correct,
+                    void* stream) {
+  if (!h || !d_H || !d_W || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  if (d_correct && !d_labels) return LBCNN_ERR_INVALID_ARG;
+  if (n > 2147483647LL || F > 2147483647LL || n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
+  return lb_launch_score(h, d_H, n, F, h_scale, d_W, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
+}
+
+int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_train,
+                            const int32_t* d_train_labels, int64_t n_train, const uint8_t* d_test,
+                            const int32_t* d_test_labels, int64_t n_test, int32_t n_classes, float C,
+                            const int8_t* d_kernels, const int32_t* d_bias, int32_t n_cand, float* d_acc,
+                            int32_t* d_correct, int32_t* d_info, int32_t* d_best, float* d_W_best, void* stream) {
+  if (!h || !arch || !d_train || !d_train_labels || !d_test || !d_test_labels || !d_kernels || !d_acc || !d_correct ||
+      !d_info || !d_best)
+    return LBCNN_ERR_INVALID_ARG;
+  if (n_train < 1 || n_test < 1 || n_classes < 2 || n_cand < 1 || !(C > 0.0f) || !(arch->feature_scale > 0.0f))
+    return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  if (!h->ws) return LBCNN_ERR_WORKSPACE;
+  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, h->ws_bytes);
+  if (kc < 1) return LBCNN_ERR_WORKSPACE;
+  SearchPlan p;
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, &p);
+  char* base = reinterpret_cast<char*>(h->ws);
+  float* Htr = reinterpret_cast<float*>(base + p.htr_off);
+  float* Hte = reinterpret_cast<float*>(base + p.hte_off);
+  float* Wall = reinterpret_cast<float*>(base + p.w_off);
+  cudaStream_t st = (cudaStream_t)stream;
+  const float hs = arch->feature_scale;
+  const int64_t wel = s.F * n_classes;
+  for (int k0 = 0; k0 < n_cand; k0 += kc) {
+    const int kn = (n_cand - k0 < kc) ? n_cand - k0 : kc;
+    const int8_t* ker = d_kernels + (int64_t)k0 * s.n_weights;
+    const int32_t* bias = d_bias ? d_bias + (int64_t)k0 * s.n_bias : nullptr;
+    // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale
+    rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, st);
+    if (rc) return rc;
+    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, st);
+    if (rc) return rc;
+    FitPlan fp;
+    lb_fit_plan(n_train, s.F, n_classes, kn, 0, &fp);
+    rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn,
+                       Wall + (int64_t)k0 * wel, d_info + k0, st);
+    if (rc) return rc;
+    rc = lb_launch_score(h, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn, nullptr,
+                         d_correct + k0, st);
+    if (rc) return rc;
+  }
+  return lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, Wall, wel, d_W_best, st);
+}
+
+}  // extern "C"
