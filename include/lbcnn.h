@@ -147,6 +147,16 @@ int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch,
  * bench.py's gpu_launches claim). */
 int lbcnn_launch_count(lbcnn_handle_t h, int64_t* count);
 
+/* Per-phase device timing, for measurement only (bench.py's roofline object).  With profiling on,
+ * every phase the library enqueues is bracketed by a pair of CUDA events on the caller's stream.
+ * lbcnn_get_phase_times BLOCKS until the recorded events have completed (the one call of this
+ * library that synchronises), adds the elapsed milliseconds and launch-bracket counts per phase
+ * into h_ms / h_count (host arrays of LBCNN_N_PHASES entries, overwritten) and clears the record. */
+enum { LBCNN_PHASE_EXPAND = 0, LBCNN_PHASE_GRAM = 1, LBCNN_PHASE_RHS = 2, LBCNN_PHASE_SOLVE = 3,
+       LBCNN_PHASE_SCORE = 4, LBCNN_PHASE_FINISH = 5, LBCNN_N_PHASES = 6 };
+int lbcnn_set_profiling(lbcnn_handle_t h, int enable);
+int lbcnn_get_phase_times(lbcnn_handle_t h, float* h_ms, int32_t* h_count);
+
 #ifdef __cplusplus
 }
 #endif

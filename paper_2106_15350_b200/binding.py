@@ -20,7 +20,9 @@ H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
-           "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_launch_count")
+           "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_launch_count", "lbcnn_set_profiling",
+           "lbcnn_get_phase_times")
+PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
 class Layer(C.Structure):
@@ -172,6 +174,16 @@ class Handle:
         n = C.c_int64()
         _check(lib().lbcnn_launch_count(self._h, C.byref(n)), "lbcnn_launch_count")
         return n.value
+
+    def set_profiling(self, enable: bool):
+        _check(lib().lbcnn_set_profiling(self._h, int(bool(enable))), "lbcnn_set_profiling")
+
+    def phase_times(self):
+        """blocks until the recorded phase events completed; returns {phase: (ms, brackets)}."""
+        ms = (C.c_float * len(PHASES))()
+        cnt = (C.c_int32 * len(PHASES))()
+        _check(lib().lbcnn_get_phase_times(self._h, ms, cnt), "lbcnn_get_phase_times")
+        return {p: (float(ms[i]), int(cnt[i])) for i, p in enumerate(PHASES)}
 
     # ---- the four calls of the path ----------------------------------------------------------
     def expand(self, arch: Arch, images, kernels, bias=None, out=None):

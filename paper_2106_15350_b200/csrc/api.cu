@@ -80,13 +80,35 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   p->device = device;
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device));
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
-  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0;
+  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
   *h = p;
   return LBCNN_OK;
 }
 
+int lbcnn_set_profiling(lbcnn_handle_t h, int enable) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  h->profiling = enable ? 1 : 0;
+  return LBCNN_OK;
+}
+
+int lbcnn_get_phase_times(lbcnn_handle_t h, float* h_ms, int32_t* h_count) {
+  if (!h || !h_ms || !h_count) return LBCNN_ERR_INVALID_ARG;
+  for (int i = 0; i < LBCNN_N_PHASES; ++i) { h_ms[i] = 0.0f; h_count[i] = 0; }
+  int rc = LBCNN_OK;
+  for (LbPhaseRec& r : h->recs) {
+    float ms = 0.0f;
+    if (cudaEventSynchronize(r.stop) != cudaSuccess || cudaEventElapsedTime(&ms, r.start, r.stop) != cudaSuccess)
+      rc = LBCNN_ERR_CUDA;
+    if (r.phase >= 0 && r.phase < LBCNN_N_PHASES) { h_ms[r.phase] += ms; h_count[r.phase] += 1; }
+    cudaEventDestroy(r.start); cudaEventDestroy(r.stop);
+  }
+  h->recs.clear();
+  return rc;
+}
+
 int lbcnn_destroy(lbcnn_handle_t h) {
   if (!h) return LBCNN_ERR_INVALID_ARG;
+  for (LbPhaseRec& r : h->recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
   delete h;
   return LBCNN_OK;
 }

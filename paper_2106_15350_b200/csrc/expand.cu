@@ -180,6 +180,7 @@ __global__ void __launch_bounds__(256) expand_kernel(const ExpandParams p) {
 
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, cudaStream_t st) {
+  LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
   ExpandParams p{};
   p.n_layers = s.n_layers;
   int act_words = 0, w_words = 0, b_words = 0, max_items = 0;

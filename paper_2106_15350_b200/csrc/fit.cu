@@ -263,6 +263,8 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
 
   if (pl.primal) {
     // F1: A = U^T U + lam I (lower tiles), operands read with k = sample (slow) and i = feature (contiguous)
+    {
+    LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     GemmP g{};
     g.A = d_H; g.sAr = 1; g.sAk = F; g.bA = n * F;
     g.B = d_H; g.sBr = 1; g.sBk = F; g.bB = n * F;
@@ -270,13 +272,17 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     g.M = (int)F; g.N = (int)F; g.K = (int)n; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
     rc = launch_gemm<float, float, double, false, false>(h, g, n_cand, st);
     if (rc) return rc;
+    }
     // F2: appended rows = (U^T T)^T
+    LbPhase ph2(h, LBCNN_PHASE_RHS, st);
     label_perm_kernel<<<1, 1024, (c + 1) * sizeof(int), st>>>(d_labels, (int)n, c, perm, off);
     h->launches += 1;
     dim3 gr((unsigned)((F + 127) / 128), (unsigned)c, (unsigned)n_cand);
     rhs_primal_kernel<<<gr, 128, 0, st>>>(d_H, n, F, perm, off, A, a_stride, dim);
     h->launches += 1;
   } else {
+    {
+    LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     GemmP g{};
     g.A = d_H; g.sAr = F; g.sAk = 1; g.bA = n * F;
     g.B = d_H; g.sBr = F; g.sBk = 1; g.bB = n * F;
@@ -284,12 +290,15 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     g.M = (int)n; g.N = (int)n; g.K = (int)F; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
     rc = launch_gemm<float, float, double, true, true>(h, g, n_cand, st);
     if (rc) return rc;
+    }
+    LbPhase ph2(h, LBCNN_PHASE_RHS, st);
     dim3 gr((unsigned)((n * c + 255) / 256), 1, (unsigned)n_cand);
     rhs_dual_kernel<<<gr, 256, 0, st>>>(d_labels, n, c, A, a_stride);
     h->launches += 1;
   }
   LB_CUDA_OK(cudaGetLastError());
 
+  LbPhase ph3(h, LBCNN_PHASE_SOLVE, st);
   const size_t tr_smem = 2 * NB * (NB + 1) * sizeof(double);
   LB_CUDA_OK(cudaFuncSetAttribute(trsm_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));
   LB_CUDA_OK(cudaFuncSetAttribute(bs_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));

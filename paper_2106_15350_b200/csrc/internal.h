@@ -5,6 +5,9 @@
 #include <stdint.h>
 #include <stddef.h>
 #include "../../include/lbcnn.h"
+#include <vector>
+
+struct LbPhaseRec { int phase; cudaEvent_t start, stop; };
 
 struct lbcnn_handle_s {
   int device;
@@ -13,6 +16,17 @@ struct lbcnn_handle_s {
   void* ws;
   size_t ws_bytes;
   int64_t launches;
+  int profiling;                    // record CUDA events around each phase of the path
+  std::vector<LbPhaseRec> recs;
+};
+
+// RAII phase marker: records start/stop events on the stream when profiling is on
+struct LbPhase {
+  lbcnn_handle_s* h; cudaStream_t st; LbPhaseRec r; bool on;
+  LbPhase(lbcnn_handle_s* h_, int phase, cudaStream_t st_) : h(h_), st(st_), on(h_->profiling != 0) {
+    if (on) { r.phase = phase; cudaEventCreate(&r.start); cudaEventCreate(&r.stop); cudaEventRecord(r.start, st); }
+  }
+  ~LbPhase() { if (on) { cudaEventRecord(r.stop, st); h->recs.push_back(r); } }
 };
 
 #define LB_CUDA_OK(expr)                                  \

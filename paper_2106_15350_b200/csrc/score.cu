@@ -100,6 +100,7 @@ __global__ void finish_kernel(const int32_t* __restrict__ correct, const int32_t
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                     int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
                     cudaStream_t st) {
+  LbPhase ph(h, LBCNN_PHASE_SCORE, st);
   if (d_correct) {
     int rc = lb_launch_zero_i32(h, d_correct, n_cand, st);
     if (rc) return rc;
@@ -121,6 +122,7 @@ int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,
                      cudaStream_t st) {
+  LbPhase ph(h, LBCNN_PHASE_FINISH, st);
   finish_kernel<<<1, 1024, 0, st>>>(d_correct, d_info, n_test, n_cand, d_acc, d_best, d_W_all, w_elems, d_W_best);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());

@@ -1,0 +1,307 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json `north_star`'s:
+  integer features (feature_scale = 1)   bit-exact
+  scaled features                        max relative error <= 1e-5 (exact zeros must match)
+  ELM weights                            relative Frobenius error <= 1e-3
+  predicted labels                       agreement >= 99.9 %
+  accuracy                               within 0.2 percentage points
+"""
+import dataclasses
+import zlib
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2106_15350_b200 import binding as lb
+from paper_2106_15350_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_FEAT_REL = 1e-5
+TOL_W_FRO = 1e-3
+TOL_LABEL_AGREE = 0.999
+TOL_ACC_PP = 0.2
+
+
+@pytest.fixture(scope="module")
+def handle():
+    h = lb.Handle(0)
+    yield h
+    h.close()
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _orc_arch(w):
+    return orc.make_arch(w.in_h, w.in_w, w.in_c, w.layers)
+
+
+def _small(name, n_train, n_test, n_cand):
+    return synth.scaled(synth.WORKLOADS[name], n_train, n_test, n_cand)
+
+
+# sizes chosen ragged on purpose (not multiples of 64 / of the CTA's candidate group of 8)
+EXPAND_CASES = [("tiny_mnist", 37, 11), ("mnist", 21, 9), ("gtsrb", 13, 3), ("orl", 5, 10), ("vggface", 7, 2),
+                ("paper_anchor", 9, 2)]
+
+
+@pytest.mark.parametrize("name,n,K", EXPAND_CASES)
+def test_expand_bit_exact(handle, name, n, K):
+    w = _small(name, n, 40 if name == "orl" else 4, K)
+    if name == "orl":
+        w = dataclasses.replace(w, n_train=40)
+    trx, _, _, _ = synth.make_dataset(w)
+    trx = trx[:n]
+    ker = synth.make_kernels(w, K)
+    H = handle.expand(lb.arch_of(w, 1.0), _dev(trx), _dev(ker)).cpu().numpy()
+    oa = _orc_arch(w)
+    for k in range(K):
+        u = orc.expand(oa, trx, ker[k])
+        assert np.array_equal(H[k].astype(np.int64), u), (name, k)
+        assert np.array_equal(H[k], u.astype(np.float32))
+
+
+def _variant_arch_cases():
+    F, D = lb.CONV_FULL, lb.CONV_DEPTHWISE
+    return [
+        # paper pool (4,2,1,cover_all) on the config-2/3 layer stacks: same F as the (2,2,0) reading
+        ("mnist_paperpool", (28, 28, 1), [(F, 10, 3, 0, 4, 2, 1, 1), (F, 20, 3, 0, 4, 2, 1, 1)]),
+        ("gtsrb_paperpool", (32, 32, 3), [(F, 16, 3, 0, 4, 2, 1, 1), (F, 32, 3, 0, 4, 2, 1, 1)]),
+        # three layers, mixed types, relu, odd channel counts, 5x5 then 3x3, no pool in the middle
+        ("three_layers", (19, 23, 2), [(F, 5, 5, 1, 2, 2, 0, 0), (D, 3, 3, 0, 1, 1, 0, 0), (F, 7, 3, 1, 3, 2, 1, 1)]),
+        # Table II family (40,2,2) depthwise: F = 2560
+        ("mnist_40_2_2", (28, 28, 1), [(D, 40, 3, 0, 4, 2, 1, 1), (D, 2, 3, 0, 4, 2, 1, 1), (D, 2, 3, 0, 4, 2, 1, 1)]),
+        ("k7_single", (9, 8, 1), [(F, 2, 7, 0, 3, 3, 0, 1)]),
+    ]
+
+
+@pytest.mark.parametrize("name,shape,layers", _variant_arch_cases(), ids=[c[0] for c in _variant_arch_cases()])
+def test_expand_variants_with_bias(handle, name, shape, layers):
+    rng = np.random.default_rng(zlib.crc32(name.encode()))
+    n, K = 6, 3
+    x = rng.integers(0, 256, size=(n,) + shape, dtype=np.uint8)
+    arch = lb.make_arch(*shape, layers, 1.0)
+    nw, nb = lb.kernel_set_size(arch)
+    ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+    bias = rng.integers(-300, 300, size=(K, nb)).astype(np.int32)
+    oa = orc.make_arch(*shape, layers)
+    F, _ = lb.feature_dim(arch)
+    assert F == orc.feature_dim(oa)[0]
+    for use_bias in (False, True):
+        H = handle.expand(arch, _dev(x), _dev(ker), _dev(bias) if use_bias else None).cpu().numpy()
+        for k in range(K):
+            u = orc.expand(oa, x, ker[k], bias[k] if use_bias else None)
+            assert np.array_equal(H[k].astype(np.int64), u), (name, use_bias, k)
+
+
+def test_expand_scaled_features(handle):
+    w = _small("gtsrb", 17, 4, 2)
+    trx, _, _, _ = synth.make_dataset(w)
+    ker = synth.make_kernels(w, 2)
+    s = np.float32(1.0 / 255.0)
+    H = handle.expand(lb.arch_of(w, float(s)), _dev(trx), _dev(ker)).cpu().numpy().astype(np.float64)
+    for k in range(2):
+        ref = orc.expand(_orc_arch(w), trx, ker[k]).astype(np.float64) * float(s)
+        z = ref == 0
+        assert np.array_equal(H[k][z], ref[z])
+        rel = np.abs(H[k][~z] - ref[~z]) / np.abs(ref[~z])
+        assert rel.max() <= TOL_FEAT_REL
+
+
+def _fro(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def _fit_case(handle, H, y, c, Creg, s, flags=0):
+    K = H.shape[0]
+    n, F = H.shape[1], H.shape[2]
+    handle.ensure_workspace((max(n, F) + c + 8) * max(n, F) * 8 * K + n * 4 + 4096 * 8)
+    W, info = handle.elm_fit(_dev(H), _dev(y), c, Creg, h_scale=s, flags=flags)
+    return W.cpu().numpy().astype(np.float64), info.cpu().numpy()
+
+
+@pytest.mark.parametrize("n,F,c,flags", [(150, 70, 5, 0), (70, 150, 5, 0), (130, 130, 3, 0), (257, 129, 11, lb.FORCE_DUAL),
+                                         (90, 200, 7, lb.FORCE_PRIMAL), (64, 64, 2, 0), (3, 2, 2, 0)])
+def test_fit_matches_oracle_general_fp32(handle, n, F, c, flags):
+    rng = np.random.default_rng(n * 1000 + F)
+    K = 3
+    H = rng.standard_normal((K, n, F)).astype(np.float32)
+    y = rng.integers(0, c, size=n).astype(np.int32)
+    y[:c] = np.arange(c) if n >= c else y[:c]
+    W, info = _fit_case(handle, H, y, c, 10.0, 1.0, flags)
+    assert (info == 0).all()
+    for k in range(K):
+        Wo, inf, br = orc.elm_fit(H[k].astype(np.float64), y, c, 10.0)
+        assert inf == 0
+        assert _fro(W[k], Wo) <= TOL_W_FRO
+        assert _fro(W[k], Wo) <= 1e-5     # what the fp64 path actually delivers (fp32 rounding of W)
+
+
+def test_fit_worked_example(handle):
+    # tests/golden/worked_examples.txt [elm_small]: H=[[1,0],[0,1],[1,1]], labels [0,1,0], C=1 -> W=[[.625,-.125],[.125,.375]]
+    H = np.array([[[1, 0], [0, 1], [1, 1]]], dtype=np.float32)
+    y = np.array([0, 1, 0], dtype=np.int32)
+    for flags in (lb.FORCE_PRIMAL, lb.FORCE_DUAL, 0):
+        W, info = _fit_case(handle, H, y, 2, 1.0, 1.0, flags)
+        assert info[0] == 0
+        assert np.allclose(W[0], [[0.625, -0.125], [0.125, 0.375]], atol=1e-7)
+    # scale identity W(sH, C) = W(H, C s^2)/s, here through h_scale
+    W2, _ = _fit_case(handle, H, y, 2, 4.0, 0.5)
+    assert np.allclose(W2[0], 2.0 * np.array([[0.625, -0.125], [0.125, 0.375]]), atol=1e-6)
+
+
+def test_fit_failure_is_reported_per_candidate(handle):
+    rng = np.random.default_rng(5)
+    H = rng.standard_normal((3, 40, 8)).astype(np.float32)
+    H[1, 3, 2] = np.nan
+    y = rng.integers(0, 3, size=40).astype(np.int32)
+    W, info = _fit_case(handle, H, y, 3, 1.0, 1.0)
+    assert info[0] == 0 and info[2] == 0 and info[1] > 0
+    Wo, _, _ = orc.elm_fit(H[2].astype(np.float64), y, 3, 1.0)
+    assert _fro(W[2], Wo) <= 1e-5
+
+
+def test_score_matches_oracle_and_ties(handle):
+    rng = np.random.default_rng(11)
+    K, n, F, c = 2, 203, 97, 70
+    H = rng.integers(-50, 50, size=(K, n, F)).astype(np.float32)
+    W = rng.standard_normal((K, F, c)).astype(np.float32)
+    y = rng.integers(0, c, size=n).astype(np.int32)
+    pred, corr = handle.elm_score(_dev(H), _dev(W), _dev(y), h_scale=0.25)
+    pred, corr = pred.cpu().numpy(), corr.cpu().numpy()
+    for k in range(K):
+        po, co, _ = orc.elm_score(H[k].astype(np.float64) * 0.25, W[k].astype(np.float64), y)
+        assert np.array_equal(pred[k], po)
+        assert corr[k] == co
+    # exact ties -> lowest class index; all-zero W -> class 0
+    Wz = np.zeros((1, F, c), dtype=np.float32)
+    pz, _ = handle.elm_score(_dev(H[:1]), _dev(Wz))
+    assert (pz.cpu().numpy() == 0).all()
+    Wt = np.zeros((1, F, c), dtype=np.float32)
+    Wt[0, :, 65] = 1.0
+    Wt[0, :, 3] = 1.0
+    Hp = np.abs(H[:1]) + 1
+    pt, _ = handle.elm_score(_dev(Hp), _dev(Wt))
+    assert (pt.cpu().numpy() == 3).all()
+
+
+def _search_both(handle, w, budget=None):
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    full, mn = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, budget or 0)
+    handle.set_workspace(None)
+    handle.ensure_workspace(full)
+    out = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    torch.cuda.synchronize()
+    ref = orc.search(_orc_arch(w), trx, try_, tex, tey, w.n_classes, w.C, ker, feature_scale=w.feature_scale, keep=True)
+    return {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}, ref
+
+
+def _check_search(w, got, ref):
+    K = w.n_cand
+    assert (got["info"] == 0).all() and (ref["info"] == 0).all()
+    agree = 1.0 - np.abs(got["correct"].astype(np.int64) - ref["correct"]) / float(w.n_test)
+    assert (agree >= TOL_LABEL_AGREE).all()          # a lower bound on label agreement from the counts
+    assert (np.abs(got["acc"].astype(np.float64) - ref["acc"]) * 100.0 <= TOL_ACC_PP).all()
+    b, wst = int(got["best"][0]), int(got["best"][1])
+    top = np.sort(ref["acc"])[::-1]
+    if b != ref["best"]:
+        assert abs(ref["acc"][b] - ref["acc"][ref["best"]]) * 100.0 <= TOL_ACC_PP      # near-tie only
+    if wst != ref["worst"]:
+        assert abs(ref["acc"][wst] - ref["acc"][ref["worst"]]) * 100.0 <= TOL_ACC_PP
+    assert _fro(got["W_best"].astype(np.float64), ref["W"][b]) <= TOL_W_FRO
+    assert K == len(ref["acc"]) and top[0] >= top[-1]
+
+
+SEARCH_CASES = [("tiny_mnist", None, None, None), ("mnist", 1500, 700, 5), ("gtsrb", 2600, 500, 3),
+                ("orl", 280, 120, 12), ("vggface", 900, 300, 2), ("paper_anchor", 300, 200, 2)]
+
+
+@pytest.mark.parametrize("name,ntr,nte,K", SEARCH_CASES, ids=[c[0] for c in SEARCH_CASES])
+def test_search_matches_oracle(handle, name, ntr, nte, K):
+    w = synth.WORKLOADS[name] if ntr is None else _small(name, ntr, nte, K)
+    got, ref = _search_both(handle, w)
+    _check_search(w, got, ref)
+
+
+def test_search_chunked_equals_unchunked(handle):
+    w = _small("mnist", 400, 150, 7)
+    arch = lb.arch_of(w)
+    full, mn = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)
+    a, _ = _search_both(handle, w)
+    # a workspace that only fits 2-3 candidates per chunk must give identical results
+    b, _ = _search_both(handle, w, budget=mn + (full - mn) // 3)
+    for k in ("acc", "correct", "info", "best", "W_best"):
+        assert np.array_equal(a[k], b[k]), k
+    handle.set_workspace(None)
+    handle.ensure_workspace(mn - 256)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    with pytest.raises(lb.LbcnnError) as e:
+        handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C,
+                                 _dev(synth.make_kernels(w)))
+    assert e.value.status == lb.ERR_WORKSPACE
+
+
+def test_staged_calls_replay_the_search(handle):
+    """expand -> fit -> score through the three stand-alone entry points reproduces the driver's numbers
+    (replay of the best kernels, PAPER.md:94 `use_stored`), and labels agree with the oracle's one by one."""
+    w = _small("gtsrb", 1200, 400, 2)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    got, ref = _search_both(handle, w)
+    a1 = lb.arch_of(w, 1.0)
+    Htr = handle.expand(a1, _dev(trx), _dev(ker))
+    Hte = handle.expand(a1, _dev(tex), _dev(ker))
+    s = float(np.float32(w.feature_scale))
+    handle.set_workspace(None)
+    handle.ensure_workspace(lb.workspace_bytes(a1, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+    W, info = handle.elm_fit(Htr, _dev(try_), w.n_classes, w.C, h_scale=s, flags=lb.H_INTEGER)
+    pred, corr = handle.elm_score(Hte, W, _dev(tey), h_scale=s)
+    assert np.array_equal(corr.cpu().numpy(), got["correct"])
+    pred = pred.cpu().numpy()
+    for k in range(w.n_cand):
+        assert (pred[k] == ref["pred"][k]).mean() >= TOL_LABEL_AGREE
+        assert _fro(W[k].cpu().numpy().astype(np.float64), ref["W"][k]) <= TOL_W_FRO
+
+
+def test_full_size_bench_config_sampled(handle):
+    """BASELINE configs[1] (the bench workload) at full size, in the launch configuration bench.py times:
+    sampled feature rows, and two whole candidates' W / labels / accuracy, against the oracle."""
+    w = synth.WORKLOADS["mnist"]
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    full, _ = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)
+    handle.set_workspace(None)
+    handle.ensure_workspace(full)
+    out = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    acc = out["acc"].cpu().numpy()
+    correct = out["correct"].cpu().numpy()
+    assert (out["info"].cpu().numpy() == 0).all()
+    best = int(out["best"][0])
+    assert best == int(np.argmax(correct)) and int(out["best"][1]) == int(np.argmin(correct))
+    oa = _orc_arch(w)
+    s = float(np.float32(w.feature_scale))
+    # sampled feature rows of sampled candidates, through lbcnn_expand at full n
+    rows = np.array([0, 1, 63, 64, 4097, 19999])
+    H = handle.expand(lb.arch_of(w, 1.0), _dev(trx), _dev(ker[60:64])).cpu().numpy()
+    for j, k in enumerate(range(60, 64)):
+        assert np.array_equal(H[j][rows].astype(np.int64), orc.expand(oa, trx[rows], ker[k]))
+    del H
+    # the best candidate and candidate 0, whole
+    for k in sorted({best, 0}):
+        Htr = orc.expand(oa, trx, ker[k]).astype(np.float64) * s
+        Hte = orc.expand(oa, tex, ker[k]).astype(np.float64) * s
+        Wo, inf, _ = orc.elm_fit(Htr, try_, w.n_classes, w.C)
+        po, co, _ = orc.elm_score(Hte, Wo, tey)
+        assert inf == 0
+        assert abs(co - int(correct[k])) <= (1.0 - TOL_LABEL_AGREE) * w.n_test
+        assert abs(co / w.n_test - acc[k]) * 100.0 <= TOL_ACC_PP
+        if k == best:
+            assert _fro(out["W_best"].cpu().numpy().astype(np.float64), Wo) <= TOL_W_FRO
