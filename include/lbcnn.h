@@ -143,6 +143,23 @@ int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch,
                             float* d_acc /*[n_cand]*/, int32_t* d_correct /*[n_cand]*/, int32_t* d_info /*[n_cand]*/,
                             int32_t* d_best /*[2]*/, float* d_W_best /*[F][n_classes] or NULL*/, void* stream);
 
+/* The same search loop with HOST buffers: every h_* pointer is host memory (pinned memory
+ * makes the copies asynchronous), layouts as in lbcnn_search_candidates.  The call stages the inputs into the
+ * first lbcnn_host_staging_bytes() bytes of the workspace with cudaMemcpyAsync on `stream` (the notebook's
+ * Cell 2 "move train/test to GPU memory"), runs the loop in the rest of the workspace, copies
+ * acc / correct / info / best (/ W_best) back and SYNCHRONISES the stream before returning (the only
+ * compute entry point that does).  Workspace needed: lbcnn_host_staging_bytes + a size
+ * lbcnn_workspace_bytes accepts (>= its min_bytes); too small -> LBCNN_ERR_WORKSPACE. */
+int lbcnn_host_staging_bytes(const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test, int32_t n_classes,
+                             int32_t n_cand, int32_t has_bias, size_t* bytes);
+int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch,
+                                 const uint8_t* h_train, const int32_t* h_train_labels, int64_t n_train,
+                                 const uint8_t* h_test, const int32_t* h_test_labels, int64_t n_test,
+                                 int32_t n_classes, float C,
+                                 const int8_t* h_kernels, const int32_t* h_bias /*or NULL*/, int32_t n_cand,
+                                 float* h_acc /*[n_cand]*/, int32_t* h_correct /*[n_cand]*/, int32_t* h_info /*[n_cand]*/,
+                                 int32_t* h_best /*[2]*/, float* h_W_best /*[F][n_classes] or NULL*/, void* stream);
+
 /* Number of kernel launches the library has enqueued through this handle since creation (for
  * bench.py's gpu_launches claim). */
 int lbcnn_launch_count(lbcnn_handle_t h, int64_t* count);

@@ -20,7 +20,8 @@ H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
-           "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_launch_count", "lbcnn_set_profiling",
+           "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
+           "lbcnn_launch_count", "lbcnn_set_profiling",
            "lbcnn_get_phase_times")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
@@ -116,6 +117,25 @@ def workspace_bytes(arch: Arch, n_train: int, n_test: int, n_classes: int, n_can
                                        C.c_int32(n_cand), C.c_size_t(budget_bytes), C.byref(b), C.byref(m)),
            "lbcnn_workspace_bytes")
     return b.value, m.value
+
+
+def host_staging_bytes(arch: Arch, n_train: int, n_test: int, n_classes: int, n_cand: int, has_bias: bool = False) -> int:
+    b = C.c_size_t()
+    _check(lib().lbcnn_host_staging_bytes(C.byref(arch), C.c_int64(n_train), C.c_int64(n_test), C.c_int32(n_classes),
+                                          C.c_int32(n_cand), C.c_int32(int(has_bias)), C.byref(b)),
+           "lbcnn_host_staging_bytes")
+    return b.value
+
+
+def _hptr(t, dtype=None, allow_none: bool = False):
+    """host pointer of a contiguous CPU torch tensor (pinned or not) or NULL."""
+    if t is None:
+        if allow_none:
+            return C.c_void_p(None)
+        raise LbcnnError(ERR_INVALID_ARG, "null tensor")
+    if t.is_cuda or not t.is_contiguous() or (dtype is not None and t.dtype != dtype):
+        raise LbcnnError(ERR_INVALID_ARG, "tensor must be a contiguous CPU tensor of dtype %s" % dtype)
+    return C.c_void_p(t.data_ptr())
 
 
 def _ptr(t, dtype=None, allow_none: bool = False):
@@ -241,4 +261,26 @@ class Handle:
             C.c_float(Creg), _ptr(kernels, torch.int8), _ptr(bias, torch.int32, True), C.c_int32(K),
             _ptr(out["acc"]), _ptr(out["correct"]), _ptr(out["info"]), _ptr(out["best"]),
             _ptr(out["W_best"], None, True), _stream()), "lbcnn_search_candidates")
+        return out
+
+    def search_candidates_host(self, arch: Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: float,
+                               kernels, bias=None, want_W: bool = True, out=None):
+        """lbcnn_search_candidates_host: all tensors are CPU tensors (pin them for asynchronous copies); the
+        call copies them in, runs the loop, copies the results back and synchronises.  Returns CPU tensors."""
+        import torch
+        F, _ = feature_dim(arch)
+        K = kernels.shape[0]
+        if out is None:
+            pin = torch.cuda.is_available()
+            out = dict(acc=torch.empty(K, dtype=torch.float32, pin_memory=pin),
+                       correct=torch.empty(K, dtype=torch.int32, pin_memory=pin),
+                       info=torch.empty(K, dtype=torch.int32, pin_memory=pin),
+                       best=torch.empty(2, dtype=torch.int32, pin_memory=pin),
+                       W_best=torch.empty((F, n_classes), dtype=torch.float32, pin_memory=pin) if want_W else None)
+        _check(lib().lbcnn_search_candidates_host(
+            self._h, C.byref(arch), _hptr(train_x, torch.uint8), _hptr(train_y, torch.int32),
+            C.c_int64(train_x.shape[0]), _hptr(test_x, torch.uint8), _hptr(test_y, torch.int32),
+            C.c_int64(test_x.shape[0]), C.c_int32(n_classes), C.c_float(Creg), _hptr(kernels, torch.int8),
+            _hptr(bias, torch.int32, True), C.c_int32(K), _hptr(out["acc"]), _hptr(out["correct"]), _hptr(out["info"]),
+            _hptr(out["best"]), _hptr(out["W_best"], None, True), _stream()), "lbcnn_search_candidates_host")
         return out

@@ -235,11 +235,14 @@ int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, fl
   return lb_launch_score(h, d_H, n, F, h_scale, d_W, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
 }
 
-int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_train,
-                            const int32_t* d_train_labels, int64_t n_train, const uint8_t* d_test,
-                            const int32_t* d_test_labels, int64_t n_test, int32_t n_classes, float C,
-                            const int8_t* d_kernels, const int32_t* d_bias, int32_t n_cand, float* d_acc,
-                            int32_t* d_correct, int32_t* d_info, int32_t* d_best, float* d_W_best, void* stream) {
+}  // extern "C"
+
+// the search loop on device buffers, scratch taken from [ws, ws + ws_bytes)
+static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_arch_t* arch, const uint8_t* d_train,
+                       const int32_t* d_train_labels, int64_t n_train, const uint8_t* d_test,
+                       const int32_t* d_test_labels, int64_t n_test, int32_t n_classes, float C,
+                       const int8_t* d_kernels, const int32_t* d_bias, int32_t n_cand, float* d_acc,
+                       int32_t* d_correct, int32_t* d_info, int32_t* d_best, float* d_W_best, void* stream) {
   if (!h || !arch || !d_train || !d_train_labels || !d_test || !d_test_labels || !d_kernels || !d_acc || !d_correct ||
       !d_info || !d_best)
     return LBCNN_ERR_INVALID_ARG;
@@ -248,12 +251,12 @@ int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const ui
   ArchShape s;
   int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
-  if (!h->ws) return LBCNN_ERR_WORKSPACE;
-  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, h->ws_bytes);
+  if (!ws) return LBCNN_ERR_WORKSPACE;
+  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, ws_bytes);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
   SearchPlan p;
   plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, &p);
-  char* base = reinterpret_cast<char*>(h->ws);
+  char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
   float* Wall = reinterpret_cast<float*>(base + p.w_off);
@@ -279,6 +282,100 @@ int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const ui
     if (rc) return rc;
   }
   return lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, Wall, wel, d_W_best, st);
+}
+
+// ---- host-buffer staging layout (lbcnn_search_candidates_host) ----------------------------------
+namespace {
+struct HostStage {
+  size_t train, train_y, test, test_y, ker, bias, acc, correct, info, best, wbest, total;
+};
+void plan_host_stage(const ArchShape& s, int64_t n_train, int64_t n_test, int c, int n_cand, int has_bias, HostStage* p) {
+  const int64_t px = (int64_t)s.L[0].hin * s.L[0].win * s.L[0].cin;
+  size_t off = 0;
+  auto take = [&](int64_t bytes) { size_t o = off; off += (size_t)lb_align_up(bytes, 256); return o; };
+  p->train = take(n_train * px);
+  p->train_y = take(n_train * 4);
+  p->test = take(n_test * px);
+  p->test_y = take(n_test * 4);
+  p->ker = take((int64_t)n_cand * s.n_weights);
+  p->bias = take(has_bias ? (int64_t)n_cand * s.n_bias * 4 : 0);
+  p->acc = take((int64_t)n_cand * 4);
+  p->correct = take((int64_t)n_cand * 4);
+  p->info = take((int64_t)n_cand * 4);
+  p->best = take(8);
+  p->wbest = take(s.F * c * 4);
+  p->total = off;
+}
+}  // namespace
+
+extern "C" {
+
+int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_train,
+                            const int32_t* d_train_labels, int64_t n_train, const uint8_t* d_test,
+                            const int32_t* d_test_labels, int64_t n_test, int32_t n_classes, float C,
+                            const int8_t* d_kernels, const int32_t* d_bias, int32_t n_cand, float* d_acc,
+                            int32_t* d_correct, int32_t* d_info, int32_t* d_best, float* d_W_best, void* stream) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  return search_impl(h, h->ws, h->ws_bytes, arch, d_train, d_train_labels, n_train, d_test, d_test_labels, n_test,
+                     n_classes, C, d_kernels, d_bias, n_cand, d_acc, d_correct, d_info, d_best, d_W_best, stream);
+}
+
+int lbcnn_host_staging_bytes(const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test, int32_t n_classes,
+                             int32_t n_cand, int32_t has_bias, size_t* bytes) {
+  if (!bytes || n_train < 1 || n_test < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  HostStage p;
+  plan_host_stage(s, n_train, n_test, n_classes, n_cand, has_bias, &p);
+  *bytes = p.total;
+  return LBCNN_OK;
+}
+
+int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* h_train,
+                                 const int32_t* h_train_labels, int64_t n_train, const uint8_t* h_test,
+                                 const int32_t* h_test_labels, int64_t n_test, int32_t n_classes, float C,
+                                 const int8_t* h_kernels, const int32_t* h_bias, int32_t n_cand, float* h_acc,
+                                 int32_t* h_correct, int32_t* h_info, int32_t* h_best, float* h_W_best, void* stream) {
+  if (!h || !arch || !h_train || !h_train_labels || !h_test || !h_test_labels || !h_kernels || !h_acc || !h_correct ||
+      !h_info || !h_best)
+    return LBCNN_ERR_INVALID_ARG;
+  if (n_train < 1 || n_test < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  HostStage p;
+  plan_host_stage(s, n_train, n_test, n_classes, n_cand, h_bias != nullptr, &p);
+  if (!h->ws || h->ws_bytes <= p.total) return LBCNN_ERR_WORKSPACE;
+  char* base = reinterpret_cast<char*>(h->ws);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t px = (int64_t)s.L[0].hin * s.L[0].win * s.L[0].cin;
+  LB_CUDA_OK(cudaMemcpyAsync(base + p.train, h_train, (size_t)(n_train * px), cudaMemcpyHostToDevice, st));
+  LB_CUDA_OK(cudaMemcpyAsync(base + p.train_y, h_train_labels, (size_t)n_train * 4, cudaMemcpyHostToDevice, st));
+  LB_CUDA_OK(cudaMemcpyAsync(base + p.test, h_test, (size_t)(n_test * px), cudaMemcpyHostToDevice, st));
+  LB_CUDA_OK(cudaMemcpyAsync(base + p.test_y, h_test_labels, (size_t)n_test * 4, cudaMemcpyHostToDevice, st));
+  LB_CUDA_OK(cudaMemcpyAsync(base + p.ker, h_kernels, (size_t)n_cand * s.n_weights, cudaMemcpyHostToDevice, st));
+  if (h_bias)
+    LB_CUDA_OK(cudaMemcpyAsync(base + p.bias, h_bias, (size_t)n_cand * s.n_bias * 4, cudaMemcpyHostToDevice, st));
+  float* d_acc = reinterpret_cast<float*>(base + p.acc);
+  int32_t* d_correct = reinterpret_cast<int32_t*>(base + p.correct);
+  int32_t* d_info = reinterpret_cast<int32_t*>(base + p.info);
+  int32_t* d_best = reinterpret_cast<int32_t*>(base + p.best);
+  float* d_wb = h_W_best ? reinterpret_cast<float*>(base + p.wbest) : nullptr;
+  rc = search_impl(h, base + p.total, h->ws_bytes - p.total, arch, reinterpret_cast<const uint8_t*>(base + p.train),
+                   reinterpret_cast<const int32_t*>(base + p.train_y), n_train,
+                   reinterpret_cast<const uint8_t*>(base + p.test), reinterpret_cast<const int32_t*>(base + p.test_y),
+                   n_test, n_classes, C, reinterpret_cast<const int8_t*>(base + p.ker),
+                   h_bias ? reinterpret_cast<const int32_t*>(base + p.bias) : nullptr, n_cand, d_acc, d_correct, d_info,
+                   d_best, d_wb, stream);
+  if (rc) return rc;
+  LB_CUDA_OK(cudaMemcpyAsync(h_acc, d_acc, (size_t)n_cand * 4, cudaMemcpyDeviceToHost, st));
+  LB_CUDA_OK(cudaMemcpyAsync(h_correct, d_correct, (size_t)n_cand * 4, cudaMemcpyDeviceToHost, st));
+  LB_CUDA_OK(cudaMemcpyAsync(h_info, d_info, (size_t)n_cand * 4, cudaMemcpyDeviceToHost, st));
+  LB_CUDA_OK(cudaMemcpyAsync(h_best, d_best, 8, cudaMemcpyDeviceToHost, st));
+  if (h_W_best) LB_CUDA_OK(cudaMemcpyAsync(h_W_best, d_wb, (size_t)(s.F * n_classes) * 4, cudaMemcpyDeviceToHost, st));
+  LB_CUDA_OK(cudaStreamSynchronize(st));
+  return LBCNN_OK;
 }
 
 }  // extern "C"
