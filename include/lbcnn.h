@@ -50,7 +50,7 @@ enum { LBCNN_CONV_FULL = 0, LBCNN_CONV_DEPTHWISE = 1 };
 enum { LBCNN_ACT_NONE = 0, LBCNN_ACT_RELU = 1 };
 
 /* flags of lbcnn_elm_fit */
-#define LBCNN_H_INTEGER 1u /* stored H values are integers with abs < 2^24 (the expander's output with feature_scale = 1) */
+#define LBCNN_H_INTEGER 1u /* stored H values are integers with abs < 2^23 (the expander's output with feature_scale = 1): the Gram is then computed exactly on the tensor cores */
 #define LBCNN_FORCE_PRIMAL 2u /* testing: take the F x F branch whatever F and n are */
 #define LBCNN_FORCE_DUAL 4u   /* testing: take the n x n branch */
 

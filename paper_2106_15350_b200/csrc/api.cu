@@ -156,8 +156,8 @@ struct SearchPlan {
   FitPlan fit;
   size_t fit_off, htr_off, hte_off, w_off, total;
 };
-void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, SearchPlan* p) {
-  lb_fit_plan(n_train, F, c, kc, 0, &p->fit);
+void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, SearchPlan* p) {
+  lb_fit_plan(n_train, F, c, kc, flags, &p->fit);
   size_t off = 0;
   p->fit_off = off; off += p->fit.total;
   p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * n_train * F * 4, 256);
@@ -165,15 +165,17 @@ void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, 
   p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
   p->total = off;
 }
+// the driver's features are exact integers; below 2^23 the fit may use the exact tensor-core Gram
+uint32_t search_fit_flags(const ArchShape& s) { return s.max_abs < (1LL << 23) ? LBCNN_H_INTEGER : 0u; }
 // largest chunk size whose plan fits in `bytes` (0 if none)
-int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, size_t bytes) {
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t bytes) {
   SearchPlan p;
-  plan_search(F, n_train, n_test, c, n_cand, n_cand, &p);
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, &p);
   if (p.total <= bytes) return n_cand;
   int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
   while (hi - lo > 1) {
     const int mid = lo + (hi - lo) / 2;
-    plan_search(F, n_train, n_test, c, n_cand, mid, &p);
+    plan_search(F, n_train, n_test, c, n_cand, mid, flags, &p);
     if (p.total <= bytes) lo = mid; else hi = mid;
   }
   return lo;
@@ -190,16 +192,16 @@ int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_
   const int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
   SearchPlan p1;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, &p1);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, search_fit_flags(s), &p1);
   if (min_bytes) *min_bytes = p1.total;
   int kc = n_cand;
   if (budget_bytes) {
-    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, budget_bytes);
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, search_fit_flags(s), budget_bytes);
     if (kc < 1) kc = 1;
   }
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, &p);
-  FitPlan fp;   // a stand-alone lbcnn_elm_fit over all n_cand candidates must fit as well
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, search_fit_flags(s), &p);
+  FitPlan fp;   // a stand-alone lbcnn_elm_fit over all n_cand candidates (flags = 0) must fit as well
   lb_fit_plan(n_train, s.F, n_classes, n_cand, 0, &fp);
   *bytes = p.total > fp.total ? p.total : fp.total;
   return LBCNN_OK;
@@ -252,10 +254,11 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
   if (!ws) return LBCNN_ERR_WORKSPACE;
-  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, ws_bytes);
+  const uint32_t fflags = search_fit_flags(s);
+  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, ws_bytes);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, &p);
   char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
@@ -273,7 +276,7 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
     rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, st);
     if (rc) return rc;
     FitPlan fp;
-    lb_fit_plan(n_train, s.F, n_classes, kn, 0, &fp);
+    lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp);
     rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn,
                        Wall + (int64_t)k0 * wel, d_info + k0, st);
     if (rc) return rc;

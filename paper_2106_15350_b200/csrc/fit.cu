@@ -241,6 +241,8 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->perm_off = off; off += (size_t)lb_align_up(n * 4, 256);
   p->off_off = off;  off += (size_t)lb_align_up(((int64_t)n_classes + 1) * 4, 256);
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
+  p->use_tc = ((flags & LBCNN_H_INTEGER) && primal && lb_gram_tc_usable(n, F)) ? 1 : 0;
+  p->tc_off = off;   if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand);
   p->total = off;
 }
 
@@ -265,6 +267,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     // F1: A = U^T U + lam I (lower tiles), operands read with k = sample (slow) and i = feature (contiguous)
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
+    if (pl.use_tc) {
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, st);
+      if (rc) return rc;
+    } else {
     GemmP g{};
     g.A = d_H; g.sAr = 1; g.sAk = F; g.bA = n * F;
     g.B = d_H; g.sBr = 1; g.sBk = F; g.bB = n * F;
@@ -272,6 +278,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     g.M = (int)F; g.N = (int)F; g.K = (int)n; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
     rc = launch_gemm<float, float, double, false, false>(h, g, n_cand, st);
     if (rc) return rc;
+    }
     }
     // F2: appended rows = (U^T T)^T
     LbPhase ph2(h, LBCNN_PHASE_RHS, st);

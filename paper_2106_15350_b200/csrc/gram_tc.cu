@@ -1,0 +1,262 @@
+// gram_tc.cu -- K2 on the tensor pipe: the EXACT Gram matrix of integer-valued features (F1, PAPER.md:66-70
+// `cp.dot(H,H.T)`), A = U^T U + lam I, with tcgen05.mma kind::i8 and int32 accumulators in TMEM.
+//
+// The expander's features are exact integers (R14).  Every integer u with |u| < 2^23 is written
+// as balanced radix-256 digits  u = d0 + 256 d1 + 65536 d2,  d in [-128, 127]  (1, 2 or 3 digits, chosen
+// per candidate from the data), so
+//     G[i][j] = sum_n u[n][i] u[n][j] = sum_s 256^s P_s[i][j],   P_s = sum_{a+b=s} D_a^T D_b
+// where every P_s is a sum of int8 x int8 products: exact in the tensor core's int32 accumulators as long as
+// 3 * 128^2 * n < 2^31, i.e. n <= 43690 samples (larger n takes the fp64 SIMT path).  The epilogue
+// recombines the P_s in int64 and rounds ONCE to fp64 -- the Gram is bit-exact, which is what the
+// conditioning of the configs' systems needs (cond ~ 1e6; an fp32-accumulated Gram misses the 1e-3
+// tolerance on W).  9 int8 MMAs (3 digits) cost 2.25 TF32-MMA equivalents, 4 (2 digits)
+// cost 1 -- cheaper than 3xTF32 and exact.
+//
+// Pipeline (one CTA per 128 x 96 output tile of one candidate, lower-triangle tiles only):
+//   split kernel : fp32 H [K][n][F] -> digit planes int8 [K][3][n][Fp] (F contiguous) + digits needed per candidate
+//   warp 0       : TMA producer, 64-sample stages of the digit planes (128-byte swizzle), mbarrier ring
+//   warp 1       : one thread issues tcgen05.mma (M=128, N=96, K=32; MN-major operands: the feature index
+//                  is contiguous in memory, no transpose anywhere); tcgen05.commit frees stages
+//   warps 2..5   : epilogue, tcgen05.ld the 2L-1 accumulators, int64 recombination, fp64 store
+#include "internal.h"
+#include "tc_common.cuh"
+#include <cuda.h>
+
+namespace {
+
+constexpr int TM = 128;        // output tile rows (features i)   = UMMA M
+constexpr int TN = 96;         // output tile columns (features j) = UMMA N
+constexpr int KS = 64;         // samples per pipeline stage (two K = 32 MMA steps)
+constexpr int BOXW = 128;      // TMA box width in features (= bytes): one 128-byte swizzle row
+constexpr int TILE_BYTES = KS * BOXW;          // 8 KB per digit plane per operand per stage
+constexpr int MAXL = 3;
+constexpr int STAGE_BYTES = 2 * MAXL * TILE_BYTES;   // 48 KB
+constexpr int NSTAGE = 4;
+constexpr int TMEM_COLS = 512; // 5 accumulators x 96 columns = 480
+constexpr int NTHREADS = 192;
+
+struct GramTcParams {
+  const int32_t* nlimb;   // [n_cand] digits needed (1..3)
+  double* A; long long a_stride, ld;
+  int F, n, n_iters;
+  double lam;
+};
+
+// ---- digit split ----------------------------------------------------------------------------------
+// thread = 16 consecutive features of one sample of one candidate
+__global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
+                                                    int8_t* __restrict__ planes, int32_t* __restrict__ nlimb) {
+  const int z = blockIdx.y;
+  const long long chunks_per_row = Fp / 16;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int need = 1;
+  if (t < n * chunks_per_row) {
+    const long long row = t / chunks_per_row;
+    const int f0 = (int)(t % chunks_per_row) * 16;
+    const float* src = U + ((long long)z * n + row) * F + f0;
+    int v[16];
+    if ((F & 3) == 0 && f0 + 16 <= F) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float4 x = *reinterpret_cast<const float4*>(src + 4 * q);
+        v[4 * q] = (int)x.x; v[4 * q + 1] = (int)x.y; v[4 * q + 2] = (int)x.z; v[4 * q + 3] = (int)x.w;
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < 16; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
+    }
+    uint32_t w[3][4] = {};
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      const int u = v[q];
+      const int d0 = ((u + 128) & 255) - 128;
+      const int u1 = (u - d0) >> 8;
+      const int d1 = ((u1 + 128) & 255) - 128;
+      const int d2 = (u1 - d1) >> 8;
+      if (u1 != 0) need = max(need, 2);
+      if (d2 != 0) need = max(need, 3);
+      w[0][q >> 2] |= (uint32_t)(d0 & 255) << (8 * (q & 3));
+      w[1][q >> 2] |= (uint32_t)(d1 & 255) << (8 * (q & 3));
+      w[2][q >> 2] |= (uint32_t)(d2 & 255) << (8 * (q & 3));
+    }
+#pragma unroll
+    for (int l = 0; l < 3; ++l) {
+      int8_t* dst = planes + (((long long)z * 3 + l) * n + row) * Fp + f0;
+      *reinterpret_cast<uint4*>(dst) = make_uint4(w[l][0], w[l][1], w[l][2], w[l][3]);
+    }
+  }
+  need = __reduce_max_sync(0xffffffffu, need);
+  if ((threadIdx.x & 31) == 0 && need > 1) atomicMax(&nlimb[z], need);
+}
+
+__global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < n) p[t] = v;
+}
+
+// ---- the Gram kernel ------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const GramTcParams p) {
+  const int ti = blockIdx.y, tj = blockIdx.x, z = blockIdx.z;
+  const int i0 = ti * TM, j0 = tj * TN;
+  if (j0 > i0 + TM - 1) return;                 // tile entirely above the diagonal
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  // 1024-byte alignment for the 128-byte swizzle atoms
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  __shared__ __align__(8) uint64_t bar_full[NSTAGE], bar_empty[NSTAGE], bar_tmem;
+  __shared__ uint32_t tmem_base_s;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int L = p.nlimb[z];
+  const uint32_t smem0 = tc::smem_u32(smem);
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tensormap(&tmap);
+    for (int s = 0; s < NSTAGE; ++s) { tc::mbar_init(tc::smem_u32(&bar_full[s]), 1); tc::mbar_init(tc::smem_u32(&bar_empty[s]), 1); }
+    tc::mbar_init(tc::smem_u32(&bar_tmem), 1);
+    tc::fence_barrier_init();
+  }
+  if (warp == 1) tc::tmem_alloc(tc::smem_u32(&tmem_base_s), TMEM_COLS);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      for (int it = 0; it < p.n_iters; ++it) {
+        const int s = it % NSTAGE;
+        tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ((it / NSTAGE) & 1) ^ 1);
+        const uint32_t full = tc::smem_u32(&bar_full[s]);
+        tc::mbar_arrive_expect_tx(full, 2 * L * TILE_BYTES);
+        const uint32_t base = smem0 + s * STAGE_BYTES;
+        for (int a = 0; a < L; ++a) {
+          tc::tma_load_3d(base + a * TILE_BYTES, &tmap, full, i0, it * KS, z * 3 + a);
+          tc::tma_load_3d(base + (MAXL + a) * TILE_BYTES, &tmap, full, j0, it * KS, z * 3 + a);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      constexpr uint32_t idesc = tc::idesc_i8(TM, TN, 1, 1, 1, 1);
+      uint32_t started = 0;   // bit s set once accumulator s holds data
+      for (int it = 0; it < p.n_iters; ++it) {
+        const int s = it % NSTAGE;
+        tc::mbar_wait(tc::smem_u32(&bar_full[s]), (it / NSTAGE) & 1);
+        tc::tc_fence_after();
+        const uint32_t base = smem0 + s * STAGE_BYTES;
+#pragma unroll
+        for (int kk = 0; kk < KS / 32; ++kk) {
+          for (int a = 0; a < L; ++a) {
+            const uint64_t da = tc::smem_desc(base + a * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+            for (int b = 0; b < L; ++b) {
+              const uint64_t db = tc::smem_desc(base + (MAXL + b) * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+              const int sidx = a + b;
+              tc::mma_i8(tmem + sidx * TN, da, db, idesc, (started >> sidx) & 1u);
+              started |= 1u << sidx;
+            }
+          }
+        }
+        tc::mma_commit(tc::smem_u32(&bar_empty[s]));     // stage free once these MMAs have read it
+      }
+      tc::mma_commit(tc::smem_u32(&bar_tmem));           // accumulators complete
+    }
+  } else {
+    // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp % 4) .. +31 =====
+    const int q = warp & 3;
+    tc::mbar_wait(tc::smem_u32(&bar_tmem), 0);
+    tc::tc_fence_after();
+    const int i = i0 + q * 32 + lane;
+    double* Arow = p.A + (long long)z * p.a_stride + (long long)i * p.ld;
+    const int nacc = 2 * L - 1;
+    for (int c0 = 0; c0 < TN; c0 += 16) {
+      uint32_t r[5][16];
+#pragma unroll
+      for (int s = 0; s < 5; ++s)
+        if (s < nacc) tc::tmem_ld16(tmem + ((uint32_t)(q * 32) << 16) + s * TN + c0, r[s]);
+      tc::tmem_ld_wait();
+      if (i < p.F) {
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+          const int j = j0 + c0 + e;
+          if (j < p.F) {
+            long long g = 0;
+#pragma unroll
+            for (int s = 4; s >= 0; --s)
+              if (s < nacc) g = g * 256 + (long long)(int32_t)r[s][e];
+            double v = (double)g;
+            if (i == j) v += p.lam;
+            Arow[j] = v;
+          }
+        }
+      }
+    }
+    tc::tc_fence_before();
+  }
+  __syncthreads();
+  if (warp == 1) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, TMEM_COLS); }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+}  // namespace
+
+// ---- host side --------------------------------------------------------------------------------------
+int64_t lb_gram_tc_fp(int64_t F) { return lb_align_up(F, 16); }
+
+bool lb_gram_tc_usable(int64_t n, int64_t F) { return n >= 1 && n <= 43690 && F >= 1 && F < (1 << 30); }
+
+size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand) {
+  return (size_t)lb_align_up((int64_t)n_cand * 3 * n * lb_gram_tc_fp(F), 256) + (size_t)lb_align_up((int64_t)n_cand * 4, 256);
+}
+
+// A[z] (lower triangle, fp64, leading dimension ld) = U[z]^T U[z] + lam I for integer-valued U, |U| < 2^23
+int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
+                      long long a_stride, long long ld, cudaStream_t st) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return LBCNN_ERR_CUDA;
+  const int64_t Fp = lb_gram_tc_fp(F);
+  int8_t* planes = reinterpret_cast<int8_t*>(ws);
+  int32_t* nlimb = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + lb_align_up((int64_t)n_cand * 3 * n * Fp, 256));
+  fill_i32_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(nlimb, n_cand, 1);
+  h->launches += 1;
+  {
+    const long long work = n * (Fp / 16);
+    dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
+    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb);
+    h->launches += 1;
+  }
+  LB_CUDA_OK(cudaGetLastError());
+  CUtensorMap tmap;
+  const cuuint64_t gdim[3] = {(cuuint64_t)F, (cuuint64_t)n, (cuuint64_t)n_cand * 3};
+  const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)n * Fp};
+  const cuuint32_t box[3] = {BOXW, KS, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, planes, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return LBCNN_ERR_CUDA;
+  GramTcParams p{};
+  p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld;
+  p.F = (int)F; p.n = (int)n; p.n_iters = (int)((n + KS - 1) / KS); p.lam = lam;
+  const size_t smem = (size_t)NSTAGE * STAGE_BYTES + 1024;
+  LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  dim3 grid((unsigned)((F + TN - 1) / TN), (unsigned)((F + TM - 1) / TM), (unsigned)n_cand);
+  gram_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmap, p);
+  h->launches += 1;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}

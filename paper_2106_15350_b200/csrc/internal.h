@@ -62,12 +62,19 @@ struct FitPlan {
   int64_t dim;           // system dimension
   int64_t rows;          // dim + n_classes (right-hand sides appended as rows)
   size_t a_bytes;        // per candidate: rows * dim doubles
-  size_t perm_off, off_off, a_off, total; // offsets inside the fit workspace
+  size_t perm_off, off_off, a_off, tc_off, total; // offsets inside the fit workspace
+  int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
 };
 void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p);
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_H, int64_t n, int64_t F, float h_scale,
                   const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
                   cudaStream_t st);
+
+// ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
+bool lb_gram_tc_usable(int64_t n, int64_t F);
+size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand);
+int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
+                      long long a_stride, long long ld, cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,

@@ -305,3 +305,34 @@ def test_full_size_bench_config_sampled(handle):
         assert abs(co / w.n_test - acc[k]) * 100.0 <= TOL_ACC_PP
         if k == best:
             assert _fro(out["W_best"].cpu().numpy().astype(np.float64), Wo) <= TOL_W_FRO
+
+
+# ---- exact integer Gram on the tensor cores (gram_tc.cu) -------------------------------------------------
+TC_CASES = [  # n, F, c, max_abs, K : digits 1 / 2 / 3, ragged n (not a multiple of 64) and F (not of 16 / 96 / 128)
+    (300, 70, 5, 100, 2), (1000, 200, 7, 30000, 3), (777, 333, 4, 900000, 2), (2049, 129, 3, 8000000, 1),
+    (130, 97, 3, 20000, 2), (5000, 980, 10, 16000, 1)]
+
+
+@pytest.mark.parametrize("n,F,c,amax,K", TC_CASES)
+def test_integer_fit_tensor_core_gram_is_exact(handle, n, F, c, amax, K):
+    """LBCNN_H_INTEGER routes the Gram through tcgen05 int8 digit planes; it must reproduce the fp64 SIMT
+    Gram (flags = 0) exactly -- both are exact for integer data -- and the oracle's W within tolerance."""
+    rng = np.random.default_rng(n * 131 + F)
+    # low-rank + noise integer features with a common mode (ill-conditioned like the expander's output)
+    base = rng.integers(-amax // 4, amax // 4, size=(K, 1, F))
+    H = (base + rng.integers(-amax // 2, amax // 2, size=(K, n, F))).astype(np.float32)
+    H[0, 0, 0] = float(amax - 1)
+    H[0, 1, min(1, F - 1)] = float(-(amax - 1))
+    y = rng.integers(0, c, size=n).astype(np.int32)
+    s, Creg = 1.0 / 255.0, 1e3
+    Hd, yd = _dev(H), _dev(y)
+    handle.set_workspace(None)
+    handle.ensure_workspace(64 << 20 if n * F < 3e5 else 1 << 30)
+    W_tc, info_tc = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=lb.H_INTEGER)
+    W_ref, info_ref = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=0)
+    torch.cuda.synchronize()
+    assert (info_tc.cpu().numpy() == 0).all() and (info_ref.cpu().numpy() == 0).all()
+    assert torch.equal(W_tc, W_ref)
+    sc = float(np.float32(s))
+    Wo, inf, _ = orc.elm_fit(H[0].astype(np.float64) * sc, y, c, Creg)
+    assert inf == 0 and _fro(W_tc[0].cpu().numpy().astype(np.float64), Wo) <= TOL_W_FRO
