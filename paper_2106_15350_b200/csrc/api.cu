@@ -2,6 +2,7 @@
 // planning and the search driver.  All compute is in expand.cu / fit.cu / score.cu; there is no CPU path.
 #include "internal.h"
 #include <new>
+#include <stdlib.h>
 
 // ---- host shape logic -------------------------------------------------------------------------
 // pooling output size (PAPER.md:54 max_pooling_2d(ksize, stride, pad, cover_all=True); PAPER.md:104 28->14->7)
@@ -81,6 +82,8 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device));
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
+  const char* fs = getenv("LBCNN_FORCE_SIMT_EXPAND");
+  p->force_simt_expand = (fs && fs[0] == '1') ? 1 : 0;
   *h = p;
   return LBCNN_OK;
 }

@@ -180,6 +180,8 @@ __global__ void __launch_bounds__(256) expand_kernel(const ExpandParams p) {
 
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, cudaStream_t st) {
+  if (!h->force_simt_expand && lb_expand_tc_usable(h, s, d_bias != nullptr))
+    return lb_launch_expand_tc(h, s, feature_scale, d_images, n, d_kernels, n_cand, d_H, st);
   LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
   ExpandParams p{};
   p.n_layers = s.n_layers;

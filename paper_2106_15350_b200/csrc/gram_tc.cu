@@ -30,8 +30,8 @@ constexpr int KS = 64;         // samples per pipeline stage (two K = 32 MMA ste
 constexpr int BOXW = 128;      // TMA box width in features (= bytes): one 128-byte swizzle row
 constexpr int TILE_BYTES = KS * BOXW;          // 8 KB per digit plane per operand per stage
 constexpr int MAXL = 3;
-constexpr int STAGE_BYTES = 2 * MAXL * TILE_BYTES;   // 48 KB
-constexpr int NSTAGE = 4;
+constexpr int RING_BYTES = 24 * TILE_BYTES;   // 192 KB of operand stages: 12 / 6 / 4 stages for 1 / 2 / 3 digits
+constexpr int MAXSTAGE = 12;
 constexpr int TMEM_COLS = 512; // 5 accumulators x 96 columns = 480
 constexpr int NTHREADS = 192;
 
@@ -43,31 +43,29 @@ struct GramTcParams {
 };
 
 // ---- digit split ----------------------------------------------------------------------------------
-// thread = 16 consecutive features of one sample of one candidate
+// thread = 4 consecutive features of one sample of one candidate: one coalesced float4 load, one 32-bit
+// store per digit plane (a warp writes 128 contiguous bytes per plane)
 __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
                                                     int8_t* __restrict__ planes, int32_t* __restrict__ nlimb) {
   const int z = blockIdx.y;
-  const long long chunks_per_row = Fp / 16;
+  const long long quads_per_row = Fp / 4;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int need = 1;
-  if (t < n * chunks_per_row) {
-    const long long row = t / chunks_per_row;
-    const int f0 = (int)(t % chunks_per_row) * 16;
+  if (t < n * quads_per_row) {
+    const long long row = t / quads_per_row;
+    const int f0 = (int)(t % quads_per_row) * 4;
     const float* src = U + ((long long)z * n + row) * F + f0;
-    int v[16];
-    if ((F & 3) == 0 && f0 + 16 <= F) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float4 x = *reinterpret_cast<const float4*>(src + 4 * q);
-        v[4 * q] = (int)x.x; v[4 * q + 1] = (int)x.y; v[4 * q + 2] = (int)x.z; v[4 * q + 3] = (int)x.w;
-      }
+    int v[4];
+    if ((F & 3) == 0 && f0 + 4 <= F) {
+      const float4 x = __ldcs(reinterpret_cast<const float4*>(src));
+      v[0] = (int)x.x; v[1] = (int)x.y; v[2] = (int)x.z; v[3] = (int)x.w;
     } else {
 #pragma unroll
-      for (int q = 0; q < 16; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
+      for (int q = 0; q < 4; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
     }
-    uint32_t w[3][4] = {};
+    uint32_t w[3] = {0, 0, 0};
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
+    for (int q = 0; q < 4; ++q) {
       const int u = v[q];
       const int d0 = ((u + 128) & 255) - 128;
       const int u1 = (u - d0) >> 8;
@@ -75,14 +73,14 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
       const int d2 = (u1 - d1) >> 8;
       if (u1 != 0) need = max(need, 2);
       if (d2 != 0) need = max(need, 3);
-      w[0][q >> 2] |= (uint32_t)(d0 & 255) << (8 * (q & 3));
-      w[1][q >> 2] |= (uint32_t)(d1 & 255) << (8 * (q & 3));
-      w[2][q >> 2] |= (uint32_t)(d2 & 255) << (8 * (q & 3));
+      w[0] |= (uint32_t)(d0 & 255) << (8 * q);
+      w[1] |= (uint32_t)(d1 & 255) << (8 * q);
+      w[2] |= (uint32_t)(d2 & 255) << (8 * q);
     }
 #pragma unroll
     for (int l = 0; l < 3; ++l) {
       int8_t* dst = planes + (((long long)z * 3 + l) * n + row) * Fp + f0;
-      *reinterpret_cast<uint4*>(dst) = make_uint4(w[l][0], w[l][1], w[l][2], w[l][3]);
+      *reinterpret_cast<uint32_t*>(dst) = w[l];
     }
   }
   need = __reduce_max_sync(0xffffffffu, need);
@@ -102,11 +100,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // 1024-byte alignment for the 128-byte swizzle atoms
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  __shared__ __align__(8) uint64_t bar_full[NSTAGE], bar_empty[NSTAGE], bar_tmem;
+  __shared__ __align__(8) uint64_t bar_full[MAXSTAGE], bar_empty[MAXSTAGE], bar_tmem;
   __shared__ uint32_t tmem_base_s;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int L = p.nlimb[z];
+  const int STAGE_BYTES = 2 * L * TILE_BYTES;
+  const int NSTAGE = 12 / L;
   const uint32_t smem0 = tc::smem_u32(smem);
 
   if (warp == 0 && lane == 0) {
@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
         const uint32_t base = smem0 + s * STAGE_BYTES;
         for (int a = 0; a < L; ++a) {
           tc::tma_load_3d(base + a * TILE_BYTES, &tmap, full, i0, it * KS, z * 3 + a);
-          tc::tma_load_3d(base + (MAXL + a) * TILE_BYTES, &tmap, full, j0, it * KS, z * 3 + a);
+          tc::tma_load_3d(base + (L + a) * TILE_BYTES, &tmap, full, j0, it * KS, z * 3 + a);
         }
       }
     }
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
           for (int a = 0; a < L; ++a) {
             const uint64_t da = tc::smem_desc(base + a * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
             for (int b = 0; b < L; ++b) {
-              const uint64_t db = tc::smem_desc(base + (MAXL + b) * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+              const uint64_t db = tc::smem_desc(base + (L + b) * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
               const int sidx = a + b;
               tc::mma_i8(tmem + sidx * TN, da, db, idesc, (started >> sidx) & 1u);
               started |= 1u << sidx;
@@ -235,7 +235,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   fill_i32_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(nlimb, n_cand, 1);
   h->launches += 1;
   {
-    const long long work = n * (Fp / 16);
+    const long long work = n * (Fp / 4);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
     split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb);
     h->launches += 1;
@@ -252,7 +252,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   GramTcParams p{};
   p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld;
   p.F = (int)F; p.n = (int)n; p.n_iters = (int)((n + KS - 1) / KS); p.lam = lam;
-  const size_t smem = (size_t)NSTAGE * STAGE_BYTES + 1024;
+  const size_t smem = (size_t)RING_BYTES + 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   dim3 grid((unsigned)((F + TN - 1) / TN), (unsigned)((F + TM - 1) / TM), (unsigned)n_cand);
   gram_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmap, p);

@@ -16,6 +16,7 @@ struct lbcnn_handle_s {
   void* ws;
   size_t ws_bytes;
   int64_t launches;
+  int force_simt_expand;            // testing: keep the expander on the SIMT kernel (LBCNN_FORCE_SIMT_EXPAND=1)
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
 };
@@ -55,6 +56,11 @@ int lb_arch_shape(const lbcnn_arch_t* a, ArchShape* s);
 // ---- expander (expand.cu) ------------------------------------------------------------------
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, cudaStream_t st);
+
+// tensor-core expander (expand_tc.cu): FULL convolutions, non-overlapping pooling, 1-2 layers, no bias
+bool lb_expand_tc_usable(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias);
+int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
+                        const int8_t* d_kernels, int n_cand, float* d_H, cudaStream_t st);
 
 // ---- fit (fit.cu) --------------------------------------------------------------------------
 struct FitPlan {
