@@ -81,7 +81,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   p->device = device;
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device));
   LB_CUDA_OK(cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
-  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
+  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0; p->xw = nullptr; p->xw_bytes = 0;
   const char* fs = getenv("LBCNN_FORCE_SIMT_EXPAND");
   p->force_simt_expand = (fs && fs[0] == '1') ? 1 : 0;
   *h = p;
@@ -112,6 +112,7 @@ int lbcnn_get_phase_times(lbcnn_handle_t h, float* h_ms, int32_t* h_count) {
 int lbcnn_destroy(lbcnn_handle_t h) {
   if (!h) return LBCNN_ERR_INVALID_ARG;
   for (LbPhaseRec& r : h->recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
+  if (h->xw) cudaFree(h->xw);
   delete h;
   return LBCNN_OK;
 }

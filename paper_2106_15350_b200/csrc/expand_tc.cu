@@ -1,320 +1,582 @@
 // expand_tc.cu -- K1 on the tensor pipe: the LB-CNN expander for FULL convolutions with
 // non-overlapping pooling, as exact integer implicit GEMMs on tcgen05.mma kind::i8 (int32 accumulators in TMEM).
 //
-// Layer 1 (Cin = 1..3 channels of uint8 pixels): explicit im2col rows [position][k*k*Cin -> 32 bytes] built in
-// shared memory, one set of rows per POOL PHASE (py,px); u8 x s8 -> s32 MMAs with M = 128 pooled positions,
-// N = 16 output channels, K = 32.  The pool is then an element-wise max over the P*P phase accumulators in the
-// SAME TMEM lane -- no shuffles ("Nonlinearity achieved in Max-pool").
-// Layer 2 (Cin = layer-1 channels, values up to +-8159): the pooled layer-1 map is written to shared memory
-// as balanced radix-64 digits v = lo + 64 hi (both int8), split into P*P phase planes
-// plane[sy][sx](i,j) = a[P i + sy][P j + sx] with a shared zero halo.  For output phase (py,px) and tap (dy,dx)
-// the A operand is a plane shifted by a constant number of positions, i.e. just a different start address of a
-// K-major no-swizzle descriptor ("tap-shifted implicit GEMM"): 9 taps accumulate into one TMEM accumulator,
-// weights are +-1 (lo digits) and +-64 (hi digits) in the same int8 B operand, so the int32 result is the exact
-// convolution.  Pool = max over the phase accumulators again; flatten C,H,W; one multiply by feature_scale.
+// Layer 1 ("patch GEMM").  A pooled output position (i,j) sees a (P+k-1)^2 x Cin patch of uint8 pixels; all P*P
+// conv outputs under its pooling window are linear in that one patch.  A1 = [pooled position][patch bytes]
+// (built ONCE per CTA in shared memory, shared by every candidate), B1 = [patch byte][o * P*P + phase] holds the
+// candidate's +-1 taps shifted per pool phase (zero elsewhere): one u8 x s8 -> s32 MMA chain per 128 positions
+// gives every pre-pool value of the tile, the pool is a max over P*P adjacent TMEM columns of the thread's own
+// lane -- no shuffles ("Nonlinearity achieved in Max-pool").
+// Layer 2 ("tap-shifted implicit GEMM").  The pooled layer-1 map (|v| < 8192) is written to shared memory as
+// two int8 digits v = 64 hi + lo (lo = v & 63, hi = v >> 6), split into P2*P2 phase planes
+// plane[sy][sx](i,j) = a[P2 i + sy][P2 j + sx] that share one zero halo.  For output phase (py,px) and tap
+// (dy,dx) the A operand is a plane shifted by a constant number of positions = a different start address of a
+// K-major no-swizzle descriptor; the k*k taps accumulate into one TMEM accumulator, the B operand holds +-1
+// (lo digits) and +-64 (hi digits), so the int32 result is the exact convolution.  Pool = max over the phase
+// accumulators; flatten C,H,W; one multiply by feature_scale; H written once.
 //
-// CTA = a batch of B images x a range of candidates, 128 threads (thread t owns TMEM lane t), thread 0 issues
-// the MMAs; tcgen05.commit -> mbarrier hands accumulators to the epilogue.  Two CTAs are resident per SM
-// (<= 256 TMEM columns, ~100 KB shared memory each) so one CTA's epilogue overlaps the other's MMAs.
+// One CTA = a batch of B images x a range of candidates, 18 warps, warp specialised, everything handed over
+// through mbarriers so that the tensor pipe, the TMEM reads and the ALU epilogues of neighbouring candidates overlap:
+//   warp 0      layer-1 MMA issuer (+ bulk-copy of the candidate's prepared B1)    -> accumulator ring R1
+//   warp 1      layer-2 MMA issuer (+ bulk-copy of B2), waits for the planes       -> accumulator ring R2
+//   warps 2-9   E1: R1 -> max-pool -> digits -> phase planes (double buffered) [single layer: -> H, 16 warps]
+//   warps 10-17 E2: R2 -> max-pool -> scale -> H
+// The +-1 kernel sets are re-laid-out once per launch by a small kernel into the exact shared-memory images of
+// B1 / B2 (handle-owned scratch), so the hot loop stages them with one cp.async.bulk each.
+// Measured on B200: an MMA with M = 128 reads (128 + N) x 32 operand bytes from shared memory at 128 B/clk, so
+// these small-N MMAs are bound by shared-memory bandwidth (32 + N/4 clk), not by the tensor pipe (N/2 clk).
 // Anything outside this kernel's envelope (depthwise, overlapping / padded / cover_all pooling, bias, three
 // layers, wide layers) takes the exact SIMT kernel in expand.cu.
 #include "internal.h"
 #include "tc_common.cuh"
+#include <stdio.h>
+#include <stdlib.h>
 
 namespace {
 
+constexpr int XT_WARPS = 18;
+constexpr int XT_THREADS = XT_WARPS * 32;
+
 struct XtcParams {
   const uint8_t* img; long long n_img; int H, W, C;
-  const int8_t* ker; int n_weights; int n_cand, cand_per_cta;
+  const uint8_t* wblob; int blob_bytes, w1_bytes, w2_bytes;   // per candidate: [B1 image | B2 image]
+  int n_cand, cand_per_cta;
   float* Hout; long long F; float scale;
   int n_layers;
   // layer 1
-  int k1, pd1, P1, Cout1, K1, K1p, Ho1, Wo1, act1, w1_off;
+  int k1, pd1, P1, nph1, Cout1, Cp1, N1, K1, K1p, Pk1, Ho1, Wo1, act1;
   // layer 2
-  int k2, pd2, P2, Cout2, Ho2, Wo2, act2, w2_off, Wq, Hq, base0, NPOS2, N2;
-  int B, NP1, T1, NM2, T2, cache;
+  int k2, pd2, P2, nph2, Cout2, N2, Ho2, Wo2, act2, Wq, Hq, base0, NPOS2;
+  int B, NP1, NP1p, T1, NM2, T2, NPB, lg_nslot1;
   // shared-memory offsets (bytes)
-  int off_img, off_w1, off_w2, off_col, off_pl, col_slot_bytes, plane_bytes;
+  int off_img, off_a1, off_w1, off_w2, off_pl, off_tab1, off_tab2, plane_bytes, plbuf_bytes;
+  // TMEM column offsets
+  int tm_r1, tm_r2;
 };
+
+// barrier slots
+enum { W1_FULL = 0, W1_EMPTY = 2, W2_FULL = 4, W2_EMPTY = 7, R1_FULL = 10, R1_EMPTY = 14, PL_FULL = 18, PL_EMPTY = 20,
+       R2_FULL = 22, R2_EMPTY = 24, N_BARS = 26 };
+
+// ---- kernel sets -> shared-memory images of the B operands ---------------------------------------------------
+// B1: K-major no-swizzle [16-byte K chunk kc][column n][16 B], K index kk = (c*Pk + yy)*Pk + xx over the patch,
+//     column n = o*nph1 + (py*P1 + px):  w1[o][c][yy-py][xx-px] where that tap exists, else 0.
+// B2: per tap [chunk 0: lo digits | chunk 1: hi digits][column o][16 B = input channel]: w2[o][c][tap], 64 w2[o][c][tap].
+struct PrepParams {
+  const int8_t* ker; int n_weights; uint8_t* blob; int blob_bytes, w1_bytes, n_layers;
+  int k1, P1, nph1, Cout1, N1, K1, K1p, Pk1, Cin1, w1_off;
+  int k2, Cout2, N2, w2_off;
+};
+__global__ void __launch_bounds__(256) xtc_prep_kernel(const PrepParams p) {
+  const int cand = blockIdx.y;
+  const int8_t* kw = p.ker + (long long)cand * p.n_weights;
+  uint8_t* out = p.blob + (long long)cand * p.blob_bytes;
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < p.blob_bytes; t += gridDim.x * blockDim.x) {
+    int v = 0;
+    if (t < p.w1_bytes) {
+      const int kb = t & 15, n = (t >> 4) % p.N1, kc = (t >> 4) / p.N1;
+      const int kk = kc * 16 + kb;
+      const int o = n / p.nph1, ph = n - o * p.nph1;
+      if (kk < p.K1 && o < p.Cout1) {
+        const int pk2 = p.Pk1 * p.Pk1;
+        const int c = kk / pk2, r = kk - c * pk2;
+        const int yy = r / p.Pk1, xx = r - yy * p.Pk1;
+        const int py = ph / p.P1, px = ph - py * p.P1;
+        const int dy = yy - py, dx = xx - px;
+        if (dy >= 0 && dy < p.k1 && dx >= 0 && dx < p.k1) v = kw[p.w1_off + ((o * p.Cin1 + c) * p.k1 + dy) * p.k1 + dx];
+      }
+    } else if (p.n_layers == 2) {
+      const int u = t - p.w1_bytes;
+      const int c = u & 15, o = (u >> 4) % p.N2, half = ((u >> 4) / p.N2) & 1, tap = (u >> 4) / (2 * p.N2);
+      if (o < p.Cout2 && c < p.Cout1) {
+        v = kw[p.w2_off + (o * p.Cout1 + c) * (p.k2 * p.k2) + tap];
+        if (half) v *= 64;
+      }
+    }
+    out[t] = (uint8_t)(int8_t)v;
+  }
+}
 
 __device__ __forceinline__ int floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 
-__global__ void __launch_bounds__(128, 2) expand_tc_kernel(const XtcParams p) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ __align__(8) uint64_t bar;
-  __shared__ uint32_t tmem_base_s;
-  const int tid = threadIdx.x, warp = tid >> 5;
-  const long long img0 = (long long)blockIdx.x * p.B;
-  const int nb = (int)min((long long)p.B, p.n_img - img0);         // images really present in this batch
-  const int c_begin = blockIdx.y * p.cand_per_cta;
-  const int c_end = min(c_begin + p.cand_per_cta, p.n_cand);
-  const uint32_t s_base = tc::smem_u32(smem);
-  const uint32_t bar_a = tc::smem_u32(&bar);
-
-  if (tid == 0) { tc::mbar_init(bar_a, 1); tc::fence_barrier_init(); }
-  __syncwarp();
-  if (warp == 0) tc::tmem_alloc(tc::smem_u32(&tmem_base_s), 256);
-  // raw images of the batch -> shared memory (zero for images beyond n_img); zero the layer-2 planes once
-  {
-    const int npx = p.H * p.W * p.C;
-    const uint8_t* src = p.img + img0 * npx;
-    for (int t = tid; t < p.B * npx; t += 128) smem[p.off_img + t] = (t < nb * npx) ? src[t] : (uint8_t)0;
-    if (p.n_layers == 2) {
-      uint4* pl = reinterpret_cast<uint4*>(smem + p.off_pl);
-      const int n16 = p.P2 * p.P2 * p.plane_bytes / 16;
-      for (int t = tid; t < n16; t += 128) pl[t] = make_uint4(0, 0, 0, 0);
-    }
+// max over NPH adjacent columns for each of the 16 / NPH channels of one 16-column group
+template <int NPH>
+__device__ __forceinline__ void pool_group(const uint32_t (&r)[16], int* mx) {
+#pragma unroll
+  for (int q = 0; q < 16 / NPH; ++q) {
+    int m = (int)r[q * NPH];
+#pragma unroll
+    for (int ph = 1; ph < NPH; ++ph) m = max(m, (int)r[q * NPH + ph]);
+    mx[q] = m;
   }
-  tc::tc_fence_before();
-  __syncthreads();
-  tc::tc_fence_after();
-  const uint32_t tmem = tmem_base_s;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-  uint32_t parity = 0;
+}
 
-  constexpr uint32_t IDESC1 = tc::idesc_i8(128, 16, 0, 1, 0, 0);   // u8 pixels x s8 weights, K-major both
-  const uint32_t idesc2 = tc::idesc_i8(128, p.N2, 1, 1, 0, 0);
-  const int nph1 = p.P1 * p.P1;
-  const int plane1 = p.Ho1 * p.Wo1;
+__device__ __forceinline__ uint32_t bar_addr(const uint64_t* bars, int i) { return tc::smem_u32(bars + i); }
 
-  for (int cand = c_begin; cand < c_end; ++cand) {
-    const int8_t* kw = p.ker + (long long)cand * p.n_weights;
-    // ---- weights of this candidate -> B operands (K-major, no swizzle: [16-byte K chunk][row][16 B]) ----
-    {
-      // layer 1: row o (16 rows), K index = (c*k + dy)*k + dx -- the kernel set's own order
-      for (int t = tid; t < 16 * p.K1p; t += 128) {
-        const int o = t / p.K1p, kk = t % p.K1p;
-        const int8_t v = (o < p.Cout1 && kk < p.K1) ? kw[p.w1_off + o * p.K1 + kk] : (int8_t)0;
-        smem[p.off_w1 + (kk >> 4) * 256 + o * 16 + (kk & 15)] = (uint8_t)v;
-      }
-      if (p.n_layers == 2) {
-        // layer 2, per tap: rows o (N2), chunk 0 = +-1 on the lo digits of channel c, chunk 1 = +-64 on the hi digits
-        const int kk2 = p.k2 * p.k2, cin2 = p.Cout1;
-        for (int t = tid; t < kk2 * p.N2 * 16; t += 128) {
-          const int c = t & 15, o = (t >> 4) % p.N2, tap = (t >> 4) / p.N2;
-          int v = 0;
-          if (o < p.Cout2 && c < cin2) v = kw[p.w2_off + (o * cin2 + c) * kk2 + tap];
-          uint8_t* dst = smem + p.off_w2 + tap * (p.N2 * 32) + o * 16 + c;
-          dst[0] = (uint8_t)(int8_t)v;
-          dst[p.N2 * 16] = (uint8_t)(int8_t)(64 * v);
-        }
-      }
-    }
-    // ---- layer 1: tiles of 128 pooled positions ----
+// ---- E1, two layers: R1 -> max-pool -> (relu) -> digits -> phase planes of layer 2 --------------------------------
+// tab1[m] = byte offset of pooled position m inside one plane buffer (phase plane + halo-sharing position), -1 = none
+template <int NPH>
+__device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, const uint64_t* bars, uint32_t tmem,
+                                             int set, int quad, int lane, int n_cta_cand) {
+  constexpr int CPG = 16 / NPH;          // channels per 16-column group
+  const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
+  const int mask = (1 << p.lg_nslot1) - 1;
+  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
+  const uint32_t taddr = tmem + lane_base + p.tm_r1 + set * p.N1;
+  for (int ci = 0; ci < n_cta_cand; ++ci) {
+    const int buf = (p.NPB == 2) ? (ci & 1) : 0;
+    const int use = (p.NPB == 2) ? (ci >> 1) : ci;
+    bool waited = false;
     for (int t1 = 0; t1 < p.T1; ++t1) {
-      const int slot = p.cache ? t1 : 0;
-      const int m1 = t1 * 128 + tid;
-      const bool in_range = m1 < p.NP1;
-      const int b = in_range ? m1 / plane1 : 0;
-      const int rem = in_range ? m1 - b * plane1 : 0;
-      const int i1 = rem / p.Wo1, j1 = rem - i1 * p.Wo1;
-      if (!p.cache || cand == c_begin) {
-        // im2col row of this thread's position for every pool phase: K1p bytes = k*k*Cin pixels, zero padded
-        const uint8_t* im = smem + p.off_img + b * (p.H * p.W * p.C);
-        for (int ph = 0; ph < nph1; ++ph) {
-          const int py = ph / p.P1, px = ph - py * p.P1;
-          const int y0 = p.P1 * i1 + py - p.pd1, x0 = p.P1 * j1 + px - p.pd1;
-          uint8_t* dst = smem + p.off_col + slot * p.col_slot_bytes + ph * (p.K1p * 128) + tid * 16;
-          for (int q = 0; q < p.K1p / 16; ++q) {
-            uint32_t w[4] = {0, 0, 0, 0};
-            if (in_range) {
-#pragma unroll 4
-              for (int e = 0; e < 16; ++e) {
-                const int kk = q * 16 + e;
-                if (kk < p.K1) {
-                  const int c = kk / (p.k1 * p.k1), r2 = kk - c * (p.k1 * p.k1);
-                  const int dy = r2 / p.k1, dx = r2 - dy * p.k1;
-                  const int y = y0 + dy, x = x0 + dx;
-                  if (y >= 0 && y < p.H && x >= 0 && x < p.W)
-                    w[e >> 2] |= (uint32_t)im[(y * p.W + x) * p.C + c] << (8 * (e & 3));
-                }
-              }
-            }
-            *reinterpret_cast<uint4*>(dst + q * 2048) = make_uint4(w[0], w[1], w[2], w[3]);
-          }
-        }
-      }
-      tc::fence_proxy_async();      // generic-proxy smem writes (im2col, weights, planes) -> visible to the MMA
-      tc::tc_fence_before();
-      __syncthreads();
-      if (tid == 0) {
-        tc::tc_fence_after();
-        for (int ph = 0; ph < nph1; ++ph) {
-          const uint32_t a0 = s_base + p.off_col + slot * p.col_slot_bytes + ph * (p.K1p * 128);
-          for (int ks = 0; ks < p.K1p / 32; ++ks) {
-            const uint64_t da = tc::smem_desc(a0 + ks * 4096, 2048, 128, tc::LAYOUT_NONE);
-            const uint64_t db = tc::smem_desc(s_base + p.off_w1 + ks * 512, 256, 128, tc::LAYOUT_NONE);
-            tc::mma_i8(tmem + ph * 16, da, db, IDESC1, ks > 0);
-          }
-        }
-        tc::mma_commit(bar_a);
-      }
-      tc::mbar_wait(bar_a, parity);
-      parity ^= 1;
+      const int n1 = ci * p.T1 + t1;
+      if ((n1 & mask) != set) continue;
+      tc::mbar_wait(bar_addr(bars, R1_FULL + set), (n1 >> p.lg_nslot1) & 1);
       tc::tc_fence_after();
-      // epilogue 1: pool = max over the phase accumulators of this lane
       int mx[16];
 #pragma unroll
-      for (int e = 0; e < 16; ++e) mx[e] = INT_MIN;
-      for (int ph = 0; ph < nph1; ++ph) {
-        uint32_t r[16];
-        tc::tmem_ld16(tmem + lane_base + ph * 16, r);
-        tc::tmem_ld_wait();
+      for (int e = 0; e < 16; ++e) mx[e] = 0;
 #pragma unroll
-        for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], (int)r[e]);
-      }
-      if (p.act1 == LBCNN_ACT_RELU) {
+      for (int gb = 0; gb < NPH; gb += 4) {
+        if (gb * 16 < p.N1) {
+          uint32_t r[4][16];
 #pragma unroll
-        for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], 0);
-      }
-      if (p.n_layers == 1) {
-        if (in_range && b < nb) {
-          float* Hrow = p.Hout + ((long long)cand * p.n_img + img0 + b) * p.F;
+          for (int q = 0; q < 4; ++q)
+            if (gb + q < NPH && (gb + q) * 16 < p.N1) tc::tmem_ld16(taddr + (gb + q) * 16, r[q]);
+          tc::tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 16; ++e)
-            if (e < p.Cout1) Hrow[(e * p.Ho1 + i1) * p.Wo1 + j1] = p.scale * (float)mx[e];
+          for (int q = 0; q < 4; ++q)
+            if (gb + q < NPH && (gb + q) * 16 < p.N1) pool_group<NPH>(r[q], &mx[(gb + q) * CPG]);
         }
-      } else if (in_range) {
-        // balanced radix-64 digits of the pooled map -> phase plane (i1 % P2, j1 % P2) of layer 2
+      }
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + set));      // accumulator slot free again
+      if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; }
+      const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
+      if (off >= 0) {
         uint32_t lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-          const int v = mx[e];
-          const int l = ((v + 32) & 63) - 32;
-          const int h = (v - l) >> 6;
-          lo[e >> 2] |= (uint32_t)(l & 255) << (8 * (e & 3));
-          hi[e >> 2] |= (uint32_t)(h & 255) << (8 * (e & 3));
+          int v = mx[e];
+          if (p.act1 == LBCNN_ACT_RELU) v = max(v, 0);
+          lo[e >> 2] |= (uint32_t)(v & 63) << (8 * (e & 3));              // v = 64 (v >> 6) + (v & 63), both int8
+          hi[e >> 2] |= (uint32_t)((v >> 6) & 255) << (8 * (e & 3));
         }
-        const int sy = i1 % p.P2, sx = j1 % p.P2;
-        const int pos = p.base0 + (b * p.Hq + i1 / p.P2) * p.Wq + j1 / p.P2;
-        uint8_t* dst = smem + p.off_pl + (sy * p.P2 + sx) * p.plane_bytes + pos * 16;
+        uint8_t* dst = smem + p.off_pl + buf * p.plbuf_bytes + off;
         *reinterpret_cast<uint4*>(dst) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
         *reinterpret_cast<uint4*>(dst + p.NPOS2 * 16) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
       }
     }
-    if (p.n_layers == 1) continue;
-    // ---- layer 2: tiles of 128 positions of the (halo-sharing) pooled output grid ----
-    for (int t2 = 0; t2 < p.T2; ++t2) {
-      tc::fence_proxy_async();
-      tc::tc_fence_before();
-      __syncthreads();
-      if (tid == 0) {
-        tc::tc_fence_after();
-        for (int py = 0; py < p.P2; ++py)
-          for (int px = 0; px < p.P2; ++px) {
-            const uint32_t d = tmem + (py * p.P2 + px) * p.N2;
-            uint32_t acc = 0;
-            for (int dy = 0; dy < p.k2; ++dy) {
-              const int ry = py + dy - p.pd2, qy = floordiv(ry, p.P2), sy = ry - qy * p.P2;
-              for (int dx = 0; dx < p.k2; ++dx) {
-                const int rx = px + dx - p.pd2, qx = floordiv(rx, p.P2), sx = rx - qx * p.P2;
-                const uint32_t a_addr = s_base + p.off_pl + (sy * p.P2 + sx) * p.plane_bytes +
-                                        (p.base0 + t2 * 128 + qy * p.Wq + qx) * 16;
-                const uint64_t da = tc::smem_desc(a_addr, p.NPOS2 * 16, 128, tc::LAYOUT_NONE);
-                const uint64_t db = tc::smem_desc(s_base + p.off_w2 + (dy * p.k2 + dx) * (p.N2 * 32), p.N2 * 16, 128, tc::LAYOUT_NONE);
-                tc::mma_i8(d, da, db, idesc2, acc);
-                acc = 1;
+    if (!waited) tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1);   // never run ahead of the buffer's phase
+    tc::fence_proxy_async();                 // generic-proxy plane writes -> visible to the MMA's async proxy
+    __syncwarp();
+    if (lane == 0) tc::mbar_arrive(bar_addr(bars, PL_FULL + buf));
+  }
+}
+
+// ---- E1, single layer: R1 -> max-pool -> (relu) -> scale -> H -------------------------------------------------------
+// tab1[m] = b*F + i*Wo + j of pooled position m (flatten C,H,W adds o*Ho*Wo), -1 = none
+template <int NPH>
+__device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem,
+                                          int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
+  constexpr int CPG = 16 / NPH;
+  const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
+  const int mask = (1 << p.lg_nslot1) - 1;
+  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
+  const uint32_t taddr = tmem + lane_base + p.tm_r1 + set * p.N1;
+  const int G1 = p.N1 >> 4, hw = p.Ho1 * p.Wo1;
+  for (int ci = 0; ci < n_cta_cand; ++ci) {
+    float* Hc = p.Hout + ((long long)(c_begin + ci) * p.n_img + img0) * p.F;
+    for (int t1 = 0; t1 < p.T1; ++t1) {
+      const int n1 = ci * p.T1 + t1;
+      if ((n1 & mask) != set) continue;
+      tc::mbar_wait(bar_addr(bars, R1_FULL + set), (n1 >> p.lg_nslot1) & 1);
+      tc::tc_fence_after();
+      const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
+      for (int gb = 0; gb < G1; gb += 4) {
+        uint32_t r[4][16];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (gb + q < G1) tc::tmem_ld16(taddr + (gb + q) * 16, r[q]);
+        tc::tmem_ld_wait();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (gb + q < G1) {
+            int mx[CPG];
+            pool_group<NPH>(r[q], mx);
+#pragma unroll
+            for (int k = 0; k < CPG; ++k) {
+              const int o = (gb + q) * CPG + k;
+              if (off >= 0 && o < p.Cout1) {
+                int v = mx[k];
+                if (p.act1 == LBCNN_ACT_RELU) v = max(v, 0);
+                Hc[off + o * hw] = p.scale * (float)v;
               }
             }
           }
-        tc::mma_commit(bar_a);
+        }
       }
-      tc::mbar_wait(bar_a, parity);
-      parity ^= 1;
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + set));
+    }
+  }
+}
+
+// ---- E2: R2 -> max over the pool-phase accumulators -> (relu) -> scale -> H ------------------------------------------
+// tab2[m] = b*F + i*Wo2 + j of row m of the halo-sharing output grid, -1 = halo / beyond the batch
+__device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem, int set,
+                                       int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
+  const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
+  const int32_t* tab2 = reinterpret_cast<const int32_t*>(smem + p.off_tab2);
+  const uint32_t taddr = tmem + lane_base + p.tm_r2 + set * (p.nph2 * p.N2);
+  const int hw = p.Ho2 * p.Wo2;
+  for (int ci = 0; ci < n_cta_cand; ++ci) {
+    float* Hc = p.Hout + ((long long)(c_begin + ci) * p.n_img + img0) * p.F;
+    for (int t2 = 0; t2 < p.T2; ++t2) {
+      const int n2 = ci * p.T2 + t2;
+      if ((n2 & 1) != set) continue;
+      tc::mbar_wait(bar_addr(bars, R2_FULL + set), (n2 >> 1) & 1);
       tc::tc_fence_after();
-      const int m2 = t2 * 128 + tid;
-      const int b = m2 / (p.Hq * p.Wq);
-      const int rem = m2 - b * (p.Hq * p.Wq);
-      const int i2 = rem / p.Wq, j2 = rem - i2 * p.Wq;
-      const bool valid = (m2 < p.NM2) && (b < nb) && (i2 < p.Ho2) && (j2 < p.Wo2);
-      float* Hrow = p.Hout + ((long long)cand * p.n_img + img0 + (valid ? b : 0)) * p.F;
-      for (int c0 = 0; c0 < p.N2; c0 += 16) {
+      const int32_t off = tab2[t2 * 128 + quad * 32 + lane];
+      for (int c0 = 0; c0 < p.Cout2; c0 += 16) {
         int mx[16];
 #pragma unroll
         for (int e = 0; e < 16; ++e) mx[e] = INT_MIN;
-        for (int ph = 0; ph < p.P2 * p.P2; ++ph) {
-          uint32_t r[16];
-          tc::tmem_ld16(tmem + lane_base + ph * p.N2 + c0, r);
+        for (int ph0 = 0; ph0 < p.nph2; ph0 += 4) {
+          uint32_t r[4][16];
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (ph0 + q < p.nph2) tc::tmem_ld16(taddr + (ph0 + q) * p.N2 + c0, r[q]);
           tc::tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], (int)r[e]);
+          for (int q = 0; q < 4; ++q)
+            if (ph0 + q < p.nph2) {
+#pragma unroll
+              for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], (int)r[q][e]);
+            }
         }
-        if (valid) {
+        if (off >= 0) {
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
             const int o = c0 + e;
             if (o < p.Cout2) {
               int v = mx[e];
               if (p.act2 == LBCNN_ACT_RELU) v = max(v, 0);
-              Hrow[(o * p.Ho2 + i2) * p.Wo2 + j2] = p.scale * (float)v;     // flatten C,H,W
+              Hc[off + o * hw] = p.scale * (float)v;                       // flatten C,H,W
             }
           }
         }
       }
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R2_EMPTY + set));
     }
+  }
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParams p) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t bars[N_BARS];
+  __shared__ uint32_t tmem_base_s;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = tc::uniform_warp_id();
+  const long long img0 = (long long)blockIdx.x * p.B;
+  const int nb = (int)min((long long)p.B, p.n_img - img0);         // images really present in this batch
+  const int c_begin = blockIdx.y * p.cand_per_cta;
+  const int n_cta_cand = min(p.cand_per_cta, p.n_cand - c_begin);
+  const uint32_t s_base = tc::smem_u32(smem);
+  const int nslot1 = 1 << p.lg_nslot1;
+  const int n_e1_warps = 4 * nslot1;
+
+  if (tid == 0) {
+    for (int i = 0; i < N_BARS; ++i) {
+      int cnt = 1;
+      if (i >= R1_EMPTY && i < R1_EMPTY + 4) cnt = 4;
+      if (i >= R2_EMPTY && i < R2_EMPTY + 2) cnt = 4;
+      if (i >= PL_FULL && i < PL_FULL + 2) cnt = n_e1_warps;
+      tc::mbar_init(bar_addr(bars, i), cnt);
+    }
+    tc::fence_barrier_init();
+  }
+  if (warp == 0) tc::tmem_alloc(tc::smem_u32(&tmem_base_s), 512);
+  // ---- set-up shared by every candidate of this CTA ----
+  const int npx = p.H * p.W * p.C;
+  {
+    const uint8_t* src = p.img + img0 * npx;
+    const int total = p.B * npx, have = nb * npx;
+    if ((npx & 15) == 0) {          // every image (and so the batch) starts 16-byte aligned
+      const uint4* s4 = reinterpret_cast<const uint4*>(src);
+      uint4* d4 = reinterpret_cast<uint4*>(smem + p.off_img);
+      for (int t = tid; t < total / 16; t += XT_THREADS) d4[t] = (t * 16 < have) ? s4[t] : make_uint4(0, 0, 0, 0);
+    } else {
+      for (int t = tid; t < total; t += XT_THREADS) smem[p.off_img + t] = (t < have) ? src[t] : (uint8_t)0;
+    }
+    if (p.n_layers == 2) {
+      uint4* pl = reinterpret_cast<uint4*>(smem + p.off_pl);
+      const int n16 = p.NPB * p.plbuf_bytes / 16;
+      for (int t = tid; t < n16; t += XT_THREADS) pl[t] = make_uint4(0, 0, 0, 0);
+      // tab2: row m of the halo-sharing output grid -> b*F + i2*Wo2 + j2
+      int32_t* tab2 = reinterpret_cast<int32_t*>(smem + p.off_tab2);
+      for (int m = tid; m < p.T2 * 128; m += XT_THREADS) {
+        const int b = m / (p.Hq * p.Wq), rem = m - b * (p.Hq * p.Wq);
+        const int i2 = rem / p.Wq, j2 = rem - i2 * p.Wq;
+        const bool ok = (m < p.NM2) && (b < nb) && (i2 < p.Ho2) && (j2 < p.Wo2);
+        tab2[m] = ok ? (int32_t)(b * p.F + i2 * p.Wo2 + j2) : -1;
+      }
+    }
+    // tab1: pooled layer-1 position m -> plane offset (two layers) or b*F + i1*Wo1 + j1 (single layer)
+    int32_t* tab1 = reinterpret_cast<int32_t*>(smem + p.off_tab1);
+    const int plane1 = p.Ho1 * p.Wo1;
+    for (int m = tid; m < p.NP1p; m += XT_THREADS) {
+      int32_t v = -1;
+      if (m < p.NP1) {
+        const int b = m / plane1, rem = m - b * plane1;
+        const int i1 = rem / p.Wo1, j1 = rem - i1 * p.Wo1;
+        if (p.n_layers == 2) {
+          const int sy = i1 % p.P2, sx = j1 % p.P2;
+          const int pos = p.base0 + (b * p.Hq + i1 / p.P2) * p.Wq + j1 / p.P2;
+          v = (sy * p.P2 + sx) * p.plane_bytes + pos * 16;
+        } else if (b < nb) {
+          v = (int32_t)(b * p.F + i1 * p.Wo1 + j1);
+        }
+      }
+      tab1[m] = v;
+    }
+  }
+  __syncthreads();          // images in shared memory
+  {
+    // A1: [16-byte K chunk][pooled position][16 B]; K index = (c*Pk + yy)*Pk + xx over the (P+k-1)^2 x Cin patch
+    const int plane1 = p.Ho1 * p.Wo1, pk2 = p.Pk1 * p.Pk1;
+    const int nchunk = p.K1p / 16;
+    for (int t = tid; t < p.NP1p * nchunk; t += XT_THREADS) {
+      const int m = t % p.NP1p, kc = t / p.NP1p;
+      uint32_t w[4] = {0, 0, 0, 0};
+      if (m < p.NP1) {
+        const int b = m / plane1, rem = m - b * plane1;
+        const int i1 = rem / p.Wo1, j1 = rem - i1 * p.Wo1;
+        const uint8_t* im = smem + p.off_img + b * npx;
+        const int y0 = p.P1 * i1 - p.pd1, x0 = p.P1 * j1 - p.pd1;
+#pragma unroll 4
+        for (int e = 0; e < 16; ++e) {
+          const int kk = kc * 16 + e;
+          if (kk < p.K1) {
+            const int c = kk / pk2, r = kk - c * pk2;
+            const int yy = r / p.Pk1, xx = r - yy * p.Pk1;
+            const int y = y0 + yy, x = x0 + xx;
+            if (y >= 0 && y < p.H && x >= 0 && x < p.W) w[e >> 2] |= (uint32_t)im[(y * p.W + x) * p.C + c] << (8 * (e & 3));
+          }
+        }
+      }
+      *reinterpret_cast<uint4*>(smem + p.off_a1 + (kc * p.NP1p + m) * 16) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+  }
+  tc::fence_proxy_async();      // generic-proxy writes (A1, zeroed planes) -> visible to the MMA's async proxy
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp == 0) {
+    // ===== layer-1 issuer =====
+    const uint32_t idesc1 = tc::idesc_i8(128, p.N1, 0, 1, 0, 0);     // u8 pixels x s8 weights, K-major both
+    const int nks = p.K1p / 32;
+    const uint32_t lbo_a = (uint32_t)p.NP1p * 16, lbo_b = (uint32_t)p.N1 * 16;
+    int n1 = 0;
+    for (int ci = 0; ci < n_cta_cand; ++ci) {
+      if (ci == 0 && tc::elect_one()) {
+        tc::mbar_arrive_expect_tx(bar_addr(bars, W1_FULL), p.w1_bytes);
+        tc::bulk_load(s_base + p.off_w1, p.wblob + (long long)c_begin * p.blob_bytes, p.w1_bytes, bar_addr(bars, W1_FULL));
+      }
+      if (ci + 1 < n_cta_cand) {          // stage the next candidate's B1 while this one computes
+        const int slot = (ci + 1) & 1, use = (ci + 1) >> 1;
+        tc::mbar_wait(bar_addr(bars, W1_EMPTY + slot), (use & 1) ^ 1);
+        if (tc::elect_one()) {
+          tc::mbar_arrive_expect_tx(bar_addr(bars, W1_FULL + slot), p.w1_bytes);
+          tc::bulk_load(s_base + p.off_w1 + slot * p.w1_bytes, p.wblob + (long long)(c_begin + ci + 1) * p.blob_bytes, p.w1_bytes,
+                        bar_addr(bars, W1_FULL + slot));
+        }
+      }
+      tc::mbar_wait(bar_addr(bars, W1_FULL + (ci & 1)), (ci >> 1) & 1);
+      const uint32_t b_base = s_base + p.off_w1 + (ci & 1) * p.w1_bytes;
+      for (int t1 = 0; t1 < p.T1; ++t1, ++n1) {
+        const int slot = n1 & (nslot1 - 1);
+        tc::mbar_wait(bar_addr(bars, R1_EMPTY + slot), ((n1 >> p.lg_nslot1) & 1) ^ 1);
+        tc::tc_fence_after();
+        const uint32_t d = tmem + p.tm_r1 + slot * p.N1;
+        for (int ks = 0; ks < nks; ++ks) {
+          const uint64_t da = tc::smem_desc(s_base + p.off_a1 + (2 * ks * p.NP1p + t1 * 128) * 16, lbo_a, 128, tc::LAYOUT_NONE);
+          const uint64_t db = tc::smem_desc(b_base + 2 * ks * p.N1 * 16, lbo_b, 128, tc::LAYOUT_NONE);
+          if (tc::elect_one()) tc::mma_i8(d, da, db, idesc1, ks > 0);
+        }
+        if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R1_FULL + slot));
+        __syncwarp();
+      }
+      if (tc::elect_one()) tc::mma_commit(bar_addr(bars, W1_EMPTY + (ci & 1)));
+      __syncwarp();
+    }
+  } else if (warp == 1) {
+    // ===== layer-2 issuer =====
+    if (p.n_layers == 2) {
+      const uint32_t idesc2 = tc::idesc_i8(128, p.N2, 1, 1, 0, 0);
+      const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)p.N2 * 16;
+      const int acc_cols = p.nph2 * p.N2;
+      int n2 = 0;
+      for (int ci = 0; ci < n_cta_cand; ++ci) {
+        if (ci == 0 && tc::elect_one()) {
+          tc::mbar_arrive_expect_tx(bar_addr(bars, W2_FULL), p.w2_bytes);
+          tc::bulk_load(s_base + p.off_w2, p.wblob + (long long)c_begin * p.blob_bytes + p.w1_bytes, p.w2_bytes, bar_addr(bars, W2_FULL));
+        }
+        if (ci + 1 < n_cta_cand) {
+          const int slot = (ci + 1) % 3, use = (ci + 1) / 3;
+          tc::mbar_wait(bar_addr(bars, W2_EMPTY + slot), (use & 1) ^ 1);
+          if (tc::elect_one()) {
+            tc::mbar_arrive_expect_tx(bar_addr(bars, W2_FULL + slot), p.w2_bytes);
+            tc::bulk_load(s_base + p.off_w2 + slot * p.w2_bytes, p.wblob + (long long)(c_begin + ci + 1) * p.blob_bytes + p.w1_bytes,
+                          p.w2_bytes, bar_addr(bars, W2_FULL + slot));
+          }
+        }
+        const int wslot = ci % 3;
+        tc::mbar_wait(bar_addr(bars, W2_FULL + wslot), (ci / 3) & 1);
+        const int buf = (p.NPB == 2) ? (ci & 1) : 0;
+        const int use = (p.NPB == 2) ? (ci >> 1) : ci;
+        tc::mbar_wait(bar_addr(bars, PL_FULL + buf), use & 1);
+        const uint32_t pl_base = s_base + p.off_pl + buf * p.plbuf_bytes;
+        const uint32_t b_base = s_base + p.off_w2 + wslot * p.w2_bytes;
+        for (int t2 = 0; t2 < p.T2; ++t2, ++n2) {
+          const int slot = n2 & 1;
+          tc::mbar_wait(bar_addr(bars, R2_EMPTY + slot), ((n2 >> 1) & 1) ^ 1);
+          tc::tc_fence_after();
+          const uint32_t d0 = tmem + p.tm_r2 + slot * acc_cols;
+          const int row0 = p.base0 + t2 * 128;
+          for (int py = 0; py < p.P2; ++py)
+            for (int px = 0; px < p.P2; ++px) {
+              const uint32_t d = d0 + (py * p.P2 + px) * p.N2;
+              for (int dy = 0; dy < p.k2; ++dy) {
+                const int ry = py + dy - p.pd2, qy = floordiv(ry, p.P2), sy = ry - qy * p.P2;
+                for (int dx = 0; dx < p.k2; ++dx) {
+                  const int rx = px + dx - p.pd2, qx = floordiv(rx, p.P2), sx = rx - qx * p.P2;
+                  const uint32_t a_addr = pl_base + (sy * p.P2 + sx) * p.plane_bytes + (row0 + qy * p.Wq + qx) * 16;
+                  const uint64_t da = tc::smem_desc(a_addr, lbo_a, 128, tc::LAYOUT_NONE);
+                  const uint64_t db = tc::smem_desc(b_base + (dy * p.k2 + dx) * (p.N2 * 32), lbo_b, 128, tc::LAYOUT_NONE);
+                  if (tc::elect_one()) tc::mma_i8(d, da, db, idesc2, (dy | dx) != 0);
+                }
+              }
+            }
+          if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R2_FULL + slot));
+          __syncwarp();
+        }
+        if (tc::elect_one()) {
+          tc::mma_commit(bar_addr(bars, PL_EMPTY + buf));
+          tc::mma_commit(bar_addr(bars, W2_EMPTY + wslot));
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp < 2 + n_e1_warps) {
+    const int set = (warp - 2) >> 2, quad = warp & 3;
+    if (p.n_layers == 2) {
+      if (p.nph1 == 1) e1_two_layer<1>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else if (p.nph1 == 4) e1_two_layer<4>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else e1_two_layer<16>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+    } else {
+      if (p.nph1 == 1) e1_single<1>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+      else if (p.nph1 == 4) e1_single<4>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+      else e1_single<16>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+    }
+  } else if (p.n_layers == 2) {
+    const int set = (warp - 2 - n_e1_warps) >> 2, quad = warp & 3;
+    e2_run(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
   }
   tc::tc_fence_before();
   __syncthreads();
-  if (warp == 0) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, 256); }
+  if (warp == 0) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, 512); }
 }
 
 }  // namespace
 
+// ---- host side ------------------------------------------------------------------------------------------------------------
 // Is the architecture inside the tensor-core kernel's envelope?  Fills the launch parameters if so.
 static bool plan_xtc(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, XtcParams* q, size_t* smem_bytes) {
   if (has_bias || s.n_layers < 1 || s.n_layers > 2) return false;
   for (int l = 0; l < s.n_layers; ++l) {
     const LayerShape& L = s.L[l];
-    if (L.conv_type != LBCNN_CONV_FULL || L.pp != 0 || L.cover != 0 || L.pk != L.ps || L.pk < 1) return false;
+    if (L.conv_type != LBCNN_CONV_FULL || L.pp != 0 || L.cover != 0 || L.pk != L.ps) return false;
+    if (L.pk != 1 && L.pk != 2 && L.pk != 4) return false;
     if (L.hin % L.pk != 0 || L.win % L.pk != 0) return false;
   }
   XtcParams p{};
   const LayerShape& A = s.L[0];
   p.H = A.hin; p.W = A.win; p.C = A.cin; p.n_layers = s.n_layers;
-  p.k1 = A.k; p.pd1 = (A.k - 1) / 2; p.P1 = A.pk; p.Cout1 = A.cout; p.K1 = A.k * A.k * A.cin;
-  p.K1p = (p.K1 + 31) / 32 * 32; p.Ho1 = A.hout; p.Wo1 = A.wout; p.act1 = A.act; p.w1_off = (int)A.w_off;
-  if (p.Cout1 > 16 || p.K1p > 128 || p.P1 * p.P1 * 16 > 256) return false;
+  p.k1 = A.k; p.pd1 = (A.k - 1) / 2; p.P1 = A.pk; p.nph1 = A.pk * A.pk; p.Cout1 = A.cout;
+  p.Pk1 = A.pk + A.k - 1; p.K1 = p.Pk1 * p.Pk1 * A.cin; p.K1p = (p.K1 + 31) / 32 * 32;
+  p.Ho1 = A.hout; p.Wo1 = A.wout; p.act1 = A.act;
+  const int cpg = p.nph1 >= 16 ? 1 : 16 / p.nph1;                 // channels per 16-column group
+  p.Cp1 = (p.Cout1 + cpg - 1) / cpg * cpg;
+  p.N1 = p.Cp1 * p.nph1;
+  if (p.N1 > 256 || p.K1p > 256) return false;
+  p.w1_bytes = p.K1p * p.N1;
   int halo = 0;
   if (s.n_layers == 2) {
     const LayerShape& Bq = s.L[1];
-    p.k2 = Bq.k; p.pd2 = (Bq.k - 1) / 2; p.P2 = Bq.pk; p.Cout2 = Bq.cout; p.Ho2 = Bq.hout; p.Wo2 = Bq.wout;
-    p.act2 = Bq.act; p.w2_off = (int)Bq.w_off;
+    if (p.Cout1 > 16 || 255LL * A.k * A.k * A.cin > 8191) return false;   // 16 channels per K chunk; two int8 digits
+    p.k2 = Bq.k; p.pd2 = (Bq.k - 1) / 2; p.P2 = Bq.pk; p.nph2 = Bq.pk * Bq.pk; p.Cout2 = Bq.cout;
+    p.Ho2 = Bq.hout; p.Wo2 = Bq.wout; p.act2 = Bq.act;
     p.N2 = (p.Cout2 + 15) / 16 * 16;
-    if (p.N2 > 256 || p.P2 * p.P2 * p.N2 > 256) return false;
-    if (255LL * p.K1 > 8159) return false;                       // two balanced radix-64 int8 digits
+    if (p.N2 > 256) return false;
+    p.tm_r1 = 0; p.tm_r2 = 2 * p.N1; p.lg_nslot1 = 1;
+    if (2 * p.N1 + 2 * p.nph2 * p.N2 > 512) return false;
+    p.w2_bytes = p.k2 * p.k2 * p.N2 * 32;
     const int hq = (p.pd2 + p.P2 - 1) / p.P2, qmax = (p.P2 - 1 + p.pd2) / p.P2;
     halo = hq > qmax ? hq : qmax;
     p.Wq = p.Wo2 + halo; p.Hq = p.Ho2 + halo; p.base0 = halo * p.Wq + halo;
+  } else {
+    p.tm_r1 = 0; p.lg_nslot1 = (4 * p.N1 <= 512) ? 2 : 1;
+    p.w2_bytes = 0;
   }
-  // images per CTA: as many as keep one CTA under ~100 KB of shared memory (two CTAs per SM), at most 8
+  p.blob_bytes = p.w1_bytes + p.w2_bytes;
+  // images per CTA: the batch size (<= 8) whose 128-row tiles are best filled, within the shared-memory limit
   const int npx = p.H * p.W * p.C;
-  const int limit = 100 * 1024;
-  int bestB = 0; XtcParams best{}; size_t best_smem = 0;
+  const size_t limit = (size_t)h->max_smem_optin;
+  double best_score = -1.0; XtcParams best{}; size_t best_smem = 0;
   for (int B = 1; B <= 8; ++B) {
     XtcParams t = p;
-    t.B = B; t.NP1 = B * p.Ho1 * p.Wo1; t.T1 = (t.NP1 + 127) / 128;
-    t.col_slot_bytes = p.P1 * p.P1 * p.K1p * 128;
+    t.B = B; t.NP1 = B * p.Ho1 * p.Wo1; t.T1 = (t.NP1 + 127) / 128; t.NP1p = t.T1 * 128;
+    if ((long long)t.NP1p * 16 >= (1 << 18)) break;               // descriptor leading-offset field
     int off = 0;
     auto take = [&](int bytes) { int o = off; off += (bytes + 127) / 128 * 128; return o; };
     t.off_img = take(B * npx);
-    t.off_w1 = take(16 * p.K1p);
-    if (s.n_layers == 2) {
-      t.NM2 = B * p.Hq * p.Wq; t.T2 = (t.NM2 + 127) / 128;
-      t.NPOS2 = (p.base0 + t.T2 * 128 + halo * p.Wq + halo + 8 + 7) / 8 * 8;
-      t.plane_bytes = 2 * t.NPOS2 * 16;
-      t.off_w2 = take(p.k2 * p.k2 * p.N2 * 32);
-      t.off_pl = take(p.P2 * p.P2 * t.plane_bytes);
-      if (t.NPOS2 * 16 >= (1 << 18)) break;
+    t.off_a1 = take(t.NP1p * t.K1p);
+    t.off_w1 = take(2 * p.w1_bytes);
+    t.off_tab1 = take(t.NP1p * 4);
+    double score = (double)t.NP1 / t.NP1p;
+    for (int npb = 2; npb >= 1; --npb) {
+      XtcParams u = t; int off2 = off;
+      auto take2 = [&](int bytes) { int o = off2; off2 += (bytes + 127) / 128 * 128; return o; };
+      if (s.n_layers == 2) {
+        u.NM2 = B * p.Hq * p.Wq; u.T2 = (u.NM2 + 127) / 128;
+        u.NPOS2 = (p.base0 + u.T2 * 128 + halo * p.Wq + halo + 8 + 7) / 8 * 8;
+        if (u.NPOS2 * 16 >= (1 << 18)) break;
+        u.plane_bytes = 2 * u.NPOS2 * 16;
+        u.plbuf_bytes = p.nph2 * u.plane_bytes;
+        u.NPB = npb;
+        u.off_w2 = take2(3 * p.w2_bytes);
+        u.off_tab2 = take2(u.T2 * 128 * 4);
+        u.off_pl = take2(npb * u.plbuf_bytes);
+        score = 0.3 * t.NP1 / t.NP1p + 0.7 * u.NM2 / (u.T2 * 128.0);
+        if (npb == 1) score *= 0.8;                                // single plane buffer: less overlap
+      } else {
+        u.NPB = 1;
+        if (npb == 1) break;
+      }
+      if ((size_t)off2 + 1024 > limit) continue;
+      score += 0.002 * B;                                          // ties: larger batches amortise the set-up
+      if (score > best_score) { best_score = score; best = u; best_smem = (size_t)off2; }
+      break;
     }
-    const int fixed = off;
-    // cache the im2col rows of every layer-1 tile across candidates when they fit
-    t.cache = (fixed + t.T1 * t.col_slot_bytes <= limit) ? 1 : 0;
-    t.off_col = take((t.cache ? t.T1 : 1) * t.col_slot_bytes);
-    if (off > limit && B > 1) break;
-    if ((size_t)off > (size_t)h->max_smem_optin) break;
-    bestB = B; best = t; best_smem = (size_t)off;
   }
-  if (!bestB) return false;
+  if (best_score < 0.0) return false;
   *q = best; *smem_bytes = best_smem;
   return true;
 }
@@ -329,20 +591,47 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
   XtcParams p; size_t smem = 0;
   if (!plan_xtc(h, s, false, &p, &smem)) return LBCNN_ERR_INVALID_ARCH;
   LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
-  p.img = d_images; p.n_img = n; p.ker = d_kernels; p.n_weights = (int)s.n_weights; p.n_cand = n_cand;
+  // handle-owned scratch for the re-laid-out kernel sets (stream-ordered allocation, grown on demand)
+  const size_t need = (size_t)n_cand * p.blob_bytes;
+  if (need > h->xw_bytes) {
+    if (h->xw) LB_CUDA_OK(cudaFreeAsync(h->xw, st));
+    h->xw = nullptr; h->xw_bytes = 0;
+    const size_t cap = (need + ((size_t)1 << 20) - 1) >> 20 << 20;
+    LB_CUDA_OK(cudaMallocAsync(&h->xw, cap, st));
+    h->xw_bytes = cap;
+  }
+  {
+    PrepParams w{};
+    w.ker = d_kernels; w.n_weights = (int)s.n_weights; w.blob = reinterpret_cast<uint8_t*>(h->xw);
+    w.blob_bytes = p.blob_bytes; w.w1_bytes = p.w1_bytes; w.n_layers = p.n_layers;
+    w.k1 = p.k1; w.P1 = p.P1; w.nph1 = p.nph1; w.Cout1 = p.Cout1; w.N1 = p.N1; w.K1 = p.K1; w.K1p = p.K1p; w.Pk1 = p.Pk1;
+    w.Cin1 = p.C; w.w1_off = (int)s.L[0].w_off;
+    if (p.n_layers == 2) { w.k2 = p.k2; w.Cout2 = p.Cout2; w.N2 = p.N2; w.w2_off = (int)s.L[1].w_off; }
+    if (n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
+    dim3 grid((unsigned)((p.blob_bytes + 1023) / 1024 < 1 ? 1 : (p.blob_bytes + 1023) / 1024), (unsigned)n_cand);
+    xtc_prep_kernel<<<grid, 256, 0, st>>>(w);
+    h->launches += 1;
+    LB_CUDA_OK(cudaGetLastError());
+  }
+  p.img = d_images; p.n_img = n; p.wblob = reinterpret_cast<const uint8_t*>(h->xw); p.n_cand = n_cand;
   p.Hout = d_H; p.F = s.F; p.scale = feature_scale;
   const long long batches = (n + p.B - 1) / p.B;
-  // candidates per CTA: enough CTAs for ~8 waves of 2 CTAs per SM, otherwise as many candidates as possible
-  // per CTA (they share the staged images and, when cached, the im2col rows)
+  // candidates per CTA: as many as possible (they share the staged images and A1) while the grid still
+  // covers the SMs about four times over
   int cpc = n_cand;
-  const long long want = 8LL * 2 * h->n_sm;
-  while (cpc > 1 && batches * ((n_cand + cpc - 1) / cpc) < want) cpc = (cpc + 1) / 2;
+  const long long want = 4LL * h->n_sm;
+  while (cpc > 8 && batches * ((n_cand + cpc - 1) / cpc) < want) cpc = (cpc + 1) / 2;
   p.cand_per_cta = cpc;
   const int gy = (n_cand + cpc - 1) / cpc;
   if (batches > 2147483647LL || gy > 65535) return LBCNN_ERR_INVALID_ARG;
+  // one CTA per SM (it owns all 512 TMEM columns): ask for more than half of the SM's shared memory
+  if (smem < 120 * 1024) smem = 120 * 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(expand_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (getenv("LBCNN_DEBUG"))
+    fprintf(stderr, "[xtc] B=%d T1=%d T2=%d N1=%d K1p=%d N2=%d NPB=%d nslot1=%d smem=%zu cpc=%d grid=%lld x %d blob=%d\n", p.B, p.T1,
+            p.T2, p.N1, p.K1p, p.N2, p.NPB, 1 << p.lg_nslot1, smem, cpc, batches, gy, p.blob_bytes);
   dim3 grid((unsigned)batches, (unsigned)gy);
-  expand_tc_kernel<<<grid, 128, smem, st>>>(p);
+  expand_tc_kernel<<<grid, XT_THREADS, smem, st>>>(p);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;

@@ -16,6 +16,7 @@ struct lbcnn_handle_s {
   void* ws;
   size_t ws_bytes;
   int64_t launches;
+  void* xw; size_t xw_bytes;        // handle-owned scratch: kernel sets re-laid-out for the tensor-core expander
   int force_simt_expand;            // testing: keep the expander on the SIMT kernel (LBCNN_FORCE_SIMT_EXPAND=1)
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
