@@ -275,6 +275,35 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
   }
 }
 
+// ---- layer-2 MMA issue for one 128-row tile -------------------------------------------------------------------------
+// All P2*P2*k*k (phase, tap) MMAs of the tile.  With P2 / K2 known at compile time every plane / shift / tap index
+// folds to a constant, so one MMA costs a handful of uniform-datapath instructions (descriptor = base + offset in
+// 16-byte units; the sums stay inside the 14-bit address field because every operand lies in shared memory).
+template <int P2c, int K2c>
+__device__ __forceinline__ void l2_issue_tile(const XtcParams& p, uint32_t d0, uint64_t da0, uint64_t db0, uint32_t idesc2) {
+  const int P2 = P2c ? P2c : p.P2, K2 = K2c ? K2c : p.k2;
+  const int pd = (K2 - 1) / 2;
+  const int plane16 = p.plane_bytes >> 4, n2x2 = p.N2 * 2;
+#pragma unroll
+  for (int py = 0; py < P2; ++py)
+#pragma unroll
+    for (int px = 0; px < P2; ++px) {
+      const uint32_t d = d0 + (py * P2 + px) * p.N2;
+#pragma unroll
+      for (int dy = 0; dy < K2; ++dy) {
+        const int ry = py + dy - pd, qy = floordiv(ry, P2), sy = ry - qy * P2;
+#pragma unroll
+        for (int dx = 0; dx < K2; ++dx) {
+          const int rx = px + dx - pd, qx = floordiv(rx, P2), sx = rx - qx * P2;
+          const int a_off = (sy * P2 + sx) * plane16 + qy * p.Wq + qx;
+          const uint64_t da = da0 + (uint64_t)(long long)a_off;
+          const uint64_t db = db0 + (uint64_t)((dy * K2 + dx) * n2x2);
+          if (tc::elect_one()) tc::mma_i8(d, da, db, idesc2, (dy | dx) != 0);
+        }
+      }
+    }
+}
+
 // ---- the kernel ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParams p) {
   extern __shared__ __align__(128) uint8_t smem[];
@@ -449,21 +478,13 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
           tc::mbar_wait(bar_addr(bars, R2_EMPTY + slot), ((n2 >> 1) & 1) ^ 1);
           tc::tc_fence_after();
           const uint32_t d0 = tmem + p.tm_r2 + slot * acc_cols;
-          const int row0 = p.base0 + t2 * 128;
-          for (int py = 0; py < p.P2; ++py)
-            for (int px = 0; px < p.P2; ++px) {
-              const uint32_t d = d0 + (py * p.P2 + px) * p.N2;
-              for (int dy = 0; dy < p.k2; ++dy) {
-                const int ry = py + dy - p.pd2, qy = floordiv(ry, p.P2), sy = ry - qy * p.P2;
-                for (int dx = 0; dx < p.k2; ++dx) {
-                  const int rx = px + dx - p.pd2, qx = floordiv(rx, p.P2), sx = rx - qx * p.P2;
-                  const uint32_t a_addr = pl_base + (sy * p.P2 + sx) * p.plane_bytes + (row0 + qy * p.Wq + qx) * 16;
-                  const uint64_t da = tc::smem_desc(a_addr, lbo_a, 128, tc::LAYOUT_NONE);
-                  const uint64_t db = tc::smem_desc(b_base + (dy * p.k2 + dx) * (p.N2 * 32), lbo_b, 128, tc::LAYOUT_NONE);
-                  if (tc::elect_one()) tc::mma_i8(d, da, db, idesc2, (dy | dx) != 0);
-                }
-              }
-            }
+          const uint32_t row0 = (uint32_t)(p.base0 + t2 * 128) * 16;
+          const uint64_t da0 = tc::smem_desc(pl_base + row0, lbo_a, 128, tc::LAYOUT_NONE);
+          const uint64_t db0 = tc::smem_desc(b_base, lbo_b, 128, tc::LAYOUT_NONE);
+          if (p.P2 == 2 && p.k2 == 3) l2_issue_tile<2, 3>(p, d0, da0, db0, idesc2);
+          else if (p.P2 == 1 && p.k2 == 3) l2_issue_tile<1, 3>(p, d0, da0, db0, idesc2);
+          else if (p.P2 == 2 && p.k2 == 5) l2_issue_tile<2, 5>(p, d0, da0, db0, idesc2);
+          else l2_issue_tile<0, 0>(p, d0, da0, db0, idesc2);
           if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R2_FULL + slot));
           __syncwarp();
         }
