@@ -34,7 +34,7 @@
 
 namespace {
 
-constexpr int XT_WARPS = 18;
+constexpr int XT_WARPS = 19;
 constexpr int XT_THREADS = XT_WARPS * 32;
 
 struct XtcParams {
@@ -47,12 +47,23 @@ struct XtcParams {
   int k1, pd1, P1, nph1, Cout1, Cp1, N1, K1, K1p, Pk1, Ho1, Wo1, act1;
   // layer 2
   int k2, pd2, P2, nph2, Cout2, N2, Ho2, Wo2, act2, Wq, Hq, base0, NPOS2;
-  int B, NP1, NP1p, T1, NM2, T2, NPB, lg_nslot1;
+  int B, NP1, NP1p, T1, NM2, T2, NPB, lg_nslot1, lg_nset1;   // R1 ring slots / E1 warp sets (powers of two)
   // shared-memory offsets (bytes)
   int off_img, off_a1, off_w1, off_w2, off_pl, off_tab1, off_tab2, plane_bytes, plbuf_bytes;
   // TMEM column offsets
   int tm_r1, tm_r2;
+  long long* trace;   // debug builds (-DXTC_TRACE) only
 };
+
+#ifdef XTC_TRACE
+#define XT_TRACE(ev) do { if (tr && (threadIdx.x & 31) == 0 && trn < 8190) tr[trn++] = ((long long)clock64() << 8) | (ev); } while (0)
+#define XT_TRACE_ARGS , long long* tr, int& trn
+#define XT_TRACE_PASS , tr, trn
+#else
+#define XT_TRACE(ev) do { } while (0)
+#define XT_TRACE_ARGS
+#define XT_TRACE_PASS
+#endif
 
 // barrier slots
 enum { W1_FULL = 0, W1_EMPTY = 2, W2_FULL = 4, W2_EMPTY = 7, R1_FULL = 10, R1_EMPTY = 14, PL_FULL = 18, PL_EMPTY = 20,
@@ -117,12 +128,12 @@ __device__ __forceinline__ uint32_t bar_addr(const uint64_t* bars, int i) { retu
 // tab1[m] = byte offset of pooled position m inside one plane buffer (phase plane + halo-sharing position), -1 = none
 template <int NPH>
 __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, const uint64_t* bars, uint32_t tmem,
-                                             int set, int quad, int lane, int n_cta_cand) {
+                                             int set, int quad, int lane, int n_cta_cand XT_TRACE_ARGS) {
   constexpr int CPG = 16 / NPH;          // channels per 16-column group
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
-  const int mask = (1 << p.lg_nslot1) - 1;
+  const int mask = (1 << p.lg_nset1) - 1, smask = (1 << p.lg_nslot1) - 1;
   const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
-  const uint32_t taddr = tmem + lane_base + p.tm_r1 + set * p.N1;
+  const uint32_t taddr0 = tmem + lane_base + p.tm_r1;
   for (int ci = 0; ci < n_cta_cand; ++ci) {
     const int buf = (p.NPB == 2) ? (ci & 1) : 0;
     const int use = (p.NPB == 2) ? (ci >> 1) : ci;
@@ -130,8 +141,11 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
     for (int t1 = 0; t1 < p.T1; ++t1) {
       const int n1 = ci * p.T1 + t1;
       if ((n1 & mask) != set) continue;
-      tc::mbar_wait(bar_addr(bars, R1_FULL + set), (n1 >> p.lg_nslot1) & 1);
+      const int slot = n1 & smask;
+      const uint32_t taddr = taddr0 + slot * p.N1;
+      tc::mbar_wait(bar_addr(bars, R1_FULL + slot), (n1 >> p.lg_nslot1) & 1);
       tc::tc_fence_after();
+      XT_TRACE(6);
       int mx[16];
 #pragma unroll
       for (int e = 0; e < 16; ++e) mx[e] = 0;
@@ -150,8 +164,9 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
       }
       tc::tc_fence_before();
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + set));      // accumulator slot free again
-      if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; }
+      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + slot));     // accumulator slot free again
+      XT_TRACE(7);
+      if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; XT_TRACE(8); }
       const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
       if (off >= 0) {
         uint32_t lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};
@@ -166,11 +181,13 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
         *reinterpret_cast<uint4*>(dst) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
         *reinterpret_cast<uint4*>(dst + p.NPOS2 * 16) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
       }
+      XT_TRACE(9);
     }
     if (!waited) tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1);   // never run ahead of the buffer's phase
     tc::fence_proxy_async();                 // generic-proxy plane writes -> visible to the MMA's async proxy
     __syncwarp();
     if (lane == 0) tc::mbar_arrive(bar_addr(bars, PL_FULL + buf));
+    XT_TRACE(10);
   }
 }
 
@@ -178,19 +195,21 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
 // tab1[m] = b*F + i*Wo + j of pooled position m (flatten C,H,W adds o*Ho*Wo), -1 = none
 template <int NPH>
 __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem,
-                                          int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
+                                          int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0 XT_TRACE_ARGS) {
   constexpr int CPG = 16 / NPH;
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
-  const int mask = (1 << p.lg_nslot1) - 1;
+  const int mask = (1 << p.lg_nset1) - 1, smask = (1 << p.lg_nslot1) - 1;
   const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
-  const uint32_t taddr = tmem + lane_base + p.tm_r1 + set * p.N1;
+  const uint32_t taddr0 = tmem + lane_base + p.tm_r1;
   const int G1 = p.N1 >> 4, hw = p.Ho1 * p.Wo1;
   for (int ci = 0; ci < n_cta_cand; ++ci) {
     float* Hc = p.Hout + ((long long)(c_begin + ci) * p.n_img + img0) * p.F;
     for (int t1 = 0; t1 < p.T1; ++t1) {
       const int n1 = ci * p.T1 + t1;
       if ((n1 & mask) != set) continue;
-      tc::mbar_wait(bar_addr(bars, R1_FULL + set), (n1 >> p.lg_nslot1) & 1);
+      const int slot = n1 & smask;
+      const uint32_t taddr = taddr0 + slot * p.N1;
+      tc::mbar_wait(bar_addr(bars, R1_FULL + slot), (n1 >> p.lg_nslot1) & 1);
       tc::tc_fence_after();
       const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
       for (int gb = 0; gb < G1; gb += 4) {
@@ -218,59 +237,79 @@ __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* sme
       }
       tc::tc_fence_before();
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + set));
+      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + slot));
     }
   }
 }
 
 // ---- E2: R2 -> max over the pool-phase accumulators -> (relu) -> scale -> H ------------------------------------------
 // tab2[m] = b*F + i*Wo2 + j of row m of the halo-sharing output grid, -1 = halo / beyond the batch
+template <bool RELU, bool UNIT>
+__device__ __forceinline__ void e2_store16(float* __restrict__ Hb, uint32_t idx, uint32_t hw, const int (&mx)[16], int nreal, float scale) {
+  if (nreal == 16) {
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      int v = mx[e];
+      if (RELU) v = max(v, 0);
+      Hb[idx] = UNIT ? (float)v : scale * (float)v;                        // flatten C,H,W: channel stride Ho*Wo
+      idx += hw;
+    }
+  } else {
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      if (e < nreal) {
+        int v = mx[e];
+        if (RELU) v = max(v, 0);
+        Hb[idx] = UNIT ? (float)v : scale * (float)v;
+        idx += hw;
+      }
+    }
+  }
+}
+
+template <bool RELU, bool UNIT>
 __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem, int set,
-                                       int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
+                                       int quad, int lane, int c_begin, int n_cta_cand, long long img0 XT_TRACE_ARGS) {
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
   const int32_t* tab2 = reinterpret_cast<const int32_t*>(smem + p.off_tab2);
-  const uint32_t taddr = tmem + lane_base + p.tm_r2 + set * (p.nph2 * p.N2);
-  const int hw = p.Ho2 * p.Wo2;
-  for (int ci = 0; ci < n_cta_cand; ++ci) {
-    float* Hc = p.Hout + ((long long)(c_begin + ci) * p.n_img + img0) * p.F;
-    for (int t2 = 0; t2 < p.T2; ++t2) {
-      const int n2 = ci * p.T2 + t2;
+  const int nph2 = p.nph2, N2 = p.N2, cout2 = p.Cout2, T2 = p.T2;
+  const uint32_t hw = (uint32_t)(p.Ho2 * p.Wo2);
+  const float scale = p.scale;
+  const uint32_t taddr = tmem + lane_base + p.tm_r2 + set * (nph2 * N2);
+  const long long cand_stride = p.n_img * p.F;
+  float* Hb = p.Hout + ((long long)c_begin * p.n_img + img0) * p.F;
+  for (int ci = 0; ci < n_cta_cand; ++ci, Hb += cand_stride) {
+    for (int t2 = 0; t2 < T2; ++t2) {
+      const int n2 = ci * T2 + t2;
       if ((n2 & 1) != set) continue;
       tc::mbar_wait(bar_addr(bars, R2_FULL + set), (n2 >> 1) & 1);
       tc::tc_fence_after();
+      XT_TRACE(11);
       const int32_t off = tab2[t2 * 128 + quad * 32 + lane];
-      for (int c0 = 0; c0 < p.Cout2; c0 += 16) {
+      for (int c0 = 0; c0 < cout2; c0 += 16) {
         int mx[16];
-#pragma unroll
-        for (int e = 0; e < 16; ++e) mx[e] = INT_MIN;
-        for (int ph0 = 0; ph0 < p.nph2; ph0 += 4) {
-          uint32_t r[4][16];
-#pragma unroll
-          for (int q = 0; q < 4; ++q)
-            if (ph0 + q < p.nph2) tc::tmem_ld16(taddr + (ph0 + q) * p.N2 + c0, r[q]);
+        {
+          uint32_t r0[16], r1[16];
+          tc::tmem_ld16(taddr + c0, r0);
+          if (nph2 > 1) tc::tmem_ld16(taddr + N2 + c0, r1);
           tc::tmem_ld_wait();
 #pragma unroll
-          for (int q = 0; q < 4; ++q)
-            if (ph0 + q < p.nph2) {
-#pragma unroll
-              for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], (int)r[q][e]);
-            }
+          for (int e = 0; e < 16; ++e) mx[e] = (nph2 > 1) ? max((int)r0[e], (int)r1[e]) : (int)r0[e];
         }
-        if (off >= 0) {
+        for (int ph = 2; ph < nph2; ph += 2) {
+          uint32_t r0[16], r1[16];
+          tc::tmem_ld16(taddr + ph * N2 + c0, r0);
+          tc::tmem_ld16(taddr + (ph + 1) * N2 + c0, r1);
+          tc::tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 16; ++e) {
-            const int o = c0 + e;
-            if (o < p.Cout2) {
-              int v = mx[e];
-              if (p.act2 == LBCNN_ACT_RELU) v = max(v, 0);
-              Hc[off + o * hw] = p.scale * (float)v;                       // flatten C,H,W
-            }
-          }
+          for (int e = 0; e < 16; ++e) mx[e] = max(mx[e], max((int)r0[e], (int)r1[e]));
         }
+        if (off >= 0) e2_store16<RELU, UNIT>(Hb, (uint32_t)off + (uint32_t)c0 * hw, hw, mx, min(16, cout2 - c0), scale);
       }
       tc::tc_fence_before();
       __syncwarp();
       if (lane == 0) tc::mbar_arrive(bar_addr(bars, R2_EMPTY + set));
+      XT_TRACE(12);
     }
   }
 }
@@ -280,14 +319,16 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
 // folds to a constant, so one MMA costs a handful of uniform-datapath instructions (descriptor = base + offset in
 // 16-byte units; the sums stay inside the 14-bit address field because every operand lies in shared memory).
 template <int P2c, int K2c>
-__device__ __forceinline__ void l2_issue_tile(const XtcParams& p, uint32_t d0, uint64_t da0, uint64_t db0, uint32_t idesc2) {
+__device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint32_t d0, uint64_t da0, uint64_t db0, uint32_t idesc2) {
   const int P2 = P2c ? P2c : p.P2, K2 = K2c ? K2c : p.k2;
   const int pd = (K2 - 1) / 2;
   const int plane16 = p.plane_bytes >> 4, n2x2 = p.N2 * 2;
+  // two issuer warps share a tile: warp `half` takes the pool phases with py in its half (all of them when P2 == 1)
 #pragma unroll
   for (int py = 0; py < P2; ++py)
 #pragma unroll
     for (int px = 0; px < P2; ++px) {
+      if (P2 > 1 && (py * 2 >= P2) != (half != 0)) continue;
       const uint32_t d = d0 + (py * P2 + px) * p.N2;
 #pragma unroll
       for (int dy = 0; dy < K2; ++dy) {
@@ -317,7 +358,8 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   const int n_cta_cand = min(p.cand_per_cta, p.n_cand - c_begin);
   const uint32_t s_base = tc::smem_u32(smem);
   const int nslot1 = 1 << p.lg_nslot1;
-  const int n_e1_warps = 4 * nslot1;
+  const int n_e1_warps = 4 << p.lg_nset1;
+  const int n_l2_issuers = (p.n_layers == 2 && p.P2 > 1) ? 2 : 1;     // warps 1 and 18 split a tile's pool phases
 
   if (tid == 0) {
     for (int i = 0; i < N_BARS; ++i) {
@@ -325,6 +367,7 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
       if (i >= R1_EMPTY && i < R1_EMPTY + 4) cnt = 4;
       if (i >= R2_EMPTY && i < R2_EMPTY + 2) cnt = 4;
       if (i >= PL_FULL && i < PL_FULL + 2) cnt = n_e1_warps;
+      if ((i >= R2_FULL && i < R2_FULL + 2) || (i >= PL_EMPTY && i < PL_EMPTY + 2) || (i >= W2_EMPTY && i < W2_EMPTY + 3)) cnt = n_l2_issuers;
       tc::mbar_init(bar_addr(bars, i), cnt);
     }
     tc::fence_barrier_init();
@@ -406,6 +449,11 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = tmem_base_s;
+#ifdef XTC_TRACE
+  long long* tr = (p.trace && blockIdx.x == gridDim.x / 2 && blockIdx.y == 0) ? p.trace + warp * 8192 + 1 : nullptr;
+  int trn = 0;
+  XT_TRACE(0);
+#endif
 
   if (warp == 0) {
     // ===== layer-1 issuer =====
@@ -433,6 +481,7 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         const int slot = n1 & (nslot1 - 1);
         tc::mbar_wait(bar_addr(bars, R1_EMPTY + slot), ((n1 >> p.lg_nslot1) & 1) ^ 1);
         tc::tc_fence_after();
+        XT_TRACE(1);
         const uint32_t d = tmem + p.tm_r1 + slot * p.N1;
         for (int ks = 0; ks < nks; ++ks) {
           const uint64_t da = tc::smem_desc(s_base + p.off_a1 + (2 * ks * p.NP1p + t1 * 128) * 16, lbo_a, 128, tc::LAYOUT_NONE);
@@ -441,23 +490,25 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         }
         if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R1_FULL + slot));
         __syncwarp();
+        XT_TRACE(2);
       }
       if (tc::elect_one()) tc::mma_commit(bar_addr(bars, W1_EMPTY + (ci & 1)));
       __syncwarp();
     }
-  } else if (warp == 1) {
-    // ===== layer-2 issuer =====
-    if (p.n_layers == 2) {
+  } else if (warp == 1 || warp == XT_WARPS - 1) {
+    // ===== layer-2 issuers =====
+    const int half = (warp == 1) ? 0 : 1;
+    if (p.n_layers == 2 && half < n_l2_issuers) {
       const uint32_t idesc2 = tc::idesc_i8(128, p.N2, 1, 1, 0, 0);
       const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)p.N2 * 16;
       const int acc_cols = p.nph2 * p.N2;
       int n2 = 0;
       for (int ci = 0; ci < n_cta_cand; ++ci) {
-        if (ci == 0 && tc::elect_one()) {
+        if (half == 0 && ci == 0 && tc::elect_one()) {
           tc::mbar_arrive_expect_tx(bar_addr(bars, W2_FULL), p.w2_bytes);
           tc::bulk_load(s_base + p.off_w2, p.wblob + (long long)c_begin * p.blob_bytes + p.w1_bytes, p.w2_bytes, bar_addr(bars, W2_FULL));
         }
-        if (ci + 1 < n_cta_cand) {
+        if (half == 0 && ci + 1 < n_cta_cand) {
           const int slot = (ci + 1) % 3, use = (ci + 1) / 3;
           tc::mbar_wait(bar_addr(bars, W2_EMPTY + slot), (use & 1) ^ 1);
           if (tc::elect_one()) {
@@ -471,22 +522,24 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         const int buf = (p.NPB == 2) ? (ci & 1) : 0;
         const int use = (p.NPB == 2) ? (ci >> 1) : ci;
         tc::mbar_wait(bar_addr(bars, PL_FULL + buf), use & 1);
+        XT_TRACE(3);
         const uint32_t pl_base = s_base + p.off_pl + buf * p.plbuf_bytes;
         const uint32_t b_base = s_base + p.off_w2 + wslot * p.w2_bytes;
         for (int t2 = 0; t2 < p.T2; ++t2, ++n2) {
           const int slot = n2 & 1;
           tc::mbar_wait(bar_addr(bars, R2_EMPTY + slot), ((n2 >> 1) & 1) ^ 1);
           tc::tc_fence_after();
+          XT_TRACE(4);
           const uint32_t d0 = tmem + p.tm_r2 + slot * acc_cols;
           const uint32_t row0 = (uint32_t)(p.base0 + t2 * 128) * 16;
           const uint64_t da0 = tc::smem_desc(pl_base + row0, lbo_a, 128, tc::LAYOUT_NONE);
           const uint64_t db0 = tc::smem_desc(b_base, lbo_b, 128, tc::LAYOUT_NONE);
-          if (p.P2 == 2 && p.k2 == 3) l2_issue_tile<2, 3>(p, d0, da0, db0, idesc2);
-          else if (p.P2 == 1 && p.k2 == 3) l2_issue_tile<1, 3>(p, d0, da0, db0, idesc2);
-          else if (p.P2 == 2 && p.k2 == 5) l2_issue_tile<2, 5>(p, d0, da0, db0, idesc2);
-          else l2_issue_tile<0, 0>(p, d0, da0, db0, idesc2);
+          if (p.P2 == 2 && p.k2 == 3) l2_issue_tile<2, 3>(p, half, d0, da0, db0, idesc2);
+          else if (p.P2 == 1 && p.k2 == 3) l2_issue_tile<1, 3>(p, half, d0, da0, db0, idesc2);
+          else l2_issue_tile<0, 0>(p, half, d0, da0, db0, idesc2);
           if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R2_FULL + slot));
           __syncwarp();
+          XT_TRACE(5);
         }
         if (tc::elect_one()) {
           tc::mma_commit(bar_addr(bars, PL_EMPTY + buf));
@@ -498,18 +551,29 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   } else if (warp < 2 + n_e1_warps) {
     const int set = (warp - 2) >> 2, quad = warp & 3;
     if (p.n_layers == 2) {
-      if (p.nph1 == 1) e1_two_layer<1>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
-      else if (p.nph1 == 4) e1_two_layer<4>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
-      else e1_two_layer<16>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      if (p.nph1 == 1) e1_two_layer<1>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else if (p.nph1 == 4) e1_two_layer<4>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else e1_two_layer<16>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
     } else {
-      if (p.nph1 == 1) e1_single<1>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
-      else if (p.nph1 == 4) e1_single<4>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
-      else e1_single<16>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+      if (p.nph1 == 1) e1_single<1>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      else if (p.nph1 == 4) e1_single<4>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      else e1_single<16>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
     }
   } else if (p.n_layers == 2) {
     const int set = (warp - 2 - n_e1_warps) >> 2, quad = warp & 3;
-    e2_run(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+    const bool relu = p.act2 == LBCNN_ACT_RELU, unit = p.scale == 1.0f;
+    if (relu) {
+      if (unit) e2_run<true, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      else e2_run<true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+    } else {
+      if (unit) e2_run<false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      else e2_run<false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+    }
   }
+#ifdef XTC_TRACE
+  XT_TRACE(13);
+  if (tr && lane == 0) tr[-1] = trn;
+#endif
   tc::tc_fence_before();
   __syncthreads();
   if (warp == 0) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, 512); }
@@ -546,14 +610,22 @@ static bool plan_xtc(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias,
     p.Ho2 = Bq.hout; p.Wo2 = Bq.wout; p.act2 = Bq.act;
     p.N2 = (p.Cout2 + 15) / 16 * 16;
     if (p.N2 > 256) return false;
-    p.tm_r1 = 0; p.tm_r2 = 2 * p.N1; p.lg_nslot1 = 1;
-    if (2 * p.N1 + 2 * p.nph2 * p.N2 > 512) return false;
+    // two E1 warp sets; each owns two R1 accumulator slots when TMEM has room (so the next tile's MMA is done early)
+    p.lg_nset1 = 1; p.lg_nslot1 = (4 * p.N1 + 2 * p.nph2 * p.N2 <= 512) ? 2 : 1;
+    p.tm_r1 = 0; p.tm_r2 = (1 << p.lg_nslot1) * p.N1;
+    if (p.tm_r2 + 2 * p.nph2 * p.N2 > 512) return false;
     p.w2_bytes = p.k2 * p.k2 * p.N2 * 32;
     const int hq = (p.pd2 + p.P2 - 1) / p.P2, qmax = (p.P2 - 1 + p.pd2) / p.P2;
     halo = hq > qmax ? hq : qmax;
-    p.Wq = p.Wo2 + halo; p.Hq = p.Ho2 + halo; p.base0 = halo * p.Wq + halo;
+    // Row pitch and first row of the halo-sharing grid.  A shifted operand whose start is not a multiple of 8 rows
+    // (128 B) makes every 8-row core matrix straddle two shared-memory lines and the MMA read it in twice the
+    // wavefronts, so align the pitch when that costs few extra rows and always align the first row: the taps with
+    // no horizontal shift (two thirds of them) then read aligned operands.
+    p.Wq = p.Wo2 + halo;
+    if (p.Wq % 8 != 0 && (p.Wq + 7) / 8 * 8 * 7 <= p.Wq * 8) p.Wq = (p.Wq + 7) / 8 * 8;
+    p.Hq = p.Ho2 + halo; p.base0 = (halo * p.Wq + halo + 7) / 8 * 8;
   } else {
-    p.tm_r1 = 0; p.lg_nslot1 = (4 * p.N1 <= 512) ? 2 : 1;
+    p.tm_r1 = 0; p.lg_nslot1 = (4 * p.N1 <= 512) ? 2 : 1; p.lg_nset1 = p.lg_nslot1;
     p.w2_bytes = 0;
   }
   p.blob_bytes = p.w1_bytes + p.w2_bytes;
@@ -652,8 +724,24 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
     fprintf(stderr, "[xtc] B=%d T1=%d T2=%d N1=%d K1p=%d N2=%d NPB=%d nslot1=%d smem=%zu cpc=%d grid=%lld x %d blob=%d\n", p.B, p.T1,
             p.T2, p.N1, p.K1p, p.N2, p.NPB, 1 << p.lg_nslot1, smem, cpc, batches, gy, p.blob_bytes);
   dim3 grid((unsigned)batches, (unsigned)gy);
+  p.trace = nullptr;
+#ifdef XTC_TRACE
+  static long long* d_trace = nullptr;
+  const size_t trace_bytes = (size_t)XT_WARPS * 8192 * 8;
+  if (!d_trace) cudaMalloc(&d_trace, trace_bytes);
+  cudaMemsetAsync(d_trace, 0, trace_bytes, st);
+  p.trace = d_trace;
+#endif
   expand_tc_kernel<<<grid, XT_THREADS, smem, st>>>(p);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
+#ifdef XTC_TRACE
+  {
+    cudaStreamSynchronize(st);
+    std::vector<long long> hb(XT_WARPS * 8192);
+    cudaMemcpy(hb.data(), d_trace, trace_bytes, cudaMemcpyDeviceToHost);
+    if (FILE* fp = fopen("gpurun_out/xtc_trace.bin", "wb")) { fwrite(hb.data(), 8, hb.size(), fp); fclose(fp); }
+  }
+#endif
   return LBCNN_OK;
 }
