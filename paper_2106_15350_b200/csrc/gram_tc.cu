@@ -29,7 +29,6 @@ constexpr int TN = 96;         // output tile columns (features j) = UMMA N
 constexpr int KS = 64;         // samples per pipeline stage (two K = 32 MMA steps)
 constexpr int BOXW = 128;      // TMA box width in features (= bytes): one 128-byte swizzle row
 constexpr int TILE_BYTES = KS * BOXW;          // 8 KB per digit plane per operand per stage
-constexpr int MAXL = 3;
 constexpr int RING_BYTES = 24 * TILE_BYTES;   // 192 KB of operand stages: 12 / 6 / 4 stages for 1 / 2 / 3 digits
 constexpr int MAXSTAGE = 12;
 constexpr int TMEM_COLS = 512; // 5 accumulators x 96 columns = 480
@@ -84,7 +83,9 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
     }
   }
   need = __reduce_max_sync(0xffffffffu, need);
-  if ((threadIdx.x & 31) == 0 && need > 1) atomicMax(&nlimb[z], need);
+  // one atomic per warp only while it can still raise the count: after the first few warps of a candidate the
+  // (L2-cached) read already shows the final value and no further atomics reach that address
+  if ((threadIdx.x & 31) == 0 && need > 1 && need > *reinterpret_cast<volatile int32_t*>(&nlimb[z])) atomicMax(&nlimb[z], need);
 }
 
 __global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
@@ -93,6 +94,66 @@ __global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
 }
 
 // ---- the Gram kernel ------------------------------------------------------------------------------
+// Role loops run warp-uniformly (uniform_warp_id) and are specialised on the digit count L, so every stage / plane /
+// K-step offset is a compile-time constant and a descriptor is "base + constant": the issuing warp spends a few
+// uniform-datapath instructions per MMA instead of rebuilding descriptors in vector registers (which cost ~150 clk
+// per MMA, three times the MMA itself).
+template <int L>
+__device__ __forceinline__ void gram_produce(const CUtensorMap* tmap, const GramTcParams& p, uint32_t smem0, uint64_t* bar_full,
+                                             uint64_t* bar_empty, int i0, int j0, int z) {
+  constexpr int NSTAGE = 12 / L, STAGE_BYTES = 2 * L * TILE_BYTES;
+  int s = 0, ph = 0;
+  for (int it = 0; it < p.n_iters; ++it) {
+    tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ph ^ 1);
+    if (tc::elect_one()) {
+      const uint32_t full = tc::smem_u32(&bar_full[s]);
+      tc::mbar_arrive_expect_tx(full, STAGE_BYTES);
+      const uint32_t base = smem0 + s * STAGE_BYTES;
+#pragma unroll
+      for (int a = 0; a < L; ++a) {
+        tc::tma_load_3d(base + a * TILE_BYTES, tmap, full, i0, it * KS, z * 3 + a);
+        tc::tma_load_3d(base + (L + a) * TILE_BYTES, tmap, full, j0, it * KS, z * 3 + a);
+      }
+    }
+    __syncwarp();
+    if (++s == NSTAGE) { s = 0; ph ^= 1; }
+  }
+}
+
+template <int L>
+__device__ __forceinline__ void gram_issue(const GramTcParams& p, uint32_t smem0, uint32_t tmem, uint64_t* bar_full,
+                                           uint64_t* bar_empty, uint64_t* bar_tmem) {
+  constexpr int NSTAGE = 12 / L, STAGE_BYTES = 2 * L * TILE_BYTES;
+  constexpr uint32_t idesc = tc::idesc_i8(TM, TN, 1, 1, 1, 1);
+  // descriptor of the ring's first byte; every operand is this plus a constant number of 16-byte units
+  const uint64_t d0 = tc::smem_desc(smem0, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+  int s = 0, ph = 0;
+  for (int it = 0; it < p.n_iters; ++it) {
+    tc::mbar_wait(tc::smem_u32(&bar_full[s]), ph);
+    tc::tc_fence_after();
+    const uint64_t ds = d0 + (uint64_t)(s * (STAGE_BYTES >> 4));
+#pragma unroll
+    for (int kk = 0; kk < KS / 32; ++kk) {
+#pragma unroll
+      for (int a = 0; a < L; ++a) {
+#pragma unroll
+        for (int b = 0; b < L; ++b) {
+          const uint64_t da = ds + (uint64_t)((a * TILE_BYTES + kk * 32 * BOXW) >> 4);
+          const uint64_t db = ds + (uint64_t)(((L + b) * TILE_BYTES + kk * 32 * BOXW) >> 4);
+          // accumulator a + b; its first product of the whole tile is (a, b) with a = max(0, a + b - L + 1) at it = kk = 0
+          const bool first = (kk == 0) && (a == ((a + b) > (L - 1) ? (a + b) - (L - 1) : 0));
+          if (tc::elect_one()) tc::mma_i8(tmem + (a + b) * TN, da, db, idesc, (first && it == 0) ? 0u : 1u);
+        }
+      }
+    }
+    if (tc::elect_one()) tc::mma_commit(tc::smem_u32(&bar_empty[s]));     // stage free once these MMAs have read it
+    __syncwarp();
+    if (++s == NSTAGE) { s = 0; ph ^= 1; }
+  }
+  if (tc::elect_one()) tc::mma_commit(tc::smem_u32(bar_tmem));             // accumulators complete
+  __syncwarp();
+}
+
 __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const GramTcParams p) {
   const int ti = blockIdx.y, tj = blockIdx.x, z = blockIdx.z;
   const int i0 = ti * TM, j0 = tj * TN;
@@ -103,15 +164,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
   __shared__ __align__(8) uint64_t bar_full[MAXSTAGE], bar_empty[MAXSTAGE], bar_tmem;
   __shared__ uint32_t tmem_base_s;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = tc::uniform_warp_id(), lane = threadIdx.x & 31;
   const int L = p.nlimb[z];
-  const int STAGE_BYTES = 2 * L * TILE_BYTES;
-  const int NSTAGE = 12 / L;
   const uint32_t smem0 = tc::smem_u32(smem);
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tensormap(&tmap);
-    for (int s = 0; s < NSTAGE; ++s) { tc::mbar_init(tc::smem_u32(&bar_full[s]), 1); tc::mbar_init(tc::smem_u32(&bar_empty[s]), 1); }
+    for (int s = 0; s < MAXSTAGE; ++s) { tc::mbar_init(tc::smem_u32(&bar_full[s]), 1); tc::mbar_init(tc::smem_u32(&bar_empty[s]), 1); }
     tc::mbar_init(tc::smem_u32(&bar_tmem), 1);
     tc::fence_barrier_init();
   }
@@ -123,45 +182,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (lane == 0) {
-      for (int it = 0; it < p.n_iters; ++it) {
-        const int s = it % NSTAGE;
-        tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ((it / NSTAGE) & 1) ^ 1);
-        const uint32_t full = tc::smem_u32(&bar_full[s]);
-        tc::mbar_arrive_expect_tx(full, 2 * L * TILE_BYTES);
-        const uint32_t base = smem0 + s * STAGE_BYTES;
-        for (int a = 0; a < L; ++a) {
-          tc::tma_load_3d(base + a * TILE_BYTES, &tmap, full, i0, it * KS, z * 3 + a);
-          tc::tma_load_3d(base + (L + a) * TILE_BYTES, &tmap, full, j0, it * KS, z * 3 + a);
-        }
-      }
-    }
+    if (L == 1) gram_produce<1>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
+    else if (L == 2) gram_produce<2>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
+    else gram_produce<3>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (lane == 0) {
-      constexpr uint32_t idesc = tc::idesc_i8(TM, TN, 1, 1, 1, 1);
-      uint32_t started = 0;   // bit s set once accumulator s holds data
-      for (int it = 0; it < p.n_iters; ++it) {
-        const int s = it % NSTAGE;
-        tc::mbar_wait(tc::smem_u32(&bar_full[s]), (it / NSTAGE) & 1);
-        tc::tc_fence_after();
-        const uint32_t base = smem0 + s * STAGE_BYTES;
-#pragma unroll
-        for (int kk = 0; kk < KS / 32; ++kk) {
-          for (int a = 0; a < L; ++a) {
-            const uint64_t da = tc::smem_desc(base + a * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
-            for (int b = 0; b < L; ++b) {
-              const uint64_t db = tc::smem_desc(base + (L + b) * TILE_BYTES + kk * 32 * BOXW, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
-              const int sidx = a + b;
-              tc::mma_i8(tmem + sidx * TN, da, db, idesc, (started >> sidx) & 1u);
-              started |= 1u << sidx;
-            }
-          }
-        }
-        tc::mma_commit(tc::smem_u32(&bar_empty[s]));     // stage free once these MMAs have read it
-      }
-      tc::mma_commit(tc::smem_u32(&bar_tmem));           // accumulators complete
-    }
+    if (L == 1) gram_issue<1>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    else if (L == 2) gram_issue<2>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    else gram_issue<3>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp % 4) .. +31 =====
     const int q = warp & 3;
