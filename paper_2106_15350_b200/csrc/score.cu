@@ -1,15 +1,108 @@
 // score.cu -- K4: fused logits + argmax + correct-count ("applied the feature vector directly
 // to the Adaline output layer"; accuracy PAPER.md:23), and the search driver's final reduction.
 //
-// One CTA owns 64 test rows of one candidate and walks the classes in chunks of 64 with the fp64 tile
-// engine; the argmax never leaves registers (column-wise best per thread, then a 16-lane shuffle
-// reduction that prefers the larger value and, on equality, the lower class index).
+// The output layer is skinny (c = 10..100 classes), so this is not a tile GEMM: one CTA owns 64 test rows of one
+// candidate, stages 64 x 64 tiles of H (coalesced float4 loads) and the matching 64 x (16 NCH) slab of W in
+// shared memory, and every thread keeps 8 fp64 logits of ONE row in registers (two threads per row; c <= 16).  The
+// products are fp32 x fp32 widened to fp64 (exact), the sums fp64 -- the same arithmetic as the oracle's fp64
+// logits up to summation order; the argmax (first index on ties) and the correct count never leave the CTA.
 #include "internal.h"
 #include "gemm64.cuh"
 
 namespace {
 
-__global__ void __launch_bounds__(g64::NT) score_kernel(const float* __restrict__ U, long long n, long long F,
+constexpr int SC_ROWS = 64, SC_KT = 64, SC_THREADS = 128, SC_LDH = SC_KT + 1;
+
+template <int NCH>
+__global__ void __launch_bounds__(SC_THREADS) score_kernel(const float* __restrict__ U, long long n, long long F, double hs,
+                                                           const float* __restrict__ W, int c, const int32_t* __restrict__ y,
+                                                           int32_t* __restrict__ pred, int32_t* __restrict__ correct) {
+  constexpr int CW = 16 * NCH;                       // classes per pass
+  __shared__ float Hs[SC_ROWS * SC_LDH];
+  __shared__ __align__(16) float Ws[SC_KT * CW];
+  __shared__ int s_ok;
+  const long long z = blockIdx.y;
+  const long long i0 = (long long)blockIdx.x * SC_ROWS;
+  const float* Uz = U + z * n * F;
+  const float* Wz = W + z * F * c;
+  const int t = threadIdx.x, r = t >> 1, h = t & 1;
+  if (t == 0) s_ok = 0;
+  double best = 0.0;
+  int bidx = -1;
+  const bool vec = ((F & 3) == 0) && ((reinterpret_cast<uintptr_t>(Uz) & 15) == 0);
+  for (int cc0 = 0; cc0 < c; cc0 += CW) {
+    double acc[NCH][8];
+#pragma unroll
+    for (int q = 0; q < NCH; ++q)
+#pragma unroll
+      for (int e = 0; e < 8; ++e) acc[q][e] = 0.0;
+    for (long long k0 = 0; k0 < F; k0 += SC_KT) {
+      __syncthreads();                               // previous tile fully consumed
+      if (vec) {
+#pragma unroll
+        for (int q = 0; q < SC_ROWS * SC_KT / 4 / SC_THREADS; ++q) {
+          const int idx = t + SC_THREADS * q, row = idx >> 4, f4 = (idx & 15) * 4;
+          float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (i0 + row < n && k0 + f4 < F) v = __ldcs(reinterpret_cast<const float4*>(Uz + (i0 + row) * F + k0 + f4));
+          float* d = Hs + row * SC_LDH + f4;
+          d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+        }
+      } else {
+        for (int idx = t; idx < SC_ROWS * SC_KT; idx += SC_THREADS) {
+          const int row = idx >> 6, f = idx & 63;
+          Hs[row * SC_LDH + f] = (i0 + row < n && k0 + f < F) ? Uz[(i0 + row) * F + k0 + f] : 0.f;
+        }
+      }
+      for (int idx = t; idx < SC_KT * CW; idx += SC_THREADS) {
+        const int kf = idx / CW, cc = idx - kf * CW;
+        Ws[idx] = (k0 + kf < F && cc0 + cc < c) ? Wz[(k0 + kf) * c + cc0 + cc] : 0.f;
+      }
+      __syncthreads();
+#pragma unroll 4
+      for (int kf = 0; kf < SC_KT; ++kf) {
+        const double hv = (double)Hs[r * SC_LDH + kf];
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) {
+          const float4 w0 = *reinterpret_cast<const float4*>(Ws + kf * CW + q * 16 + h * 8);
+          const float4 w1 = *reinterpret_cast<const float4*>(Ws + kf * CW + q * 16 + h * 8 + 4);
+          acc[q][0] = fma(hv, (double)w0.x, acc[q][0]); acc[q][1] = fma(hv, (double)w0.y, acc[q][1]);
+          acc[q][2] = fma(hv, (double)w0.z, acc[q][2]); acc[q][3] = fma(hv, (double)w0.w, acc[q][3]);
+          acc[q][4] = fma(hv, (double)w1.x, acc[q][4]); acc[q][5] = fma(hv, (double)w1.y, acc[q][5]);
+          acc[q][6] = fma(hv, (double)w1.z, acc[q][6]); acc[q][7] = fma(hv, (double)w1.w, acc[q][7]);
+        }
+      }
+    }
+    // classes of this thread in increasing index order within a chunk; strict '>' keeps the lowest index on ties
+#pragma unroll
+    for (int q = 0; q < NCH; ++q)
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        const int j = cc0 + q * 16 + h * 8 + e;
+        const double l = hs * acc[q][e];
+        if (j < c && (bidx < 0 || l > best || (l == best && j < bidx))) { best = l; bidx = j; }
+      }
+  }
+  {  // the two threads of a row: larger logit wins, the lower class index on equality (R12)
+    const double ov = __shfl_xor_sync(0xffffffffu, best, 1);
+    const int oi = __shfl_xor_sync(0xffffffffu, bidx, 1);
+    if (oi >= 0 && (bidx < 0 || ov > best || (ov == best && oi < bidx))) { best = ov; bidx = oi; }
+  }
+  int ok = 0;
+  if (h == 0 && i0 + r < n) {
+    if (pred) pred[z * n + i0 + r] = bidx;
+    if (y && y[i0 + r] == bidx) ok = 1;
+  }
+  __syncthreads();
+  ok = __reduce_add_sync(0xffffffffu, ok);
+  if ((t & 31) == 0 && ok) atomicAdd(&s_ok, ok);
+  __syncthreads();
+  if (t == 0 && correct && s_ok) atomicAdd(&correct[z], s_ok);
+}
+
+// Wider output layers (c > 16): 64 rows x 64 classes per pass on the fp64 tile engine, the argmax in registers
+// (column-wise best per thread, then a 16-lane shuffle reduction preferring the larger value and, on equality,
+// the lower class index).
+__global__ void __launch_bounds__(g64::NT) score_tile_kernel(const float* __restrict__ U, long long n, long long F,
                                                         double hs, const float* __restrict__ W, int c,
                                                         const int32_t* __restrict__ y, int32_t* __restrict__ pred,
                                                         int32_t* __restrict__ correct) {
@@ -105,8 +198,10 @@ int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, f
     int rc = lb_launch_zero_i32(h, d_correct, n_cand, st);
     if (rc) return rc;
   }
-  dim3 grid((unsigned)((n + 63) / 64), (unsigned)n_cand);
-  score_kernel<<<grid, g64::NT, 0, st>>>(d_H, n, F, (double)h_scale, d_W, n_classes, d_labels, d_pred, d_correct);
+  dim3 grid((unsigned)((n + SC_ROWS - 1) / SC_ROWS), (unsigned)n_cand);
+  const int nch = (n_classes + 15) / 16;             // 16-class chunks; a pass keeps up to four of them in registers
+  if (nch == 1) score_kernel<1><<<grid, SC_THREADS, 0, st>>>(d_H, n, F, (double)h_scale, d_W, n_classes, d_labels, d_pred, d_correct);
+  else score_tile_kernel<<<grid, g64::NT, 0, st>>>(d_H, n, F, (double)h_scale, d_W, n_classes, d_labels, d_pred, d_correct);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;
