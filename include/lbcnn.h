@@ -11,7 +11,10 @@
  *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch allocations); pointers
  *     named h_* and all struct / out-parameter pointers are HOST pointers.  The library never
  *     allocates, frees or retains device memory; scratch comes from the caller-provided workspace
- *     (lbcnn_set_workspace).  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *     (lbcnn_set_workspace).  One exception, owned by the handle: the tensor-core expander keeps a small
+ *     stream-ordered scratch buffer (cudaMallocAsync on the call's stream, grown on demand, freed by
+ *     lbcnn_destroy) holding the +-1 kernel sets re-laid-out as MMA operands (about 10 KB per candidate).
+ *     `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - Every call returns an int status (LBCNN_OK = 0 ...) and only ENQUEUES work on `stream`; it
  *     never synchronises.  Numerical failure is not a status: a non-positive Cholesky pivot j
  *     writes d_info[k] = j + 1 (LAPACK convention) for candidate k and the batch continues.
@@ -107,6 +110,14 @@ int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
 int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_images /*[n][H][W][C]*/, int64_t n,
                  const int8_t* d_kernels /*[n_cand][n_weights]*/, const int32_t* d_bias /*[n_cand][n_bias] or NULL*/,
                  int32_t n_cand, float* d_H /*[n_cand][n][F]*/, void* stream);
+
+/* Which kernel lbcnn_expand takes for this architecture (host-only; `h` supplies the device's shared-memory limit):
+ * LBCNN_EXPAND_TENSOR = the tcgen05 int8 implicit-GEMM kernel (FULL convolutions, 1-2 layers, pooling with
+ * k = s in {1,2,4}, p = 0, no cover_all, sizes divisible by the pool, no bias, layer-1 Cout <= 16 when a second layer
+ * follows, 255 k^2 Cin <= 8191); LBCNN_EXPAND_SIMT = the exact int32 kernel that covers everything else
+ * (depthwise, three layers, padded / overlapping / cover_all pooling, bias).  Both compute the same integers. */
+enum { LBCNN_EXPAND_SIMT = 0, LBCNN_EXPAND_TENSOR = 1 };
+int lbcnn_expand_path(lbcnn_handle_t h, const lbcnn_arch_t* arch, int32_t has_bias, int32_t* path);
 
 /* ELM0 fit: W = argmin ||h_scale*H W - T||^2 + ||W||^2 / C with T the one-hot
  * ("categorical") coding of the labels, i.e.

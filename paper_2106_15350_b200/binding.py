@@ -17,11 +17,12 @@ OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA = rang
 CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
+EXPAND_SIMT, EXPAND_TENSOR = 0, 1
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
-           "lbcnn_launch_count", "lbcnn_set_profiling",
+           "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path",
            "lbcnn_get_phase_times")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
@@ -189,6 +190,12 @@ class Handle:
         if self._ws is None or self._ws.numel() < nbytes:
             self._ws = None
             self.set_workspace(torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % self.device))
+
+    def expand_path(self, arch: Arch, has_bias: bool = False) -> int:
+        """EXPAND_TENSOR (tcgen05 kernel) or EXPAND_SIMT (exact int32 kernel) for this architecture."""
+        p = C.c_int32()
+        _check(lib().lbcnn_expand_path(self._h, C.byref(arch), C.c_int32(int(has_bias)), C.byref(p)), "lbcnn_expand_path")
+        return p.value
 
     def launch_count(self) -> int:
         n = C.c_int64()

@@ -220,6 +220,15 @@ int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_im
   return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, (cudaStream_t)stream);
 }
 
+int lbcnn_expand_path(lbcnn_handle_t h, const lbcnn_arch_t* arch, int32_t has_bias, int32_t* path) {
+  if (!h || !arch || !path) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  *path = (!h->force_simt_expand && lb_expand_tc_usable(h, s, has_bias != 0)) ? LBCNN_EXPAND_TENSOR : LBCNN_EXPAND_SIMT;
+  return LBCNN_OK;
+}
+
 int lbcnn_elm_fit(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, float h_scale, uint32_t flags,
                   const int32_t* d_labels, int32_t n_classes, float C, int32_t n_cand, float* d_W, int32_t* d_info,
                   void* stream) {

@@ -99,6 +99,60 @@ def test_expand_variants_with_bias(handle, name, shape, layers):
             assert np.array_equal(H[k].astype(np.int64), u), (name, use_bias, k)
 
 
+def _tc_envelope_cases():
+    F = lb.CONV_FULL
+    return [
+        # relu on both layers, odd channel counts, ragged image batch and candidate split
+        ("relu2", (20, 24, 1), [(F, 6, 3, 1, 2, 2, 0, 0), (F, 9, 3, 1, 2, 2, 0, 0)], 23, 5),
+        # single layer without pooling (one phase) and with 2x2 pooling
+        ("one_layer_nopool", (16, 16, 3), [(F, 16, 3, 0, 1, 1, 0, 0)], 9, 4),
+        ("one_layer_pool2", (18, 14, 2), [(F, 7, 3, 0, 2, 2, 0, 0)], 19, 3),
+        # 5x5 kernels with 4x4 pooling (configs[3]'s family) on a non-square image
+        ("k5_pool4", (24, 20, 2), [(F, 5, 5, 0, 4, 4, 0, 0)], 7, 6),
+        # second layer without pooling and with more than 32 kernels
+        ("l2_nopool_wide", (12, 12, 1), [(F, 3, 3, 0, 2, 2, 0, 0), (F, 40, 3, 0, 1, 1, 0, 0)], 11, 3),
+        # 5x5 kernels in both layers (run-time tap loop of the layer-2 issuer)
+        ("k5_k5", (16, 16, 1), [(F, 8, 5, 0, 2, 2, 0, 0), (F, 17, 5, 1, 2, 2, 0, 0)], 10, 3),
+        # 4x4 pooling feeding a second layer
+        ("pool4_then_pool2", (32, 32, 1), [(F, 4, 3, 0, 4, 4, 0, 0), (F, 12, 3, 0, 2, 2, 0, 0)], 13, 2),
+        # many candidates over few images: candidate groups per CTA, last group ragged
+        ("many_cands", (28, 28, 1), [(F, 10, 3, 0, 2, 2, 0, 0), (F, 20, 3, 0, 2, 2, 0, 0)], 50, 70),
+    ]
+
+
+@pytest.mark.parametrize("name,shape,layers,n,K", _tc_envelope_cases(), ids=[c[0] for c in _tc_envelope_cases()])
+def test_expand_tensor_core_envelope(handle, name, shape, layers, n, K):
+    """architectures inside the tcgen05 expander's envelope: the tensor-core kernel must be the one taken and its
+    integers must equal the oracle's (and extreme pixels 0 / 255 must not overflow the int8 digits)."""
+    rng = np.random.default_rng(zlib.crc32(name.encode()))
+    x = rng.integers(0, 256, size=(n,) + shape, dtype=np.uint8)
+    x[0] = 255
+    x[-1] = 0
+    arch = lb.make_arch(*shape, layers, 1.0)
+    assert handle.expand_path(arch) == lb.EXPAND_TENSOR, name
+    nw, _ = lb.kernel_set_size(arch)
+    ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+    ker[0] = 1          # all +1: the largest layer-1 sums
+    H = handle.expand(arch, _dev(x), _dev(ker)).cpu().numpy()
+    oa = orc.make_arch(*shape, layers)
+    for k in range(min(K, 6)):
+        u = orc.expand(oa, x, ker[k])
+        assert np.array_equal(H[k].astype(np.int64), u), (name, k)
+    if K > 6:
+        u = orc.expand(oa, x, ker[K - 1])
+        assert np.array_equal(H[K - 1].astype(np.int64), u), (name, K - 1)
+
+
+def test_expand_path_selection(handle):
+    F, D = lb.CONV_FULL, lb.CONV_DEPTHWISE
+    for name in ("tiny_mnist", "mnist", "gtsrb", "orl", "vggface"):
+        assert handle.expand_path(lb.arch_of(synth.WORKLOADS[name], 1.0)) == lb.EXPAND_TENSOR, name
+    assert handle.expand_path(lb.arch_of(synth.WORKLOADS["paper_anchor"], 1.0)) == lb.EXPAND_SIMT     # depthwise, cover_all
+    assert handle.expand_path(lb.arch_of(synth.WORKLOADS["mnist"], 1.0), has_bias=True) == lb.EXPAND_SIMT
+    assert handle.expand_path(lb.make_arch(28, 28, 1, [(F, 10, 3, 0, 4, 2, 1, 1)], 1.0)) == lb.EXPAND_SIMT  # overlapping pool
+    assert handle.expand_path(lb.make_arch(28, 28, 1, [(F, 20, 3, 0, 2, 2, 0, 0), (F, 8, 3, 0, 2, 2, 0, 0)], 1.0)) == lb.EXPAND_SIMT
+
+
 def test_expand_scaled_features(handle):
     w = _small("gtsrb", 17, 4, 2)
     trx, _, _, _ = synth.make_dataset(w)
