@@ -97,12 +97,15 @@ __global__ void __launch_bounds__(128) rhs_primal_kernel(const float* __restrict
   if (f >= F) return;
   const float* Uz = U + z * n * F + f;
   const int lo = off[cls], hi = off[cls + 1];
+  // eight independent row loads in flight per thread (the rows of one class are scattered over the sample axis)
   double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
   int i = lo;
-  for (; i + 3 < hi; i += 4) {
-    const float v0 = Uz[(long long)perm[i] * F], v1 = Uz[(long long)perm[i + 1] * F];
-    const float v2 = Uz[(long long)perm[i + 2] * F], v3 = Uz[(long long)perm[i + 3] * F];
-    s0 += v0; s1 += v1; s2 += v2; s3 += v3;
+  for (; i + 7 < hi; i += 8) {
+    float v[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = __ldcs(Uz + (long long)perm[i + q] * F);
+    s0 += (double)v[0] + (double)v[4]; s1 += (double)v[1] + (double)v[5];
+    s2 += (double)v[2] + (double)v[6]; s3 += (double)v[3] + (double)v[7];
   }
   for (; i < hi; ++i) s0 += Uz[(long long)perm[i] * F];
   A[z * a_stride + (dim + cls) * dim + f] = (s0 + s1) + (s2 + s3);

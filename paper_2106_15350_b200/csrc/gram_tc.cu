@@ -42,46 +42,57 @@ struct GramTcParams {
 };
 
 // ---- digit split ----------------------------------------------------------------------------------
-// thread = 4 consecutive features of one sample of one candidate: one coalesced float4 load, one 32-bit
-// store per digit plane (a warp writes 128 contiguous bytes per plane)
+// Balanced radix-256 digits without branches: d0 = low byte of u (as int8), d1 = byte 1 of u + 128, d2 = byte 2 of
+// u + 128 + 32768 (the carries of the balanced representation are exactly those two additions); a second digit
+// is needed iff (u + 128) >> 8 != 0, a third iff (u + 32896) >> 16 != 0.  A thread converts 8 consecutive
+// features of one sample (two float4 loads) and writes 8 bytes per plane; byte packing is three PRMTs per word.
+__device__ __forceinline__ uint32_t pack_bytes(uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t sel) {
+  // byte `sel` (0..2) of a, b, c, d -> one word
+  const uint32_t s2 = sel | ((sel + 4) << 4);
+  return __byte_perm(__byte_perm(a, b, s2), __byte_perm(c, d, s2), 0x5410);
+}
 __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
                                                     int8_t* __restrict__ planes, int32_t* __restrict__ nlimb) {
   const int z = blockIdx.y;
-  const long long quads_per_row = Fp / 4;
+  const long long oct_per_row = Fp / 8;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  int need = 1;
-  if (t < n * quads_per_row) {
-    const long long row = t / quads_per_row;
-    const int f0 = (int)(t % quads_per_row) * 4;
+  uint32_t or2 = 0, or3 = 0;
+  if (t < n * oct_per_row) {
+    const long long row = t / oct_per_row;
+    const int f0 = (int)(t % oct_per_row) * 8;
     const float* src = U + ((long long)z * n + row) * F + f0;
-    int v[4];
-    if ((F & 3) == 0 && f0 + 4 <= F) {
+    int v[8];
+    if ((F & 3) == 0 && f0 + 8 <= F) {
       const float4 x = __ldcs(reinterpret_cast<const float4*>(src));
+      const float4 y = __ldcs(reinterpret_cast<const float4*>(src) + 1);
       v[0] = (int)x.x; v[1] = (int)x.y; v[2] = (int)x.z; v[3] = (int)x.w;
+      v[4] = (int)y.x; v[5] = (int)y.y; v[6] = (int)y.z; v[7] = (int)y.w;
     } else {
 #pragma unroll
-      for (int q = 0; q < 4; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
+      for (int q = 0; q < 8; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
     }
-    uint32_t w[3] = {0, 0, 0};
+    uint32_t t1[8], t2[8];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const int u = v[q];
-      const int d0 = ((u + 128) & 255) - 128;
-      const int u1 = (u - d0) >> 8;
-      const int d1 = ((u1 + 128) & 255) - 128;
-      const int d2 = (u1 - d1) >> 8;
-      if (u1 != 0) need = max(need, 2);
-      if (d2 != 0) need = max(need, 3);
-      w[0] |= (uint32_t)(d0 & 255) << (8 * q);
-      w[1] |= (uint32_t)(d1 & 255) << (8 * q);
-      w[2] |= (uint32_t)(d2 & 255) << (8 * q);
+    for (int q = 0; q < 8; ++q) {
+      t1[q] = (uint32_t)(v[q] + 128);
+      t2[q] = (uint32_t)(v[q] + 32896);
+      or2 |= t1[q] & 0xFFFFFF00u;
+      or3 |= t2[q] & 0xFFFF0000u;
     }
-#pragma unroll
-    for (int l = 0; l < 3; ++l) {
-      int8_t* dst = planes + (((long long)z * 3 + l) * n + row) * Fp + f0;
-      *reinterpret_cast<uint32_t*>(dst) = w[l];
-    }
+    uint2 w0, w1, w2;
+    w0.x = pack_bytes((uint32_t)v[0], (uint32_t)v[1], (uint32_t)v[2], (uint32_t)v[3], 0);
+    w0.y = pack_bytes((uint32_t)v[4], (uint32_t)v[5], (uint32_t)v[6], (uint32_t)v[7], 0);
+    w1.x = pack_bytes(t1[0], t1[1], t1[2], t1[3], 1);
+    w1.y = pack_bytes(t1[4], t1[5], t1[6], t1[7], 1);
+    w2.x = pack_bytes(t2[0], t2[1], t2[2], t2[3], 2);
+    w2.y = pack_bytes(t2[4], t2[5], t2[6], t2[7], 2);
+    int8_t* dst = planes + ((long long)z * 3 * n + row) * Fp + f0;
+    const long long plane = n * (long long)Fp;
+    *reinterpret_cast<uint2*>(dst) = w0;
+    *reinterpret_cast<uint2*>(dst + plane) = w1;
+    *reinterpret_cast<uint2*>(dst + 2 * plane) = w2;
   }
+  int need = or3 ? 3 : (or2 ? 2 : 1);
   need = __reduce_max_sync(0xffffffffu, need);
   // one atomic per warp only while it can still raise the count: after the first few warps of a candidate the
   // (L2-cached) read already shows the final value and no further atomics reach that address
@@ -263,7 +274,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   fill_i32_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(nlimb, n_cand, 1);
   h->launches += 1;
   {
-    const long long work = n * (Fp / 4);
+    const long long work = n * (Fp / 8);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
     split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb);
     h->launches += 1;

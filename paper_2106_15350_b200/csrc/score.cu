@@ -3,11 +3,11 @@
 //
 // The output layer is skinny (c = 10..100 classes), so this is not a tile GEMM: one CTA owns 64 test rows of one
 // candidate, stages 64 x 64 tiles of H (coalesced float4 loads) and the matching 64 x (16 NCH) slab of W in
-// shared memory, and every thread keeps 8 fp64 logits of ONE row in registers (two threads per row; c <= 16).  The
+// shared memory (widened to fp64 once per tile), and every thread keeps 8 NCH fp64 logits of ONE row in registers
+// (two threads per row; up to 64 classes per pass).  The
 // products are fp32 x fp32 widened to fp64 (exact), the sums fp64 -- the same arithmetic as the oracle's fp64
 // logits up to summation order; the argmax (first index on ties) and the correct count never leave the CTA.
 #include "internal.h"
-#include "gemm64.cuh"
 
 namespace {
 
@@ -18,8 +18,9 @@ __global__ void __launch_bounds__(SC_THREADS) score_kernel(const float* __restri
                                                            const float* __restrict__ W, int c, const int32_t* __restrict__ y,
                                                            int32_t* __restrict__ pred, int32_t* __restrict__ correct) {
   constexpr int CW = 16 * NCH;                       // classes per pass
-  __shared__ float Hs[SC_ROWS * SC_LDH];
-  __shared__ __align__(16) float Ws[SC_KT * CW];
+  extern __shared__ __align__(16) double sc_smem[];     // widened once per tile: F2F in the inner loop would bound it
+  double* Hs = sc_smem;                                 // [SC_ROWS][SC_LDH]
+  double* Ws = sc_smem + SC_ROWS * SC_LDH;              // [SC_KT][CW], 16-byte aligned (SC_ROWS * SC_LDH is even)
   __shared__ int s_ok;
   const long long z = blockIdx.y;
   const long long i0 = (long long)blockIdx.x * SC_ROWS;
@@ -44,31 +45,32 @@ __global__ void __launch_bounds__(SC_THREADS) score_kernel(const float* __restri
           const int idx = t + SC_THREADS * q, row = idx >> 4, f4 = (idx & 15) * 4;
           float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
           if (i0 + row < n && k0 + f4 < F) v = __ldcs(reinterpret_cast<const float4*>(Uz + (i0 + row) * F + k0 + f4));
-          float* d = Hs + row * SC_LDH + f4;
-          d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+          double* d = Hs + row * SC_LDH + f4;
+          d[0] = (double)v.x; d[1] = (double)v.y; d[2] = (double)v.z; d[3] = (double)v.w;
         }
       } else {
         for (int idx = t; idx < SC_ROWS * SC_KT; idx += SC_THREADS) {
           const int row = idx >> 6, f = idx & 63;
-          Hs[row * SC_LDH + f] = (i0 + row < n && k0 + f < F) ? Uz[(i0 + row) * F + k0 + f] : 0.f;
+          Hs[row * SC_LDH + f] = (i0 + row < n && k0 + f < F) ? (double)Uz[(i0 + row) * F + k0 + f] : 0.0;
         }
       }
       for (int idx = t; idx < SC_KT * CW; idx += SC_THREADS) {
         const int kf = idx / CW, cc = idx - kf * CW;
-        Ws[idx] = (k0 + kf < F && cc0 + cc < c) ? Wz[(k0 + kf) * c + cc0 + cc] : 0.f;
+        Ws[idx] = (k0 + kf < F && cc0 + cc < c) ? (double)Wz[(k0 + kf) * c + cc0 + cc] : 0.0;
       }
       __syncthreads();
 #pragma unroll 4
       for (int kf = 0; kf < SC_KT; ++kf) {
-        const double hv = (double)Hs[r * SC_LDH + kf];
+        const double hv = Hs[r * SC_LDH + kf];
 #pragma unroll
         for (int q = 0; q < NCH; ++q) {
-          const float4 w0 = *reinterpret_cast<const float4*>(Ws + kf * CW + q * 16 + h * 8);
-          const float4 w1 = *reinterpret_cast<const float4*>(Ws + kf * CW + q * 16 + h * 8 + 4);
-          acc[q][0] = fma(hv, (double)w0.x, acc[q][0]); acc[q][1] = fma(hv, (double)w0.y, acc[q][1]);
-          acc[q][2] = fma(hv, (double)w0.z, acc[q][2]); acc[q][3] = fma(hv, (double)w0.w, acc[q][3]);
-          acc[q][4] = fma(hv, (double)w1.x, acc[q][4]); acc[q][5] = fma(hv, (double)w1.y, acc[q][5]);
-          acc[q][6] = fma(hv, (double)w1.z, acc[q][6]); acc[q][7] = fma(hv, (double)w1.w, acc[q][7]);
+          const double2* wp = reinterpret_cast<const double2*>(Ws + kf * CW + q * 16 + h * 8);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const double2 w = wp[e];
+            acc[q][2 * e] = fma(hv, w.x, acc[q][2 * e]);
+            acc[q][2 * e + 1] = fma(hv, w.y, acc[q][2 * e + 1]);
+          }
         }
       }
     }
@@ -97,63 +99,6 @@ __global__ void __launch_bounds__(SC_THREADS) score_kernel(const float* __restri
   if ((t & 31) == 0 && ok) atomicAdd(&s_ok, ok);
   __syncthreads();
   if (t == 0 && correct && s_ok) atomicAdd(&correct[z], s_ok);
-}
-
-// Wider output layers (c > 16): 64 rows x 64 classes per pass on the fp64 tile engine, the argmax in registers
-// (column-wise best per thread, then a 16-lane shuffle reduction preferring the larger value and, on equality,
-// the lower class index).
-__global__ void __launch_bounds__(g64::NT) score_tile_kernel(const float* __restrict__ U, long long n, long long F,
-                                                        double hs, const float* __restrict__ W, int c,
-                                                        const int32_t* __restrict__ y, int32_t* __restrict__ pred,
-                                                        int32_t* __restrict__ correct) {
-  __shared__ g64::Smem sm;
-  __shared__ int s_ok;
-  const long long z = blockIdx.y;
-  const int i0 = blockIdx.x * 64;
-  const float* Uz = U + z * n * F;
-  const float* Wz = W + z * F * c;
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  if (threadIdx.x == 0) s_ok = 0;
-  double best[4];
-  int bidx[4];
-#pragma unroll
-  for (int a = 0; a < 4; ++a) { best[a] = 0.0; bidx[a] = -1; }
-  for (int j0 = 0; j0 < c; j0 += 64) {
-    double acc[4][4];
-    g64::tile_mma<float, float, true, false>(sm, Uz, F, 1, i0, (int)n, Wz, 1, c, j0, c, (int)F, acc);
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      double v = 0.0; int idx = -1;
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const int j = j0 + tx + 16 * b;
-        const double l = hs * acc[a][b];
-        if (j < c && (idx < 0 || l > v)) { v = l; idx = j; }
-      }
-#pragma unroll
-      for (int d = 8; d >= 1; d >>= 1) {
-        const double ov = __shfl_xor_sync(0xffffffffu, v, d);
-        const int oi = __shfl_xor_sync(0xffffffffu, idx, d);
-        if (oi >= 0 && (idx < 0 || ov > v || (ov == v && oi < idx))) { v = ov; idx = oi; }
-      }
-      if (idx >= 0 && (bidx[a] < 0 || v > best[a])) { best[a] = v; bidx[a] = idx; }   // later chunks have larger indices
-    }
-  }
-  int ok = 0;
-  if (tx == 0) {
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      const long long i = i0 + ty + 16 * a;
-      if (i < n) {
-        if (pred) pred[z * n + i] = bidx[a];
-        if (y && y[i] == bidx[a]) ok += 1;
-      }
-    }
-  }
-  __syncthreads();
-  if (ok) atomicAdd(&s_ok, ok);
-  __syncthreads();
-  if (threadIdx.x == 0 && correct && s_ok) atomicAdd(&correct[z], s_ok);
 }
 
 __global__ void zero_i32_kernel(int32_t* p, long long n) {
@@ -200,8 +145,18 @@ int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, f
   }
   dim3 grid((unsigned)((n + SC_ROWS - 1) / SC_ROWS), (unsigned)n_cand);
   const int nch = (n_classes + 15) / 16;             // 16-class chunks; a pass keeps up to four of them in registers
-  if (nch == 1) score_kernel<1><<<grid, SC_THREADS, 0, st>>>(d_H, n, F, (double)h_scale, d_W, n_classes, d_labels, d_pred, d_correct);
-  else score_tile_kernel<<<grid, g64::NT, 0, st>>>(d_H, n, F, (double)h_scale, d_W, n_classes, d_labels, d_pred, d_correct);
+  const double hs = (double)h_scale;
+#define LB_SCORE(NCH)                                                                                                     \
+  do {                                                                                                                    \
+    const size_t sm = sizeof(double) * (SC_ROWS * SC_LDH + SC_KT * 16 * NCH);                                         \
+    LB_CUDA_OK(cudaFuncSetAttribute(score_kernel<NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));            \
+    score_kernel<NCH><<<grid, SC_THREADS, sm, st>>>(d_H, n, F, hs, d_W, n_classes, d_labels, d_pred, d_correct);         \
+  } while (0)
+  if (nch == 1) LB_SCORE(1);
+  else if (nch == 2) LB_SCORE(2);
+  else if (nch == 3) LB_SCORE(3);
+  else LB_SCORE(4);
+#undef LB_SCORE
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;
