@@ -103,6 +103,8 @@ int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t*
 int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
                           int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes);
 int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
+/* Workspace a stand-alone lbcnn_elm_fit(n, F, n_classes, n_cand, flags) needs (host-only arithmetic). */
+int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes);
 
 /* Expander: d_H[k][i][:] = feature_scale * flatten(layers(image i; kernel set k)).
  * The integer feature is exact (signed adds of uint8 pixels, abs < 2^24); the only rounding is the

@@ -22,7 +22,7 @@ EXPAND_SIMT, EXPAND_TENSOR = 0, 1
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
-           "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path",
+           "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
            "lbcnn_get_phase_times")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
@@ -118,6 +118,13 @@ def workspace_bytes(arch: Arch, n_train: int, n_test: int, n_classes: int, n_can
                                        C.c_int32(n_cand), C.c_size_t(budget_bytes), C.byref(b), C.byref(m)),
            "lbcnn_workspace_bytes")
     return b.value, m.value
+
+
+def fit_workspace_bytes(n: int, F: int, n_classes: int, n_cand: int, flags: int = 0) -> int:
+    b = C.c_size_t()
+    _check(lib().lbcnn_fit_workspace_bytes(C.c_int64(n), C.c_int64(F), C.c_int32(n_classes), C.c_int32(n_cand),
+                                           C.c_uint32(flags), C.byref(b)), "lbcnn_fit_workspace_bytes")
+    return b.value
 
 
 def host_staging_bytes(arch: Arch, n_train: int, n_test: int, n_classes: int, n_cand: int, has_bias: bool = False) -> int:

@@ -220,6 +220,14 @@ int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_im
   return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, (cudaStream_t)stream);
 }
 
+int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes) {
+  if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  FitPlan p;
+  lb_fit_plan(n, F, n_classes, n_cand, flags, &p);
+  *bytes = p.total;
+  return LBCNN_OK;
+}
+
 int lbcnn_expand_path(lbcnn_handle_t h, const lbcnn_arch_t* arch, int32_t has_bias, int32_t* path) {
   if (!h || !arch || !path) return LBCNN_ERR_INVALID_ARG;
   ArchShape s;

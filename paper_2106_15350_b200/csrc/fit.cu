@@ -35,23 +35,24 @@ __global__ void __launch_bounds__(g64::NT) gemm_kernel(const GemmP p) {
   const TA* A = reinterpret_cast<const TA*>(p.A) + z * p.bA;
   const TB* B = reinterpret_cast<const TB*>(p.B) + z * p.bB;
   TC* C = reinterpret_cast<TC*>(p.C) + z * p.bC;
-  double acc[4][4];
+  double acc[2][4][2];
   g64::tile_mma<TA, TB, AK, BK>(sm, A, p.sAr, p.sAk, ti * 64, p.M, B, p.sBr, p.sBk, tj * 64, p.N, p.K, acc);
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
 #pragma unroll
-  for (int a = 0; a < 4; ++a) {
-    const int i = ti * 64 + ty + 16 * a;
+  for (int m = 0; m < 2; ++m) {
+    const int i = ti * 64 + g64::frag_row(m);
     if (i >= p.M) continue;
 #pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      const int j = tj * 64 + tx + 16 * b;
-      if (j >= p.N) continue;
-      double v = p.alpha * acc[a][b];
-      if (i == j) v += p.diag;
-      TC* c = C + (long long)i * p.ldc + j;
-      if (p.accumulate) v += (double)*c;
-      *c = (TC)v;
-    }
+    for (int nb = 0; nb < 4; ++nb)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int j = tj * 64 + g64::frag_col(nb, e);
+        if (j >= p.N) continue;
+        double v = p.alpha * acc[m][nb][e];
+        if (i == j) v += p.diag;
+        TC* c = C + (long long)i * p.ldc + j;
+        if (p.accumulate) v += (double)*c;
+        *c = (TC)v;
+      }
   }
 }
 
@@ -127,9 +128,14 @@ __global__ void rhs_dual_kernel(const int32_t* __restrict__ y, long long n, int 
 
 // factorise the nbj x nbj diagonal block at (j0, j0); a non-positive pivot records info = index + 1
 // (first failure wins) and continues with pivot 1 so that the candidate's data stays finite.
+// Also writes Linv = L11^-1 (nbj x nbj, lower triangular, zeros above the diagonal, pitch NB) to
+// linv + blockIdx.x * linv_stride: the panel solve and the backward sweep then are plain products.
 __global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A, long long a_stride, long long ld,
-                                                         int j0, int nbj, int32_t* __restrict__ info) {
-  __shared__ double S[NB][NB + 1];
+                                                         int j0, int nbj, int32_t* __restrict__ info,
+                                                         double* __restrict__ linv, long long linv_stride) {
+  extern __shared__ double potrf_sh[];
+  double (*S)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(potrf_sh);
+  double (*X)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(potrf_sh + NB * (NB + 1));
   double* Az = A + blockIdx.x * a_stride + (long long)j0 * ld + j0;
   for (int e = threadIdx.x; e < nbj * nbj; e += blockDim.x) {
     const int i = e / nbj, c = e % nbj;
@@ -159,63 +165,23 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A,
     const int i = e / nbj, c = e % nbj;
     if (c <= i) Az[(long long)i * ld + c] = S[i][c];
   }
-}
-
-// rows below the diagonal block (including the appended right-hand-side rows): X = A21 * L11^-T.
-// One thread per row, the row and L11 in shared memory.
-__global__ void __launch_bounds__(64) trsm_panel_kernel(double* __restrict__ A, long long a_stride, long long ld,
-                                                        int j0, int nbj, long long rows) {
-  extern __shared__ double sh[];
-  double (*Ls)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh);
-  double (*Rs)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh + NB * (NB + 1));
-  double* Az = A + blockIdx.y * a_stride;
-  const double* L11 = Az + (long long)j0 * ld + j0;
-  const long long r0 = (long long)j0 + nbj + (long long)blockIdx.x * 64;
-  const int t = threadIdx.x;
-  for (int i = 0; i < nbj; ++i)
-    if (t < nbj) Ls[i][t] = L11[(long long)i * ld + t];
-  const int nr = (int)min((long long)64, rows - r0);
-  for (int i = 0; i < nr; ++i)
-    if (t < nbj) Rs[i][t] = Az[(r0 + i) * ld + j0 + t];
-  __syncthreads();
-  if (t < nr) {
-    for (int c = 0; c < nbj; ++c) {
-      const double x = Rs[t][c] / Ls[c][c];
-      Rs[t][c] = x;
-      for (int c2 = c + 1; c2 < nbj; ++c2) Rs[t][c2] -= x * Ls[c2][c];
+  // inverse of the triangular factor, one column per thread by forward substitution (X = L^-1: L X = I)
+  if (threadIdx.x < nbj) {
+    const int c = threadIdx.x;
+    for (int i = 0; i < c; ++i) X[i][c] = 0.0;
+    X[c][c] = 1.0 / S[c][c];
+    for (int i = c + 1; i < nbj; ++i) {
+      double acc = 0.0;
+      for (int k = c; k < i; ++k) acc = fma(S[i][k], X[k][c], acc);
+      X[i][c] = -acc / S[i][i];
     }
   }
   __syncthreads();
-  for (int i = 0; i < nr; ++i)
-    if (t < nbj) Az[(r0 + i) * ld + j0 + t] = Rs[i][t];
-}
-
-// backward sweep, diagonal step: rows of Y^T (one per class) x * L_jj = y, solved from the last column.
-__global__ void __launch_bounds__(64) bs_diag_kernel(double* __restrict__ A, long long a_stride, long long ld,
-                                                     long long dim, int j0, int nbj, int c) {
-  extern __shared__ double sh[];
-  double (*Ls)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh);
-  double (*Rs)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(sh + NB * (NB + 1));
-  double* Az = A + blockIdx.y * a_stride;
-  const double* L11 = Az + (long long)j0 * ld + j0;
-  const int r0 = blockIdx.x * 64;
-  const int t = threadIdx.x;
-  for (int i = 0; i < nbj; ++i)
-    if (t < nbj) Ls[i][t] = (t <= i) ? L11[(long long)i * ld + t] : 0.0;
-  const int nr = min(64, c - r0);
-  for (int i = 0; i < nr; ++i)
-    if (t < nbj) Rs[i][t] = Az[(dim + r0 + i) * ld + j0 + t];
-  __syncthreads();
-  if (t < nr) {
-    for (int cc = nbj - 1; cc >= 0; --cc) {
-      const double x = Rs[t][cc] / Ls[cc][cc];
-      Rs[t][cc] = x;
-      for (int c2 = 0; c2 < cc; ++c2) Rs[t][c2] -= x * Ls[cc][c2];
-    }
+  double* Lz = linv + blockIdx.x * linv_stride;
+  for (int e = threadIdx.x; e < NB * NB; e += blockDim.x) {
+    const int i = e / NB, c = e % NB;
+    Lz[e] = (i < nbj && c < nbj) ? X[i][c] : 0.0;
   }
-  __syncthreads();
-  for (int i = 0; i < nr; ++i)
-    if (t < nbj) Az[(dim + r0 + i) * ld + j0 + t] = Rs[i][t];
 }
 
 // primal: W[f][cls] = X^T[cls][f] / s, rounded once to fp32
@@ -246,6 +212,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
   p->use_tc = ((flags & LBCNN_H_INTEGER) && primal && lb_gram_tc_usable(n, F)) ? 1 : 0;
   p->tc_off = off;   if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand);
+  p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   p->total = off;
 }
 
@@ -309,41 +276,69 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   LB_CUDA_OK(cudaGetLastError());
 
   LbPhase ph3(h, LBCNN_PHASE_SOLVE, st);
-  const size_t tr_smem = 2 * NB * (NB + 1) * sizeof(double);
-  LB_CUDA_OK(cudaFuncSetAttribute(trsm_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));
-  LB_CUDA_OK(cudaFuncSetAttribute(bs_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tr_smem));
+  double* Linv = reinterpret_cast<double*>(base + pl.linv_off);
+  const long long nblk = (dim + NB - 1) / NB;
+  const long long linv_stride = nblk * NB * NB;
 
-  // F3: right-looking blocked Cholesky over dim + c rows
-  for (long long j0 = 0; j0 < dim; j0 += NB) {
-    const int nbj = (int)((dim - j0 < NB) ? dim - j0 : NB);
-    potrf_diag_kernel<<<n_cand, 256, 0, st>>>(A, a_stride, ld, (int)j0, nbj, d_info);
-    h->launches += 1;
-    const long long below = rows - (j0 + nbj);
-    if (below > 0) {
-      dim3 gt((unsigned)((below + 63) / 64), (unsigned)n_cand);
-      trsm_panel_kernel<<<gt, 64, tr_smem, st>>>(A, a_stride, ld, (int)j0, nbj, rows);
+  // F3: right-looking blocked Cholesky over dim + c rows with two block sizes.  Inside a panel of NBO columns the
+  // 64-column steps (factor the diagonal block and invert it; panel rows X = A21 L11^-T as a product; update the
+  // REST OF THE PANEL only) touch a narrow strip; the wide trailing matrix is updated once per panel with K = NBO,
+  // which cuts its read-modify-write traffic by NBO / NB.
+  constexpr int NBO = 256;
+  const size_t potrf_smem = 2 * NB * (NB + 1) * sizeof(double);
+  LB_CUDA_OK(cudaFuncSetAttribute(potrf_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)potrf_smem));
+  for (long long J0 = 0; J0 < dim; J0 += NBO) {
+    const long long J1 = (J0 + NBO < dim) ? J0 + NBO : dim;
+    for (long long j0 = J0; j0 < J1; j0 += NB) {
+      const int nbj = (int)((dim - j0 < NB) ? dim - j0 : NB);
+      double* Lj = Linv + (j0 / NB) * NB * NB;
+      potrf_diag_kernel<<<n_cand, 256, potrf_smem, st>>>(A, a_stride, ld, (int)j0, nbj, d_info, Lj, linv_stride);
       h->launches += 1;
       const long long j1 = j0 + nbj;
-      if (dim - j1 > 0) {
-        GemmP g{};
+      if (rows - j1 > 0) {
+        GemmP g{};                                                     // X = A21 * Linv^T, in place (one column tile)
         g.A = A + j1 * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
-        g.B = A + j1 * ld + j0; g.sBr = ld; g.sBk = 1; g.bB = a_stride;
-        g.C = A + j1 * ld + j1; g.ldc = ld; g.bC = a_stride;
-        g.M = (int)(rows - j1); g.N = (int)(dim - j1); g.K = nbj; g.alpha = -1.0; g.accumulate = 1; g.lower = 1;
-        g.diag = 0.0;
+        g.B = Lj; g.sBr = NB; g.sBk = 1; g.bB = linv_stride;
+        g.C = A + j1 * ld + j0; g.ldc = ld; g.bC = a_stride;
+        g.M = (int)(rows - j1); g.N = nbj; g.K = nbj; g.alpha = 1.0; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
         rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
         if (rc) return rc;
+        if (J1 - j1 > 0) {                                             // rest of the panel: columns j1 .. J1-1
+          GemmP u{};
+          u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
+          u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
+          u.C = A + j1 * ld + j1; u.ldc = ld; u.bC = a_stride;
+          u.M = (int)(rows - j1); u.N = (int)(J1 - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
+          rc = launch_gemm<double, double, double, true, true>(h, u, n_cand, st);
+          if (rc) return rc;
+        }
       }
     }
+    if (dim - J1 > 0) {                                                // trailing matrix, K = the whole panel
+      GemmP g{};
+      g.A = A + J1 * ld + J0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
+      g.B = A + J1 * ld + J0; g.sBr = ld; g.sBk = 1; g.bB = a_stride;
+      g.C = A + J1 * ld + J1; g.ldc = ld; g.bC = a_stride;
+      g.M = (int)(rows - J1); g.N = (int)(dim - J1); g.K = (int)(J1 - J0); g.alpha = -1.0; g.accumulate = 1; g.lower = 1;
+      g.diag = 0.0;
+      rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
+      if (rc) return rc;
+    }
   }
-  // backward sweep on the appended rows: X^T L = Y^T, block columns from the last to the first
-  const long long nblk = (dim + NB - 1) / NB;
+  // backward sweep on the appended rows: X^T L = Y^T, block columns from the last to the first;
+  // the diagonal step is X_j = Y_j L_jj^-1 (a product with the stored inverse)
   for (long long jb = nblk - 1; jb >= 0; --jb) {
     const long long j0 = jb * NB;
     const int nbj = (int)((dim - j0 < NB) ? dim - j0 : NB);
-    dim3 gd((unsigned)((c + 63) / 64), (unsigned)n_cand);
-    bs_diag_kernel<<<gd, 64, tr_smem, st>>>(A, a_stride, ld, dim, (int)j0, nbj, c);
-    h->launches += 1;
+    {
+      GemmP g{};
+      g.A = A + dim * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
+      g.B = Linv + jb * NB * NB; g.sBr = 1; g.sBk = NB; g.bB = linv_stride;   // B(j, k) = Linv[k][j]
+      g.C = A + dim * ld + j0; g.ldc = ld; g.bC = a_stride;
+      g.M = c; g.N = nbj; g.K = nbj; g.alpha = 1.0; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
+      rc = launch_gemm<double, double, double, true, false>(h, g, n_cand, st);
+      if (rc) return rc;
+    }
     if (j0 > 0) {
       GemmP g{};
       g.A = A + dim * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;      // X^T[:, block]  (c x nbj)

@@ -69,7 +69,7 @@ struct FitPlan {
   int64_t dim;           // system dimension
   int64_t rows;          // dim + n_classes (right-hand sides appended as rows)
   size_t a_bytes;        // per candidate: rows * dim doubles
-  size_t perm_off, off_off, a_off, tc_off, total; // offsets inside the fit workspace
+  size_t perm_off, off_off, a_off, tc_off, linv_off, total; // offsets inside the fit workspace
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
 };
 void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p);

@@ -1,102 +1,122 @@
 // score.cu -- K4: fused logits + argmax + correct-count ("applied the feature vector directly
 // to the Adaline output layer"; accuracy PAPER.md:23), and the search driver's final reduction.
 //
-// The output layer is skinny (c = 10..100 classes), so this is not a tile GEMM: one CTA owns 64 test rows of one
-// candidate, stages 64 x 64 tiles of H (coalesced float4 loads) and the matching 64 x (16 NCH) slab of W in
-// shared memory (widened to fp64 once per tile), and every thread keeps 8 NCH fp64 logits of ONE row in registers
-// (two threads per row; up to 64 classes per pass).  The
-// products are fp32 x fp32 widened to fp64 (exact), the sums fp64 -- the same arithmetic as the oracle's fp64
-// logits up to summation order; the argmax (first index on ties) and the correct count never leave the CTA.
+// The output layer is skinny (c = 10..100 classes) and the logits are wanted in fp64 (the oracle's arithmetic; with
+// 120-sample test sets a single flipped near-tie already breaks label parity), so this runs on the fp64 tensor
+// path: mma.sync m8n8k4 (DMMA, 64 fp64 FMA/clk/SM on B200 -- the same peak as DFMA but one instruction per 256 FMAs
+// and operands reused from registers, where the plain DFMA loop was bound by shared-memory bandwidth).
+// One CTA owns 128 test rows of one candidate; a warp owns 32 rows x (16 NCH) classes of accumulators.  H tiles
+// (128 x 32, coalesced float4 loads) and the matching W slab are widened to fp64 once when staged into shared
+// memory (products of two fp32 numbers are exact in fp64); the argmax (first index on ties) and the correct count
+// never leave the CTA.
 #include "internal.h"
 
 namespace {
 
-constexpr int SC_ROWS = 64, SC_KT = 64, SC_THREADS = 128, SC_LDH = SC_KT + 1;
+constexpr int SC_ROWS = 128, SC_KT = 32, SC_THREADS = 128;
+constexpr int SC_LDH = SC_KT + 4;        // row pitch of the H tile in doubles: = 4 (mod 16) -> conflict-free A fragments
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
 
 template <int NCH>
 __global__ void __launch_bounds__(SC_THREADS) score_kernel(const float* __restrict__ U, long long n, long long F, double hs,
                                                            const float* __restrict__ W, int c, const int32_t* __restrict__ y,
                                                            int32_t* __restrict__ pred, int32_t* __restrict__ correct) {
-  constexpr int CW = 16 * NCH;                       // classes per pass
-  extern __shared__ __align__(16) double sc_smem[];     // widened once per tile: F2F in the inner loop would bound it
-  double* Hs = sc_smem;                                 // [SC_ROWS][SC_LDH]
-  double* Ws = sc_smem + SC_ROWS * SC_LDH;              // [SC_KT][CW], 16-byte aligned (SC_ROWS * SC_LDH is even)
+  constexpr int CW = 16 * NCH;             // classes per pass
+  constexpr int LDW = CW + 8;              // pitch of the W slab: = 8 (mod 16) -> conflict-free B fragments
+  extern __shared__ __align__(16) double sc_smem[];
+  double* Hs = sc_smem;                    // [SC_ROWS][SC_LDH]
+  double* Ws = sc_smem + SC_ROWS * SC_LDH; // [SC_KT][LDW]
   __shared__ int s_ok;
   const long long z = blockIdx.y;
   const long long i0 = (long long)blockIdx.x * SC_ROWS;
   const float* Uz = U + z * n * F;
   const float* Wz = W + z * F * c;
-  const int t = threadIdx.x, r = t >> 1, h = t & 1;
+  const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+  const int g = lane >> 2, q4 = lane & 3;  // fragment coordinates: row / column group and k index
   if (t == 0) s_ok = 0;
-  double best = 0.0;
-  int bidx = -1;
+  double best[4];
+  int bidx[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { best[m] = 0.0; bidx[m] = -1; }
   const bool vec = ((F & 3) == 0) && ((reinterpret_cast<uintptr_t>(Uz) & 15) == 0);
   for (int cc0 = 0; cc0 < c; cc0 += CW) {
-    double acc[NCH][8];
+    double acc[4][2 * NCH][2];             // [row block of 8][class block of 8][2 columns]
 #pragma unroll
-    for (int q = 0; q < NCH; ++q)
+    for (int m = 0; m < 4; ++m)
 #pragma unroll
-      for (int e = 0; e < 8; ++e) acc[q][e] = 0.0;
+      for (int nb = 0; nb < 2 * NCH; ++nb) { acc[m][nb][0] = 0.0; acc[m][nb][1] = 0.0; }
     for (long long k0 = 0; k0 < F; k0 += SC_KT) {
-      __syncthreads();                               // previous tile fully consumed
+      __syncthreads();                     // previous tile fully consumed
       if (vec) {
 #pragma unroll
         for (int q = 0; q < SC_ROWS * SC_KT / 4 / SC_THREADS; ++q) {
-          const int idx = t + SC_THREADS * q, row = idx >> 4, f4 = (idx & 15) * 4;
+          const int idx = t + SC_THREADS * q, row = idx >> 3, f4 = (idx & 7) * 4;
           float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
           if (i0 + row < n && k0 + f4 < F) v = __ldcs(reinterpret_cast<const float4*>(Uz + (i0 + row) * F + k0 + f4));
-          double* d = Hs + row * SC_LDH + f4;
-          d[0] = (double)v.x; d[1] = (double)v.y; d[2] = (double)v.z; d[3] = (double)v.w;
+          double2* d = reinterpret_cast<double2*>(Hs + row * SC_LDH + f4);
+          d[0] = make_double2((double)v.x, (double)v.y);
+          d[1] = make_double2((double)v.z, (double)v.w);
         }
       } else {
         for (int idx = t; idx < SC_ROWS * SC_KT; idx += SC_THREADS) {
-          const int row = idx >> 6, f = idx & 63;
+          const int row = idx >> 5, f = idx & 31;
           Hs[row * SC_LDH + f] = (i0 + row < n && k0 + f < F) ? (double)Uz[(i0 + row) * F + k0 + f] : 0.0;
         }
       }
       for (int idx = t; idx < SC_KT * CW; idx += SC_THREADS) {
         const int kf = idx / CW, cc = idx - kf * CW;
-        Ws[idx] = (k0 + kf < F && cc0 + cc < c) ? (double)Wz[(k0 + kf) * c + cc0 + cc] : 0.0;
+        Ws[kf * LDW + cc] = (k0 + kf < F && cc0 + cc < c) ? (double)Wz[(k0 + kf) * c + cc0 + cc] : 0.0;
       }
       __syncthreads();
-#pragma unroll 4
-      for (int kf = 0; kf < SC_KT; ++kf) {
-        const double hv = Hs[r * SC_LDH + kf];
+      const double* ha = Hs + (warp * 32 + g) * SC_LDH + q4;
+      const double* wb = Ws + q4 * LDW + g;
 #pragma unroll
-        for (int q = 0; q < NCH; ++q) {
-          const double2* wp = reinterpret_cast<const double2*>(Ws + kf * CW + q * 16 + h * 8);
+      for (int k4 = 0; k4 < SC_KT; k4 += 4) {
+        double a[4], b[2 * NCH];
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const double2 w = wp[e];
-            acc[q][2 * e] = fma(hv, w.x, acc[q][2 * e]);
-            acc[q][2 * e + 1] = fma(hv, w.y, acc[q][2 * e + 1]);
-          }
-        }
+        for (int m = 0; m < 4; ++m) a[m] = ha[m * 8 * SC_LDH + k4];
+#pragma unroll
+        for (int nb = 0; nb < 2 * NCH; ++nb) b[nb] = wb[k4 * LDW + nb * 8];
+#pragma unroll
+        for (int m = 0; m < 4; ++m)
+#pragma unroll
+          for (int nb = 0; nb < 2 * NCH; ++nb) dmma884(acc[m][nb][0], acc[m][nb][1], a[m], b[nb]);
       }
     }
-    // classes of this thread in increasing index order within a chunk; strict '>' keeps the lowest index on ties
+    // this lane's classes of row (warp*32 + 8m + g): 8nb + 2 q4 + {0,1}, visited in increasing index order
 #pragma unroll
-    for (int q = 0; q < NCH; ++q)
+    for (int m = 0; m < 4; ++m)
 #pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        const int j = cc0 + q * 16 + h * 8 + e;
-        const double l = hs * acc[q][e];
-        if (j < c && (bidx < 0 || l > best || (l == best && j < bidx))) { best = l; bidx = j; }
-      }
+      for (int nb = 0; nb < 2 * NCH; ++nb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int j = cc0 + nb * 8 + 2 * q4 + e;
+          const double l = hs * acc[m][nb][e];
+          if (j < c && (bidx[m] < 0 || l > best[m] || (l == best[m] && j < bidx[m]))) { best[m] = l; bidx[m] = j; }
+        }
   }
-  {  // the two threads of a row: larger logit wins, the lower class index on equality (R12)
-    const double ov = __shfl_xor_sync(0xffffffffu, best, 1);
-    const int oi = __shfl_xor_sync(0xffffffffu, bidx, 1);
-    if (oi >= 0 && (bidx < 0 || ov > best || (ov == best && oi < bidx))) { best = ov; bidx = oi; }
-  }
+  // the four lanes of a row: larger logit wins, the lower class index on equality (R12)
   int ok = 0;
-  if (h == 0 && i0 + r < n) {
-    if (pred) pred[z * n + i0 + r] = bidx;
-    if (y && y[i0 + r] == bidx) ok = 1;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+#pragma unroll
+    for (int d = 1; d <= 2; d <<= 1) {
+      const double ov = __shfl_xor_sync(0xffffffffu, best[m], d);
+      const int oi = __shfl_xor_sync(0xffffffffu, bidx[m], d);
+      if (oi >= 0 && (bidx[m] < 0 || ov > best[m] || (ov == best[m] && oi < bidx[m]))) { best[m] = ov; bidx[m] = oi; }
+    }
+    const long long i = i0 + warp * 32 + m * 8 + g;
+    if (q4 == 0 && i < n) {
+      if (pred) pred[z * n + i] = bidx[m];
+      if (y && y[i] == bidx[m]) ok += 1;
+    }
   }
   __syncthreads();
   ok = __reduce_add_sync(0xffffffffu, ok);
-  if ((t & 31) == 0 && ok) atomicAdd(&s_ok, ok);
+  if (lane == 0 && ok) atomicAdd(&s_ok, ok);
   __syncthreads();
   if (t == 0 && correct && s_ok) atomicAdd(&correct[z], s_ok);
 }
@@ -148,7 +168,7 @@ int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, f
   const double hs = (double)h_scale;
 #define LB_SCORE(NCH)                                                                                                     \
   do {                                                                                                                    \
-    const size_t sm = sizeof(double) * (SC_ROWS * SC_LDH + SC_KT * 16 * NCH);                                         \
+    const size_t sm = sizeof(double) * (SC_ROWS * SC_LDH + SC_KT * (16 * NCH + 8));                                         \
     LB_CUDA_OK(cudaFuncSetAttribute(score_kernel<NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));            \
     score_kernel<NCH><<<grid, SC_THREADS, sm, st>>>(d_H, n, F, hs, d_W, n_classes, d_labels, d_pred, d_correct);         \
   } while (0)

@@ -174,7 +174,7 @@ def _fro(a, b):
 def _fit_case(handle, H, y, c, Creg, s, flags=0):
     K = H.shape[0]
     n, F = H.shape[1], H.shape[2]
-    handle.ensure_workspace((max(n, F) + c + 8) * max(n, F) * 8 * K + n * 4 + 4096 * 8)
+    handle.ensure_workspace(lb.fit_workspace_bytes(n, F, c, K, flags))
     W, info = handle.elm_fit(_dev(H), _dev(y), c, Creg, h_scale=s, flags=flags)
     return W.cpu().numpy().astype(np.float64), info.cpu().numpy()
 
