@@ -210,7 +210,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->perm_off = off; off += (size_t)lb_align_up(n * 4, 256);
   p->off_off = off;  off += (size_t)lb_align_up(((int64_t)n_classes + 1) * 4, 256);
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
-  p->use_tc = ((flags & LBCNN_H_INTEGER) && primal && lb_gram_tc_usable(n, F)) ? 1 : 0;
+  p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
   p->tc_off = off;   if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   p->total = off;
@@ -238,7 +238,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, st);
       if (rc) return rc;
     } else {
     GemmP g{};
@@ -260,6 +260,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   } else {
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
+    if (pl.use_tc) {
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, st);
+      if (rc) return rc;
+    } else {
     GemmP g{};
     g.A = d_H; g.sAr = F; g.sAk = 1; g.bA = n * F;
     g.B = d_H; g.sBr = F; g.sBk = 1; g.bB = n * F;
@@ -267,6 +271,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     g.M = (int)n; g.N = (int)n; g.K = (int)F; g.alpha = 1.0; g.accumulate = 0; g.lower = 1; g.diag = lam;
     rc = launch_gemm<float, float, double, true, true>(h, g, n_cand, st);
     if (rc) return rc;
+    }
     }
     LbPhase ph2(h, LBCNN_PHASE_RHS, st);
     dim3 gr((unsigned)((n * c + 255) / 256), 1, (unsigned)n_cand);

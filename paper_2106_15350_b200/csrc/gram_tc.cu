@@ -37,7 +37,8 @@ constexpr int NTHREADS = 192;
 struct GramTcParams {
   const int32_t* nlimb;   // [n_cand] digits needed (1..3)
   double* A; long long a_stride, ld;
-  int F, n, n_iters;
+  int F, n, n_iters;   // F = dimension of the OUTPUT matrix (features, or samples in the dual branch)
+  int dual;            // 0: A = U^T U (operands MN-major: the feature index is contiguous); 1: A = U U^T (K-major)
   double lam;
 };
 
@@ -109,10 +110,18 @@ __global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
 // K-step offset is a compile-time constant and a descriptor is "base + constant": the issuing warp spends a few
 // uniform-datapath instructions per MMA instead of rebuilding descriptors in vector registers (which cost ~150 clk
 // per MMA, three times the MMA itself).
-template <int L>
-__device__ __forceinline__ void gram_produce(const CUtensorMap* tmap, const GramTcParams& p, uint32_t smem0, uint64_t* bar_full,
-                                             uint64_t* bar_empty, int i0, int j0, int z) {
-  constexpr int NSTAGE = 12 / L, STAGE_BYTES = 2 * L * TILE_BYTES;
+// Dual branch (A = U U^T, F >= n): the contraction runs over the contiguous feature index, so the operands are
+// K-major 128-byte-swizzled tiles [128 or 96 samples][128 features]; a stage holds 128 features (four K = 32 steps).
+constexpr int DTILE_A = TM * 128, DTILE_B = TN * 128;
+template <int L, bool DUAL> struct GramCfg {
+  static constexpr int STAGE_BYTES = DUAL ? L * (DTILE_A + DTILE_B) : 2 * L * TILE_BYTES;
+  static constexpr int NSTAGE = (RING_BYTES / STAGE_BYTES) > MAXSTAGE ? MAXSTAGE : (RING_BYTES / STAGE_BYTES);
+};
+
+template <int L, bool DUAL>
+__device__ __forceinline__ void gram_produce(const CUtensorMap* tmap, const CUtensorMap* tmapB, const GramTcParams& p, uint32_t smem0,
+                                             uint64_t* bar_full, uint64_t* bar_empty, int i0, int j0, int z) {
+  constexpr int NSTAGE = GramCfg<L, DUAL>::NSTAGE, STAGE_BYTES = GramCfg<L, DUAL>::STAGE_BYTES;
   int s = 0, ph = 0;
   for (int it = 0; it < p.n_iters; ++it) {
     tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ph ^ 1);
@@ -122,8 +131,13 @@ __device__ __forceinline__ void gram_produce(const CUtensorMap* tmap, const Gram
       const uint32_t base = smem0 + s * STAGE_BYTES;
 #pragma unroll
       for (int a = 0; a < L; ++a) {
-        tc::tma_load_3d(base + a * TILE_BYTES, tmap, full, i0, it * KS, z * 3 + a);
-        tc::tma_load_3d(base + (L + a) * TILE_BYTES, tmap, full, j0, it * KS, z * 3 + a);
+        if (DUAL) {
+          tc::tma_load_3d(base + a * DTILE_A, tmap, full, it * 128, i0, z * 3 + a);
+          tc::tma_load_3d(base + L * DTILE_A + a * DTILE_B, tmapB, full, it * 128, j0, z * 3 + a);
+        } else {
+          tc::tma_load_3d(base + a * TILE_BYTES, tmap, full, i0, it * KS, z * 3 + a);
+          tc::tma_load_3d(base + (L + a) * TILE_BYTES, tmap, full, j0, it * KS, z * 3 + a);
+        }
       }
     }
     __syncwarp();
@@ -131,26 +145,28 @@ __device__ __forceinline__ void gram_produce(const CUtensorMap* tmap, const Gram
   }
 }
 
-template <int L>
+template <int L, bool DUAL>
 __device__ __forceinline__ void gram_issue(const GramTcParams& p, uint32_t smem0, uint32_t tmem, uint64_t* bar_full,
                                            uint64_t* bar_empty, uint64_t* bar_tmem) {
-  constexpr int NSTAGE = 12 / L, STAGE_BYTES = 2 * L * TILE_BYTES;
-  constexpr uint32_t idesc = tc::idesc_i8(TM, TN, 1, 1, 1, 1);
+  constexpr int NSTAGE = GramCfg<L, DUAL>::NSTAGE, STAGE_BYTES = GramCfg<L, DUAL>::STAGE_BYTES;
+  constexpr uint32_t idesc = DUAL ? tc::idesc_i8(TM, TN, 1, 1, 0, 0) : tc::idesc_i8(TM, TN, 1, 1, 1, 1);
+  constexpr int KSTEPS = DUAL ? 4 : KS / 32;
   // descriptor of the ring's first byte; every operand is this plus a constant number of 16-byte units
-  const uint64_t d0 = tc::smem_desc(smem0, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+  // (K-major swizzled tiles: 8-row groups 1024 B apart, a K = 32 step is 32 bytes inside the 128-byte row)
+  const uint64_t d0 = DUAL ? tc::smem_desc(smem0, 16, 1024, tc::LAYOUT_SW128) : tc::smem_desc(smem0, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
   int s = 0, ph = 0;
   for (int it = 0; it < p.n_iters; ++it) {
     tc::mbar_wait(tc::smem_u32(&bar_full[s]), ph);
     tc::tc_fence_after();
     const uint64_t ds = d0 + (uint64_t)(s * (STAGE_BYTES >> 4));
 #pragma unroll
-    for (int kk = 0; kk < KS / 32; ++kk) {
+    for (int kk = 0; kk < KSTEPS; ++kk) {
 #pragma unroll
       for (int a = 0; a < L; ++a) {
 #pragma unroll
         for (int b = 0; b < L; ++b) {
-          const uint64_t da = ds + (uint64_t)((a * TILE_BYTES + kk * 32 * BOXW) >> 4);
-          const uint64_t db = ds + (uint64_t)(((L + b) * TILE_BYTES + kk * 32 * BOXW) >> 4);
+          const uint64_t da = ds + (uint64_t)((DUAL ? a * DTILE_A + kk * 32 : a * TILE_BYTES + kk * 32 * BOXW) >> 4);
+          const uint64_t db = ds + (uint64_t)((DUAL ? L * DTILE_A + b * DTILE_B + kk * 32 : (L + b) * TILE_BYTES + kk * 32 * BOXW) >> 4);
           // accumulator a + b; its first product of the whole tile is (a, b) with a = max(0, a + b - L + 1) at it = kk = 0
           const bool first = (kk == 0) && (a == ((a + b) > (L - 1) ? (a + b) - (L - 1) : 0));
           if (tc::elect_one()) tc::mma_i8(tmem + (a + b) * TN, da, db, idesc, (first && it == 0) ? 0u : 1u);
@@ -165,7 +181,8 @@ __device__ __forceinline__ void gram_issue(const GramTcParams& p, uint32_t smem0
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const GramTcParams p) {
+__global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmapB,
+                                                               const GramTcParams p) {
   const int ti = blockIdx.y, tj = blockIdx.x, z = blockIdx.z;
   const int i0 = ti * TM, j0 = tj * TN;
   if (j0 > i0 + TM - 1) return;                 // tile entirely above the diagonal
@@ -181,6 +198,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tensormap(&tmap);
+    tc::prefetch_tensormap(&tmapB);
     for (int s = 0; s < MAXSTAGE; ++s) { tc::mbar_init(tc::smem_u32(&bar_full[s]), 1); tc::mbar_init(tc::smem_u32(&bar_empty[s]), 1); }
     tc::mbar_init(tc::smem_u32(&bar_tmem), 1);
     tc::fence_barrier_init();
@@ -193,14 +211,26 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (L == 1) gram_produce<1>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
-    else if (L == 2) gram_produce<2>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
-    else gram_produce<3>(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z);
+    if (p.dual) {
+      if (L == 1) gram_produce<1, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else if (L == 2) gram_produce<2, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else gram_produce<3, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+    } else {
+      if (L == 1) gram_produce<1, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else if (L == 2) gram_produce<2, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else gram_produce<3, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+    }
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (L == 1) gram_issue<1>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-    else if (L == 2) gram_issue<2>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-    else gram_issue<3>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    if (p.dual) {
+      if (L == 1) gram_issue<1, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else if (L == 2) gram_issue<2, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else gram_issue<3, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    } else {
+      if (L == 1) gram_issue<1, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else if (L == 2) gram_issue<2, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else gram_issue<3, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    }
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp % 4) .. +31 =====
     const int q = warp & 3;
@@ -257,7 +287,12 @@ EncodeTiledFn get_encode() {
 // ---- host side --------------------------------------------------------------------------------------
 int64_t lb_gram_tc_fp(int64_t F) { return lb_align_up(F, 16); }
 
-bool lb_gram_tc_usable(int64_t n, int64_t F) { return n >= 1 && n <= 43690 && F >= 1 && F < (1 << 30); }
+// int32 accumulators stay exact while 3 * 128^2 * (contraction length) < 2^31; the contraction runs over the samples
+// (primal) or over the features (dual)
+bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal) {
+  const int64_t k = primal ? n : F;
+  return n >= 1 && F >= 1 && k <= 43690 && n < (1 << 30) && F < (1 << 30);
+}
 
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand) {
   return (size_t)lb_align_up((int64_t)n_cand * 3 * n * lb_gram_tc_fp(F), 256) + (size_t)lb_align_up((int64_t)n_cand * 4, 256);
@@ -265,7 +300,7 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand) {
 
 // A[z] (lower triangle, fp64, leading dimension ld) = U[z]^T U[z] + lam I for integer-valued U, |U| < 2^23
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, cudaStream_t st) {
+                      long long a_stride, long long ld, bool primal, cudaStream_t st) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   const int64_t Fp = lb_gram_tc_fp(F);
@@ -280,7 +315,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
     h->launches += 1;
   }
   LB_CUDA_OK(cudaGetLastError());
-  CUtensorMap tmap;
+  CUtensorMap tmap, tmapB;
   const cuuint64_t gdim[3] = {(cuuint64_t)F, (cuuint64_t)n, (cuuint64_t)n_cand * 3};
   const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)n * Fp};
   const cuuint32_t box[3] = {BOXW, KS, 1};
@@ -288,13 +323,23 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, planes, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
           CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return LBCNN_ERR_CUDA;
+  tmapB = tmap;
+  if (!primal) {      // K-major tiles: 128 features x (128 | 96) samples
+    const cuuint32_t boxA[3] = {128, TM, 1}, boxB[3] = {128, TN, 1};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, planes, gdim, gstr, boxA, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS ||
+        enc(&tmapB, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, planes, gdim, gstr, boxB, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return LBCNN_ERR_CUDA;
+  }
   GramTcParams p{};
-  p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld;
-  p.F = (int)F; p.n = (int)n; p.n_iters = (int)((n + KS - 1) / KS); p.lam = lam;
+  p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
+  const int64_t odim = primal ? F : n;
+  p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
   const size_t smem = (size_t)RING_BYTES + 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid((unsigned)((F + TN - 1) / TN), (unsigned)((F + TM - 1) / TM), (unsigned)n_cand);
-  gram_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmap, p);
+  dim3 grid((unsigned)((odim + TN - 1) / TN), (unsigned)((odim + TM - 1) / TM), (unsigned)n_cand);
+  gram_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmap, tmapB, p);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;

@@ -78,10 +78,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_
                   cudaStream_t st);
 
 // ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
-bool lb_gram_tc_usable(int64_t n, int64_t F);
+bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand);
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, cudaStream_t st);
+                      long long a_stride, long long ld, bool primal, cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
