@@ -196,7 +196,7 @@ def run_cuda(args):
     import torch
     import torch.distributed as dist
     from paper_2106_15350_b200 import binding as lb
-    from paper_2106_15350_b200 import synth
+    from paper_2106_15350_b200 import replicas, synth
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -213,7 +213,7 @@ def run_cuda(args):
         w = synth.scaled(w, n_cand=args.n_cand)
     K = w.n_cand
     trx, try_, tex, tey = synth.make_dataset(w)
-    ker = synth.make_kernels(w, K, first=rank * K)          # every rank searches its own K candidates
+    ker = synth.make_kernels(w, K, first=replicas.first_candidate(rank, K))   # every rank searches its own K candidates
     arch = lb.arch_of(w)
     F, _ = lb.feature_dim(arch)
     dev = torch.device("cuda", local)
@@ -257,10 +257,7 @@ def run_cuda(args):
     phase_ms = h.phase_times()
     h.set_profiling(False)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = replicas.max_over_ranks(ms, dev)
     acc = out["acc"].cpu().numpy()
     info = out["info"].cpu().numpy()
     if (info != 0).any() or not np.isfinite(acc).all():
@@ -274,10 +271,7 @@ def run_cuda(args):
         h.search_candidates_host(arch, *h_in[:4], w.n_classes, w.C, h_in[4], out=hout)   # synchronises inside
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, dev)
     if not np.array_equal(hout["correct"].numpy(), out["correct"].cpu().numpy()):
         raise RuntimeError("host-buffer path and device-buffer path disagree")
     h2d = sum(t.numel() * t.element_size() for t in h_in)
@@ -302,11 +296,11 @@ def run_cuda(args):
         if os.path.exists(prof):      # dram bytes per launch from the committed ncu --set full capture
             with open(prof) as f:
                 roofline["traffic"] = json.load(f).get(dominant)
-    line = dict(metric=METRIC, value=world * K * args.steps / total_s, unit=UNIT, n_gpus=world, steps=args.steps,
+    line = dict(metric=METRIC, value=replicas.job_throughput(world, K, args.steps, total_s), unit=UNIT, n_gpus=world, steps=args.steps,
                 warmup=args.warmup, ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="int8 x int8 -> int32 tensor-core expander and Gram (exact), f64 Cholesky and logits, f32 features/weights",
                 data="synthetic", config=_config(w, K, l2_note), clocks=clocks,
-                e2e=dict(value=world * K * args.steps / e2e_s, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
+                e2e=dict(value=replicas.job_throughput(world, K, args.steps, e2e_s), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
                 gpu_launches=int(launches), roofline=roofline, phases=roofs,
                 accuracy=dict(best=float(acc.max()), worst=float(acc.min()), best_index=int(out["best"][0].item())))
     if not args.no_cpu_baseline:
