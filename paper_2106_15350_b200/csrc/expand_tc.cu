@@ -72,7 +72,9 @@ enum { W1_FULL = 0, W1_EMPTY = 2, W2_FULL = 4, W2_EMPTY = 7, R1_FULL = 10, R1_EM
 // ---- kernel sets -> shared-memory images of the B operands ---------------------------------------------------
 // B1: K-major no-swizzle [16-byte K chunk kc][column n][16 B], K index kk = (c*Pk + yy)*Pk + xx over the patch,
 //     column n = o*nph1 + (py*P1 + px):  w1[o][c][yy-py][xx-px] where that tap exists, else 0.
-// B2: per tap [chunk 0: lo digits | chunk 1: hi digits][column o][16 B = input channel]: w2[o][c][tap], 64 w2[o][c][tap].
+// B2: [chunk 0: lo digits | chunk 1: hi digits][tap slot dy*k + (k-1-dx)][column o][16 B = input channel]:
+//     w2[o][c][dy][dx] and 64 w2[o][c][dy][dx].  Slots of one kernel row run with dx DEcreasing, so the 2 N2 columns that
+//     start at slot (dy, dx) are the taps dx (pool phase px = 0) and dx-1 (px = 1) which read the SAME shifted plane.
 struct PrepParams {
   const int8_t* ker; int n_weights; uint8_t* blob; int blob_bytes, w1_bytes, n_layers;
   int k1, P1, nph1, Cout1, N1, K1, K1p, Pk1, Cin1, w1_off;
@@ -97,10 +99,11 @@ __global__ void __launch_bounds__(256) xtc_prep_kernel(const PrepParams p) {
         if (dy >= 0 && dy < p.k1 && dx >= 0 && dx < p.k1) v = kw[p.w1_off + ((o * p.Cin1 + c) * p.k1 + dy) * p.k1 + dx];
       }
     } else if (p.n_layers == 2) {
-      const int u = t - p.w1_bytes;
-      const int c = u & 15, o = (u >> 4) % p.N2, half = ((u >> 4) / p.N2) & 1, tap = (u >> 4) / (2 * p.N2);
+      const int u = t - p.w1_bytes, kk2 = p.k2 * p.k2;
+      const int c = u & 15, o = (u >> 4) % p.N2, slot = ((u >> 4) / p.N2) % kk2, half = (u >> 4) / (p.N2 * kk2);
+      const int dy = slot / p.k2, dx = p.k2 - 1 - slot % p.k2;      // taps of a row stored with dx DEcreasing
       if (o < p.Cout2 && c < p.Cout1) {
-        v = kw[p.w2_off + (o * p.Cout1 + c) * (p.k2 * p.k2) + tap];
+        v = kw[p.w2_off + (o * p.Cout1 + c) * kk2 + dy * p.k2 + dx];
         if (half) v *= 64;
       }
     }
@@ -322,14 +325,47 @@ template <int P2c, int K2c>
 __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint32_t d0, uint64_t da0, uint64_t db0, uint32_t idesc2) {
   const int P2 = P2c ? P2c : p.P2, K2 = K2c ? K2c : p.k2;
   const int pd = (K2 - 1) / 2;
-  const int plane16 = p.plane_bytes >> 4, n2x2 = p.N2 * 2;
-  // two issuer warps share a tile: warp `half` takes the pool phases with py in its half (all of them when P2 == 1)
+  const int plane16 = p.plane_bytes >> 4, n2 = p.N2;
+  if (P2c == 2) {
+    // 2x2 pooling: the phases px = 0 (tap dx) and px = 1 (tap dx - 1) of one py read the same shifted plane
+    // rx = dx - pd, so one MMA with N = 2 N2 feeds both accumulators (they are adjacent in TMEM and the two taps are
+    // adjacent in B2).  Only rx = -pd (px = 0 alone) and rx = pd + 1 (px = 1 alone) stay N = N2.  Per py and dy the
+    // pair MMAs go first, so the very first MMA (dy = 0) initialises both accumulators at once.
+    const uint32_t idesc_pair = idesc2 + (((uint32_t)n2 >> 3) << 17);     // N field: 2 N2
+    const int py = half;                                                  // issuer warp `half` owns pool row py
+#pragma unroll
+    for (int dy = 0; dy < K2; ++dy) {
+      const int ry = py + dy - pd, qy = floordiv(ry, 2), sy = ry - qy * 2;
+      const uint32_t d = d0 + (py * 2) * n2;
+#pragma unroll
+      for (int rx = 1 - pd; rx <= pd; ++rx) {                             // pairs: px = 0 tap rx + pd, px = 1 tap rx + pd - 1
+        const int qx = floordiv(rx, 2), sx = rx - qx * 2;
+        const uint64_t da = da0 + (uint64_t)(long long)((sy * 2 + sx) * plane16 + qy * p.Wq + qx);
+        const uint64_t db = db0 + (uint64_t)((dy * K2 + (K2 - 1 - (rx + pd))) * n2);
+        if (tc::elect_one()) tc::mma_i8(d, da, db, idesc_pair, (dy != 0 || rx != 1 - pd) ? 1u : 0u);
+      }
+      {                                                                   // px = 0 alone: tap dx = 0, rx = -pd
+        const int rx = -pd, qx = floordiv(rx, 2), sx = rx - qx * 2;
+        const uint64_t da = da0 + (uint64_t)(long long)((sy * 2 + sx) * plane16 + qy * p.Wq + qx);
+        const uint64_t db = db0 + (uint64_t)((dy * K2 + (K2 - 1)) * n2);
+        if (tc::elect_one()) tc::mma_i8(d, da, db, idesc2, 1u);
+      }
+      {                                                                   // px = 1 alone: tap dx = K2 - 1, rx = pd + 1
+        const int rx = pd + 1, qx = floordiv(rx, 2), sx = rx - qx * 2;
+        const uint64_t da = da0 + (uint64_t)(long long)((sy * 2 + sx) * plane16 + qy * p.Wq + qx);
+        const uint64_t db = db0 + (uint64_t)((dy * K2) * n2);
+        if (tc::elect_one()) tc::mma_i8(d + n2, da, db, idesc2, 1u);
+      }
+    }
+    return;
+  }
+  // general pooling: one MMA per (phase, tap); two issuer warps share a tile by pool rows (all of them when P2 == 1)
 #pragma unroll
   for (int py = 0; py < P2; ++py)
 #pragma unroll
     for (int px = 0; px < P2; ++px) {
       if (P2 > 1 && (py * 2 >= P2) != (half != 0)) continue;
-      const uint32_t d = d0 + (py * P2 + px) * p.N2;
+      const uint32_t d = d0 + (py * P2 + px) * n2;
 #pragma unroll
       for (int dy = 0; dy < K2; ++dy) {
         const int ry = py + dy - pd, qy = floordiv(ry, P2), sy = ry - qy * P2;
@@ -338,7 +374,7 @@ __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint
           const int rx = px + dx - pd, qx = floordiv(rx, P2), sx = rx - qx * P2;
           const int a_off = (sy * P2 + sx) * plane16 + qy * p.Wq + qx;
           const uint64_t da = da0 + (uint64_t)(long long)a_off;
-          const uint64_t db = db0 + (uint64_t)((dy * K2 + dx) * n2x2);
+          const uint64_t db = db0 + (uint64_t)((dy * K2 + (K2 - 1 - dx)) * n2);
           if (tc::elect_one()) tc::mma_i8(d, da, db, idesc2, (dy | dx) != 0);
         }
       }
@@ -500,7 +536,7 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
     const int half = (warp == 1) ? 0 : 1;
     if (p.n_layers == 2 && half < n_l2_issuers) {
       const uint32_t idesc2 = tc::idesc_i8(128, p.N2, 1, 1, 0, 0);
-      const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)p.N2 * 16;
+      const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)(p.k2 * p.k2 * p.N2) * 16;   // digit-chunk strides
       const int acc_cols = p.nph2 * p.N2;
       int n2 = 0;
       for (int ci = 0; ci < n_cta_cand; ++ci) {
