@@ -15,12 +15,14 @@
 // (lo digits) and +-64 (hi digits), so the int32 result is the exact convolution.  Pool = max over the phase
 // accumulators; flatten C,H,W; one multiply by feature_scale; H written once.
 //
-// One CTA = a batch of B images x a range of candidates, 18 warps, warp specialised, everything handed over
+// One CTA = a batch of B images x a range of candidates, 19 warps, warp specialised, everything handed over
 // through mbarriers so that the tensor pipe, the TMEM reads and the ALU epilogues of neighbouring candidates overlap:
-//   warp 0      layer-1 MMA issuer (+ bulk-copy of the candidate's prepared B1)    -> accumulator ring R1
-//   warp 1      layer-2 MMA issuer (+ bulk-copy of B2), waits for the planes       -> accumulator ring R2
-//   warps 2-9   E1: R1 -> max-pool -> digits -> phase planes (double buffered) [single layer: -> H, 16 warps]
-//   warps 10-17 E2: R2 -> max-pool -> scale -> H
+//   warp 0       layer-1 MMA issuer (+ bulk-copy of the candidate's prepared B1)   -> accumulator ring R1 (4 slots)
+//   warps 1, 18  layer-2 MMA issuers, one pool row each (warp 1 also bulk-copies B2); they wait for the planes
+//                                                                                  -> accumulator ring R2 (2 slots)
+//   warps 2-9    E1: R1 -> max-pool -> digits -> phase planes (double buffered)  [single layer: -> H, warps 2-17]
+//   warps 10-17  E2: R2 -> max-pool -> scale -> H
+// With 2x2 pooling the two px phases of a pool row read the same shifted plane, so one N = 2 N2 MMA feeds both.
 // The +-1 kernel sets are re-laid-out once per launch by a small kernel into the exact shared-memory images of
 // B1 / B2 (handle-owned scratch), so the hot loop stages them with one cp.async.bulk each.
 // Measured on B200: an MMA with M = 128 reads (128 + N) x 32 operand bytes from shared memory at 128 B/clk, so
@@ -496,6 +498,13 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
     const uint32_t idesc1 = tc::idesc_i8(128, p.N1, 0, 1, 0, 0);     // u8 pixels x s8 weights, K-major both
     const int nks = p.K1p / 32;
     const uint32_t lbo_a = (uint32_t)p.NP1p * 16, lbo_b = (uint32_t)p.N1 * 16;
+    // loop invariants: descriptors are "base + offset in 16-byte units" (this warp's latency per tile is what keeps
+    // the E1 warps fed, so nothing is rebuilt inside the tile loop)
+    const uint64_t da_base = tc::smem_desc(s_base + p.off_a1, lbo_a, 128, tc::LAYOUT_NONE);
+    const uint64_t db_base = tc::smem_desc(s_base + p.off_w1, lbo_b, 128, tc::LAYOUT_NONE);
+    const uint32_t a_ks = 2 * p.NP1p, b_ks = 2 * p.N1, b_slot = p.w1_bytes >> 4, d_base = tmem + p.tm_r1, n1cols = p.N1;
+    const int T1 = p.T1, lg = p.lg_nslot1;
+    const uint32_t bar_full0 = bar_addr(bars, R1_FULL), bar_empty0 = bar_addr(bars, R1_EMPTY);
     int n1 = 0;
     for (int ci = 0; ci < n_cta_cand; ++ci) {
       if (ci == 0 && tc::elect_one()) {
@@ -512,20 +521,17 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         }
       }
       tc::mbar_wait(bar_addr(bars, W1_FULL + (ci & 1)), (ci >> 1) & 1);
-      const uint32_t b_base = s_base + p.off_w1 + (ci & 1) * p.w1_bytes;
-      for (int t1 = 0; t1 < p.T1; ++t1, ++n1) {
+      const uint64_t db_c = db_base + (uint64_t)((ci & 1) * b_slot);
+      for (int t1 = 0; t1 < T1; ++t1, ++n1) {
         const int slot = n1 & (nslot1 - 1);
-        tc::mbar_wait(bar_addr(bars, R1_EMPTY + slot), ((n1 >> p.lg_nslot1) & 1) ^ 1);
+        tc::mbar_wait(bar_empty0 + 8 * slot, ((n1 >> lg) & 1) ^ 1);
         tc::tc_fence_after();
         XT_TRACE(1);
-        const uint32_t d = tmem + p.tm_r1 + slot * p.N1;
-        for (int ks = 0; ks < nks; ++ks) {
-          const uint64_t da = tc::smem_desc(s_base + p.off_a1 + (2 * ks * p.NP1p + t1 * 128) * 16, lbo_a, 128, tc::LAYOUT_NONE);
-          const uint64_t db = tc::smem_desc(b_base + 2 * ks * p.N1 * 16, lbo_b, 128, tc::LAYOUT_NONE);
-          if (tc::elect_one()) tc::mma_i8(d, da, db, idesc1, ks > 0);
-        }
-        if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R1_FULL + slot));
-        __syncwarp();
+        const uint32_t d = d_base + slot * n1cols;
+        const uint64_t da_t = da_base + (uint64_t)(t1 * 128);
+        for (int ks = 0; ks < nks; ++ks)
+          if (tc::elect_one()) tc::mma_i8(d, da_t + (uint64_t)(ks * a_ks), db_c + (uint64_t)(ks * b_ks), idesc1, ks > 0);
+        if (tc::elect_one()) tc::mma_commit(bar_full0 + 8 * slot);
         XT_TRACE(2);
       }
       if (tc::elect_one()) tc::mma_commit(bar_addr(bars, W1_EMPTY + (ci & 1)));
