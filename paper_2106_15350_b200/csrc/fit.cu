@@ -137,34 +137,60 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A,
   double (*S)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(potrf_sh);
   double (*X)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(potrf_sh + NB * (NB + 1));
   double* Az = A + blockIdx.x * a_stride + (long long)j0 * ld + j0;
-  for (int e = threadIdx.x; e < nbj * nbj; e += blockDim.x) {
-    const int i = e / nbj, c = e % nbj;
-    S[i][c] = (c <= i) ? Az[(long long)i * ld + c] : 0.0;
-  }
+  // Right-looking factorisation with the block in REGISTERS: thread (ty, tx) of a 16 x 16 grid owns the 4 x 4
+  // elements (ty + 16 a, tx + 16 b).  Per column j: its owners publish the current column, one barrier, then every
+  // thread scales and applies the rank-1 update to its own elements (no integer division, one barrier per column).
+  __shared__ double colraw[2][NB];
+  const int ty = threadIdx.x >> 4, tx = threadIdx.x & 15;
+  double r[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int i = ty + 16 * a, c = tx + 16 * b;
+      r[a][b] = (i < nbj && c <= i) ? Az[(long long)i * ld + c] : ((i == c) ? 1.0 : 0.0);   // identity padding
+    }
   for (int j = 0; j < nbj; ++j) {
+    double* col = colraw[j & 1];
+    if (tx == (j & 15)) {
+#pragma unroll
+      for (int b = 0; b < 4; ++b)
+        if (b == (j >> 4)) {
+#pragma unroll
+          for (int a = 0; a < 4; ++a) col[ty + 16 * a] = r[a][b];
+        }
+    }
     __syncthreads();
-    double piv = S[j][j];
+    double piv = col[j];
     if (!(piv > 0.0)) {
       if (threadIdx.x == 0 && info[blockIdx.x] == 0) info[blockIdx.x] = j0 + j + 1;
       piv = 1.0;
     }
     const double l = sqrt(piv);
     const double inv = 1.0 / l;
-    __syncthreads();
-    for (int i = j + 1 + threadIdx.x; i < nbj; i += blockDim.x) S[i][j] *= inv;
-    if (threadIdx.x == 0) S[j][j] = l;
-    __syncthreads();
-    const int rem = nbj - j - 1;
-    for (int e = threadIdx.x; e < rem * rem; e += blockDim.x) {
-      const int i = j + 1 + e / rem, c = j + 1 + e % rem;
-      if (c <= i) S[i][c] -= S[i][j] * S[c][j];
+    double li[4], lc[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) li[a] = col[ty + 16 * a] * inv;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) lc[b] = col[tx + 16 * b] * inv;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        const int i = ty + 16 * a, c = tx + 16 * b;
+        if (c == j) { if (i == j) r[a][b] = l; else if (i > j) r[a][b] = li[a]; }
+        else if (c > j && c <= i) r[a][b] = fma(-li[a], lc[b], r[a][b]);
+      }
+  }
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int i = ty + 16 * a, c = tx + 16 * b;
+      S[i][c] = r[a][b];
+      if (i < nbj && c <= i) Az[(long long)i * ld + c] = r[a][b];
     }
-  }
   __syncthreads();
-  for (int e = threadIdx.x; e < nbj * nbj; e += blockDim.x) {
-    const int i = e / nbj, c = e % nbj;
-    if (c <= i) Az[(long long)i * ld + c] = S[i][c];
-  }
   // inverse of the triangular factor, one column per thread by forward substitution (X = L^-1: L X = I)
   if (threadIdx.x < nbj) {
     const int c = threadIdx.x;
