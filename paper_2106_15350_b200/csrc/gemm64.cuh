@@ -12,7 +12,7 @@
 
 namespace g64 {
 
-constexpr int TM = 64, TN = 64, TK = 16, LD = 72, NT = 256;   // LD = 8 (mod 16): conflict-free fragment loads
+constexpr int TM = 64, TN = 64, TK = 16, LD = 73, NT = 256;   // odd pitch: the transposing tile stores and the fragment loads both stay (nearly) conflict-free
 
 struct Smem {
   double a[TK][LD];
