@@ -328,7 +328,7 @@ __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint
   const int P2 = P2c ? P2c : p.P2, K2 = K2c ? K2c : p.k2;
   const int pd = (K2 - 1) / 2;
   const int plane16 = p.plane_bytes >> 4, n2 = p.N2;
-  if (P2c == 2) {
+  if constexpr (P2c == 2) {
     // 2x2 pooling: the phases px = 0 (tap dx) and px = 1 (tap dx - 1) of one py read the same shifted plane
     // rx = dx - pd, so one MMA with N = 2 N2 feeds both accumulators (they are adjacent in TMEM and the two taps are
     // adjacent in B2).  Only rx = -pd (px = 0 alone) and rx = pd + 1 (px = 1 alone) stay N = N2.  Per py and dy the
@@ -359,8 +359,7 @@ __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint
         if (tc::elect_one()) tc::mma_i8(d + n2, da, db, idesc2, 1u);
       }
     }
-    return;
-  }
+  } else {
   // general pooling: one MMA per (phase, tap); two issuer warps share a tile by pool rows (all of them when P2 == 1)
 #pragma unroll
   for (int py = 0; py < P2; ++py)
@@ -381,6 +380,7 @@ __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint
         }
       }
     }
+  }
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------------------------------

@@ -237,7 +237,8 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->off_off = off;  off += (size_t)lb_align_up(((int64_t)n_classes + 1) * 4, 256);
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
   p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
-  p->tc_off = off;   if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand);
+  p->tc_off = off;   p->fuse_rhs = (p->use_tc && primal && lb_gram_tc_fuse_rhs(F, n_classes)) ? 1 : 0;
+  if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand, p->fuse_rhs ? n_classes : 0);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   p->total = off;
 }
@@ -264,7 +265,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, d_labels, c, st);
       if (rc) return rc;
     } else {
     GemmP g{};
@@ -276,18 +277,20 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     if (rc) return rc;
     }
     }
-    // F2: appended rows = (U^T T)^T
+    // F2: appended rows = (U^T T)^T -- already written by the tensor-core Gram of [U | T]; otherwise label-segmented sums
+    if (!pl.fuse_rhs) {
     LbPhase ph2(h, LBCNN_PHASE_RHS, st);
     label_perm_kernel<<<1, 1024, (c + 1) * sizeof(int), st>>>(d_labels, (int)n, c, perm, off);
     h->launches += 1;
     dim3 gr((unsigned)((F + 127) / 128), (unsigned)c, (unsigned)n_cand);
     rhs_primal_kernel<<<gr, 128, 0, st>>>(d_H, n, F, perm, off, A, a_stride, dim);
     h->launches += 1;
+    }
   } else {
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, nullptr, 0, st);
       if (rc) return rc;
     } else {
     GemmP g{};

@@ -38,6 +38,7 @@ struct GramTcParams {
   const int32_t* nlimb;   // [n_cand] digits needed (1..3)
   double* A; long long a_stride, ld;
   int F, n, n_iters;   // F = dimension of the OUTPUT matrix (features, or samples in the dual branch)
+  int Fcols;           // columns written (primal with fused right-hand side: F features of F + c output rows)
   int dual;            // 0: A = U^T U (operands MN-major: the feature index is contiguous); 1: A = U U^T (K-major)
   double lam;
 };
@@ -98,6 +99,15 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
   // one atomic per warp only while it can still raise the count: after the first few warps of a candidate the
   // (L2-cached) read already shows the final value and no further atomics reach that address
   if ((threadIdx.x & 31) == 0 && need > 1 && need > *reinterpret_cast<volatile int32_t*>(&nlimb[z])) atomicMax(&nlimb[z], need);
+}
+
+// one-hot label columns F .. F + c - 1 of digit plane 0 (planes 1, 2 keep the zeros the split kernel wrote there)
+__global__ void onehot_kernel(const int32_t* __restrict__ y, long long n, int F, int Fp, int c, int8_t* __restrict__ planes) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n * c) return;
+  const long long row = t / c;
+  const int cls = (int)(t - row * c);
+  planes[((long long)blockIdx.y * 3 * n + row) * Fp + F + cls] = (y[row] == cls) ? 1 : 0;
 }
 
 __global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
@@ -249,7 +259,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
           const int j = j0 + c0 + e;
-          if (j < p.F) {
+          if (j < p.Fcols) {
             long long g = 0;
 #pragma unroll
             for (int s = 4; s >= 0; --s)
@@ -285,7 +295,12 @@ EncodeTiledFn get_encode() {
 }  // namespace
 
 // ---- host side --------------------------------------------------------------------------------------
-int64_t lb_gram_tc_fp(int64_t F) { return lb_align_up(F, 16); }
+// plane pitch; `c_aug` one-hot label columns are appended to the features (primal branch: the Gram of [U | T] holds
+// U^T T, the right-hand side, in its last c rows -- PAPER.md:67, 70 -- for the price of c extra columns)
+int64_t lb_gram_tc_fp(int64_t F, int c_aug) { return lb_align_up(F + c_aug, 16); }
+// worth it when the c extra rows fit into the last 128-row tile the features leave partly empty (otherwise a whole extra
+// row of tiles costs more than the separate label-segmented sum)
+bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes) { return (F + n_classes + 127) / 128 == (F + 127) / 128; }
 
 // int32 accumulators stay exact while 3 * 128^2 * (contraction length) < 2^31; the contraction runs over the samples
 // (primal) or over the features (dual)
@@ -294,16 +309,19 @@ bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal) {
   return n >= 1 && F >= 1 && k <= 43690 && n < (1 << 30) && F < (1 << 30);
 }
 
-size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand) {
-  return (size_t)lb_align_up((int64_t)n_cand * 3 * n * lb_gram_tc_fp(F), 256) + (size_t)lb_align_up((int64_t)n_cand * 4, 256);
+size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {
+  return (size_t)lb_align_up((int64_t)n_cand * 3 * n * lb_gram_tc_fp(F, c_aug), 256) + (size_t)lb_align_up((int64_t)n_cand * 4, 256);
 }
 
-// A[z] (lower triangle, fp64, leading dimension ld) = U[z]^T U[z] + lam I for integer-valued U, |U| < 2^23
+// A[z] (lower triangle, fp64, leading dimension ld) = U[z]^T U[z] + lam I for integer-valued U, |U| < 2^23 (primal), or
+// U U^T + lam I (dual).  Primal with d_labels != NULL: rows F .. F + n_classes - 1 of A[z] additionally receive
+// (U^T T)^T, T the one-hot coding of the labels (the appended right-hand-side rows of the Cholesky layout).
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, bool primal, cudaStream_t st) {
+                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, cudaStream_t st) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
-  const int64_t Fp = lb_gram_tc_fp(F);
+  const int c_aug = (primal && d_labels && lb_gram_tc_fuse_rhs(F, n_classes)) ? n_classes : 0;
+  const int64_t Fp = lb_gram_tc_fp(F, c_aug);
   int8_t* planes = reinterpret_cast<int8_t*>(ws);
   int32_t* nlimb = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + lb_align_up((int64_t)n_cand * 3 * n * Fp, 256));
   fill_i32_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(nlimb, n_cand, 1);
@@ -313,10 +331,15 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
     split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb);
     h->launches += 1;
+    if (c_aug) {
+      dim3 g1((unsigned)((n * c_aug + 255) / 256), (unsigned)n_cand);
+      onehot_kernel<<<g1, 256, 0, st>>>(d_labels, n, (int)F, (int)Fp, c_aug, planes);
+      h->launches += 1;
+    }
   }
   LB_CUDA_OK(cudaGetLastError());
   CUtensorMap tmap, tmapB;
-  const cuuint64_t gdim[3] = {(cuuint64_t)F, (cuuint64_t)n, (cuuint64_t)n_cand * 3};
+  const cuuint64_t gdim[3] = {(cuuint64_t)(F + c_aug), (cuuint64_t)n, (cuuint64_t)n_cand * 3};
   const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)n * Fp};
   const cuuint32_t box[3] = {BOXW, KS, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -334,11 +357,12 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   }
   GramTcParams p{};
   p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
-  const int64_t odim = primal ? F : n;
+  const int64_t odim = primal ? F + c_aug : n, ocols = primal ? F : n;
+  p.Fcols = (int)ocols;
   p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
   const size_t smem = (size_t)RING_BYTES + 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid((unsigned)((odim + TN - 1) / TN), (unsigned)((odim + TM - 1) / TM), (unsigned)n_cand);
+  dim3 grid((unsigned)((ocols + TN - 1) / TN), (unsigned)((odim + TM - 1) / TM), (unsigned)n_cand);
   gram_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmap, tmapB, p);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());

@@ -71,6 +71,7 @@ struct FitPlan {
   size_t a_bytes;        // per candidate: rows * dim doubles
   size_t perm_off, off_off, a_off, tc_off, linv_off, total; // offsets inside the fit workspace
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
+  int fuse_rhs;          // ... which then also produces the right-hand side (one-hot label columns)
 };
 void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p);
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_H, int64_t n, int64_t F, float h_scale,
@@ -79,9 +80,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_
 
 // ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
 bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
-size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand);
+size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug);
+bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-hot columns of the Gram's digit plane 0
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, bool primal, cudaStream_t st);
+                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
