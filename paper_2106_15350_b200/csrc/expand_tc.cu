@@ -131,24 +131,34 @@ __device__ __forceinline__ uint32_t bar_addr(const uint64_t* bars, int i) { retu
 
 // ---- E1, two layers: R1 -> max-pool -> (relu) -> digits -> phase planes of layer 2 --------------------------------
 // tab1[m] = byte offset of pooled position m inside one plane buffer (phase plane + halo-sharing position), -1 = none
-template <int NPH>
+// four values -> their low bytes in one word
+__device__ __forceinline__ uint32_t pack4(uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  return __byte_perm(__byte_perm(a, b, 0x0040), __byte_perm(c, d, 0x0040), 0x5410);
+}
+
+template <int NPH, bool RELU>
 __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, const uint64_t* bars, uint32_t tmem,
                                              int set, int quad, int lane, int n_cta_cand XT_TRACE_ARGS) {
   constexpr int CPG = 16 / NPH;          // channels per 16-column group
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
-  const int mask = (1 << p.lg_nset1) - 1, smask = (1 << p.lg_nslot1) - 1;
-  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
+  // loop invariants in registers (the asm statements' memory clobbers would otherwise re-read the parameters)
+  const int lg_slot = p.lg_nslot1, mask = (1 << p.lg_nset1) - 1, smask = (1 << lg_slot) - 1;
+  const int T1 = p.T1, N1 = p.N1, npb2 = (p.NPB == 2), nwords = (p.Cp1 + 3) >> 2;
+  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1) + quad * 32 + lane;
   const uint32_t taddr0 = tmem + lane_base + p.tm_r1;
+  uint8_t* planes0 = smem + p.off_pl;
+  const int plbuf_bytes = p.plbuf_bytes, hi_off = p.NPOS2 * 16;
+  const uint32_t bar_full0 = bar_addr(bars, R1_FULL), bar_empty0 = bar_addr(bars, R1_EMPTY);
   for (int ci = 0; ci < n_cta_cand; ++ci) {
-    const int buf = (p.NPB == 2) ? (ci & 1) : 0;
-    const int use = (p.NPB == 2) ? (ci >> 1) : ci;
+    const int buf = npb2 ? (ci & 1) : 0;
+    const int use = npb2 ? (ci >> 1) : ci;
     bool waited = false;
-    for (int t1 = 0; t1 < p.T1; ++t1) {
-      const int n1 = ci * p.T1 + t1;
+    for (int t1 = 0; t1 < T1; ++t1) {
+      const int n1 = ci * T1 + t1;
       if ((n1 & mask) != set) continue;
       const int slot = n1 & smask;
-      const uint32_t taddr = taddr0 + slot * p.N1;
-      tc::mbar_wait(bar_addr(bars, R1_FULL + slot), (n1 >> p.lg_nslot1) & 1);
+      const uint32_t taddr = taddr0 + slot * N1;
+      tc::mbar_wait(bar_full0 + 8 * slot, (n1 >> lg_slot) & 1);
       tc::tc_fence_after();
       XT_TRACE(6);
       int mx[16];
@@ -156,35 +166,39 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
       for (int e = 0; e < 16; ++e) mx[e] = 0;
 #pragma unroll
       for (int gb = 0; gb < NPH; gb += 4) {
-        if (gb * 16 < p.N1) {
+        if (gb * 16 < N1) {
           uint32_t r[4][16];
 #pragma unroll
           for (int q = 0; q < 4; ++q)
-            if (gb + q < NPH && (gb + q) * 16 < p.N1) tc::tmem_ld16(taddr + (gb + q) * 16, r[q]);
+            if (gb + q < NPH && (gb + q) * 16 < N1) tc::tmem_ld16(taddr + (gb + q) * 16, r[q]);
           tc::tmem_ld_wait();
 #pragma unroll
           for (int q = 0; q < 4; ++q)
-            if (gb + q < NPH && (gb + q) * 16 < p.N1) pool_group<NPH>(r[q], &mx[(gb + q) * CPG]);
+            if (gb + q < NPH && (gb + q) * 16 < N1) pool_group<NPH>(r[q], &mx[(gb + q) * CPG]);
         }
       }
       tc::tc_fence_before();
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + slot));     // accumulator slot free again
+      if (lane == 0) tc::mbar_arrive(bar_empty0 + 8 * slot);               // accumulator slot free again
       XT_TRACE(7);
       if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; XT_TRACE(8); }
-      const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
+      const int32_t off = tab1[t1 * 128];
       if (off >= 0) {
+        // v = 64 (v >> 6) + (v & 63): both digits fit an int8; four channels per word, words past the real channels stay 0
         uint32_t lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};
 #pragma unroll
-        for (int e = 0; e < 16; ++e) {
-          int v = mx[e];
-          if (p.act1 == LBCNN_ACT_RELU) v = max(v, 0);
-          lo[e >> 2] |= (uint32_t)(v & 63) << (8 * (e & 3));              // v = 64 (v >> 6) + (v & 63), both int8
-          hi[e >> 2] |= (uint32_t)((v >> 6) & 255) << (8 * (e & 3));
+        for (int w = 0; w < 4; ++w) {
+          if (w < nwords) {
+            int v[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) v[e] = RELU ? max(mx[4 * w + e], 0) : mx[4 * w + e];
+            lo[w] = pack4((uint32_t)v[0], (uint32_t)v[1], (uint32_t)v[2], (uint32_t)v[3]) & 0x3f3f3f3fu;
+            hi[w] = pack4((uint32_t)(v[0] >> 6), (uint32_t)(v[1] >> 6), (uint32_t)(v[2] >> 6), (uint32_t)(v[3] >> 6));
+          }
         }
-        uint8_t* dst = smem + p.off_pl + buf * p.plbuf_bytes + off;
+        uint8_t* dst = planes0 + buf * plbuf_bytes + off;
         *reinterpret_cast<uint4*>(dst) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-        *reinterpret_cast<uint4*>(dst + p.NPOS2 * 16) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<uint4*>(dst + hi_off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
       }
       XT_TRACE(9);
     }
@@ -593,9 +607,13 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   } else if (warp < 2 + n_e1_warps) {
     const int set = (warp - 2) >> 2, quad = warp & 3;
     if (p.n_layers == 2) {
-      if (p.nph1 == 1) e1_two_layer<1>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else if (p.nph1 == 4) e1_two_layer<4>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else e1_two_layer<16>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      const bool relu1 = p.act1 == LBCNN_ACT_RELU;
+      if (p.nph1 == 4 && !relu1) e1_two_layer<4, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else if (p.nph1 == 4) e1_two_layer<4, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else if (p.nph1 == 1 && !relu1) e1_two_layer<1, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else if (p.nph1 == 1) e1_two_layer<1, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else if (!relu1) e1_two_layer<16, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      else e1_two_layer<16, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
     } else {
       if (p.nph1 == 1) e1_single<1>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
       else if (p.nph1 == 4) e1_single<4>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
