@@ -212,25 +212,31 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
 
 // ---- E1, single layer: R1 -> max-pool -> (relu) -> scale -> H -------------------------------------------------------
 // tab1[m] = b*F + i*Wo + j of pooled position m (flatten C,H,W adds o*Ho*Wo), -1 = none
-template <int NPH>
+template <int NPH, bool RELU, bool UNIT>
 __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem,
                                           int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0 XT_TRACE_ARGS) {
   constexpr int CPG = 16 / NPH;
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
-  const int mask = (1 << p.lg_nset1) - 1, smask = (1 << p.lg_nslot1) - 1;
-  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1);
+  // loop invariants in registers (the asm statements' memory clobbers would otherwise re-read the parameters)
+  const int lg_slot = p.lg_nslot1, mask = (1 << p.lg_nset1) - 1, smask = (1 << lg_slot) - 1;
+  const int T1 = p.T1, N1 = p.N1, G1 = N1 >> 4, cout1 = p.Cout1;
+  const uint32_t hw = (uint32_t)(p.Ho1 * p.Wo1);
+  const float scale = p.scale;
+  const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1) + quad * 32 + lane;
   const uint32_t taddr0 = tmem + lane_base + p.tm_r1;
-  const int G1 = p.N1 >> 4, hw = p.Ho1 * p.Wo1;
-  for (int ci = 0; ci < n_cta_cand; ++ci) {
-    float* Hc = p.Hout + ((long long)(c_begin + ci) * p.n_img + img0) * p.F;
-    for (int t1 = 0; t1 < p.T1; ++t1) {
-      const int n1 = ci * p.T1 + t1;
+  const uint32_t bar_full0 = bar_addr(bars, R1_FULL), bar_empty0 = bar_addr(bars, R1_EMPTY);
+  const long long cand_stride = p.n_img * p.F;
+  float* Hb = p.Hout + ((long long)c_begin * p.n_img + img0) * p.F;
+  for (int ci = 0; ci < n_cta_cand; ++ci, Hb += cand_stride) {
+    for (int t1 = 0; t1 < T1; ++t1) {
+      const int n1 = ci * T1 + t1;
       if ((n1 & mask) != set) continue;
       const int slot = n1 & smask;
-      const uint32_t taddr = taddr0 + slot * p.N1;
-      tc::mbar_wait(bar_addr(bars, R1_FULL + slot), (n1 >> p.lg_nslot1) & 1);
+      const uint32_t taddr = taddr0 + slot * N1;
+      tc::mbar_wait(bar_full0 + 8 * slot, (n1 >> lg_slot) & 1);
       tc::tc_fence_after();
-      const int32_t off = tab1[t1 * 128 + quad * 32 + lane];
+      const int32_t off = tab1[t1 * 128];
+      uint32_t idx = (uint32_t)(off >= 0 ? off : 0);
       for (int gb = 0; gb < G1; gb += 4) {
         uint32_t r[4][16];
 #pragma unroll
@@ -242,13 +248,14 @@ __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* sme
           if (gb + q < G1) {
             int mx[CPG];
             pool_group<NPH>(r[q], mx);
+            if (off >= 0) {
 #pragma unroll
-            for (int k = 0; k < CPG; ++k) {
-              const int o = (gb + q) * CPG + k;
-              if (off >= 0 && o < p.Cout1) {
-                int v = mx[k];
-                if (p.act1 == LBCNN_ACT_RELU) v = max(v, 0);
-                Hc[off + o * hw] = p.scale * (float)v;
+              for (int k = 0; k < CPG; ++k) {
+                if ((gb + q) * CPG + k < cout1) {
+                  const int v = RELU ? max(mx[k], 0) : mx[k];
+                  Hb[idx] = UNIT ? (float)v : scale * (float)v;            // flatten C,H,W: channel stride Ho*Wo
+                  idx += hw;
+                }
               }
             }
           }
@@ -256,7 +263,7 @@ __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* sme
       }
       tc::tc_fence_before();
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive(bar_addr(bars, R1_EMPTY + slot));
+      if (lane == 0) tc::mbar_arrive(bar_empty0 + 8 * slot);
     }
   }
 }
@@ -615,9 +622,19 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
       else if (!relu1) e1_two_layer<16, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
       else e1_two_layer<16, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
     } else {
-      if (p.nph1 == 1) e1_single<1>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
-      else if (p.nph1 == 4) e1_single<4>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
-      else e1_single<16>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      // the search driver's case (no relu, scale 1) is specialised; everything else takes the general instantiation
+      const bool plain = p.act1 != LBCNN_ACT_RELU && p.scale == 1.0f;
+#define XT_E1S(NPH)                                                                                                      \
+  do {                                                                                                                   \
+    if (plain) e1_single<NPH, false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS); \
+    else if (p.act1 == LBCNN_ACT_RELU)                                                                                   \
+      e1_single<NPH, true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);         \
+    else e1_single<NPH, false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);     \
+  } while (0)
+      if (p.nph1 == 1) XT_E1S(1);
+      else if (p.nph1 == 4) XT_E1S(4);
+      else XT_E1S(16);
+#undef XT_E1S
     }
   } else if (p.n_layers == 2) {
     const int set = (warp - 2 - n_e1_warps) >> 2, quad = warp & 3;
