@@ -150,37 +150,39 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A,
       const int i = ty + 16 * a, c = tx + 16 * b;
       r[a][b] = (i < nbj && c <= i) ? Az[(long long)i * ld + c] : ((i == c) ? 1.0 : 0.0);   // identity padding
     }
-  for (int j = 0; j < nbj; ++j) {
-    double* col = colraw[j & 1];
-    if (tx == (j & 15)) {
 #pragma unroll
-      for (int b = 0; b < 4; ++b)
-        if (b == (j >> 4)) {
+  for (int jb = 0; jb < 4; ++jb) {                 // block column of the 16 x 16 thread grid: static register indices
+    for (int jj = 0; jj < 16; ++jj) {
+      const int j = jb * 16 + jj;
+      if (j >= nbj) break;
+      double* col = colraw[j & 1];
+      if (tx == jj) {
 #pragma unroll
-          for (int a = 0; a < 4; ++a) col[ty + 16 * a] = r[a][b];
-        }
-    }
-    __syncthreads();
-    double piv = col[j];
-    if (!(piv > 0.0)) {
-      if (threadIdx.x == 0 && info[blockIdx.x] == 0) info[blockIdx.x] = j0 + j + 1;
-      piv = 1.0;
-    }
-    const double l = sqrt(piv);
-    const double inv = 1.0 / l;
-    double li[4], lc[4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a) li[a] = col[ty + 16 * a] * inv;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) lc[b] = col[tx + 16 * b] * inv;
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const int i = ty + 16 * a, c = tx + 16 * b;
-        if (c == j) { if (i == j) r[a][b] = l; else if (i > j) r[a][b] = li[a]; }
-        else if (c > j && c <= i) r[a][b] = fma(-li[a], lc[b], r[a][b]);
+        for (int a = 0; a < 4; ++a) col[ty + 16 * a] = r[a][jb];
       }
+      __syncthreads();
+      double piv = col[j];
+      if (!(piv > 0.0)) {
+        if (threadIdx.x == 0 && info[blockIdx.x] == 0) info[blockIdx.x] = j0 + j + 1;
+        piv = 1.0;
+      }
+      const double inv = rsqrt(piv);               // 1 / l
+      const double l = piv * inv;
+      double li[4], lc[4];
+#pragma unroll
+      for (int a = 0; a < 4; ++a) li[a] = col[ty + 16 * a] * inv;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) lc[b] = col[tx + 16 * b] * inv;
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        const int i = ty + 16 * a;
+        if (tx == jj) r[a][jb] = (i == j) ? l : ((i > j) ? li[a] : r[a][jb]);
+        else if (tx > jj && tx + 16 * jb <= i) r[a][jb] = fma(-li[a], lc[jb], r[a][jb]);
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+          if (b > jb && tx + 16 * b <= i) r[a][b] = fma(-li[a], lc[b], r[a][b]);
+      }
+    }
   }
 #pragma unroll
   for (int a = 0; a < 4; ++a)
@@ -191,15 +193,24 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(double* __restrict__ A,
       if (i < nbj && c <= i) Az[(long long)i * ld + c] = r[a][b];
     }
   __syncthreads();
-  // inverse of the triangular factor, one column per thread by forward substitution (X = L^-1: L X = I)
-  if (threadIdx.x < nbj) {
-    const int c = threadIdx.x;
-    for (int i = 0; i < c; ++i) X[i][c] = 0.0;
-    X[c][c] = 1.0 / S[c][c];
-    for (int i = c + 1; i < nbj; ++i) {
+  // inverse of the triangular factor by forward substitution (L X = I): four adjacent lanes share a column and split
+  // the inner sum, so a warp advances eight columns with two shuffles per row
+  {
+    const int c = threadIdx.x >> 2, part = threadIdx.x & 3;
+    const int c_min = (threadIdx.x >> 5) * 8;        // first column of this warp
+    if (part == 0) {
+      for (int i = 0; i < c; ++i) X[i][c] = 0.0;
+      X[c][c] = 1.0 / S[c][c];
+    }
+    __syncwarp();
+    for (int i = c_min + 1; i < nbj; ++i) {
       double acc = 0.0;
-      for (int k = c; k < i; ++k) acc = fma(S[i][k], X[k][c], acc);
-      X[i][c] = -acc / S[i][i];
+      if (i > c)
+        for (int k = c + part; k < i; k += 4) acc = fma(S[i][k], X[k][c], acc);
+      acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+      acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+      if (part == 0 && i > c) X[i][c] = -acc / S[i][i];
+      __syncwarp();
     }
   }
   __syncthreads();
