@@ -36,6 +36,8 @@ constexpr int NTHREADS = 192;
 
 struct GramTcParams {
   const int32_t* nlimb;   // [n_cand] digits needed (1..3)
+  const int32_t* nl32;    // [n_cand][G32] digits needed per group of 32 features (primal: per-tile digit counts)
+  int G32;
   double* A; long long a_stride, ld;
   int F, n, n_iters;   // F = dimension of the OUTPUT matrix (features, or samples in the dual branch)
   int Fcols;           // columns written (primal with fused right-hand side: F features of F + c output rows)
@@ -54,7 +56,8 @@ __device__ __forceinline__ uint32_t pack_bytes(uint32_t a, uint32_t b, uint32_t 
   return __byte_perm(__byte_perm(a, b, s2), __byte_perm(c, d, s2), 0x5410);
 }
 __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
-                                                    int8_t* __restrict__ planes, int32_t* __restrict__ nlimb) {
+                                                    int8_t* __restrict__ planes, int32_t* __restrict__ nlimb,
+                                                    int32_t* __restrict__ nl32, int G32) {
   const int z = blockIdx.y;
   const long long oct_per_row = Fp / 8;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -95,6 +98,12 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
     *reinterpret_cast<uint2*>(dst + 2 * plane) = w2;
   }
   int need = or3 ? 3 : (or2 ? 2 : 1);
+  // digits needed by this thread's group of 32 features (very few values need the third digit, so most 128 x 96 tiles
+  // of the Gram run with 2 x 2 instead of 3 x 3 digit products); same cached-read trick as below
+  if (need > 1 && t < n * oct_per_row) {
+    int32_t* g = nl32 + (long long)z * G32 + (int)((t % oct_per_row) >> 2);
+    if (need > __ldg(g)) atomicMax(g, need);     // a stale (smaller) cached value only costs one redundant atomic
+  }
   need = __reduce_max_sync(0xffffffffu, need);
   // one atomic per warp only while it can still raise the count: after the first few warps of a candidate the
   // (L2-cached) read already shows the final value and no further atomics reach that address
@@ -191,6 +200,67 @@ __device__ __forceinline__ void gram_issue(const GramTcParams& p, uint32_t smem0
   __syncwarp();
 }
 
+// Primal branch with per-tile digit counts: the row tile needs Li digits, the column tile Lj (from the 32-feature
+// group counts), so only Li x Lj of the nine digit products are issued and only Li + Lj planes are loaded.  Stage =
+// Li + Lj tile slots of 8 KB (A planes, then B planes); as many stages as fit the 192 KB ring (at most 12).
+__device__ __forceinline__ void gram_produce_p(const CUtensorMap* tmap, const GramTcParams& p, uint32_t smem0, uint64_t* bar_full,
+                                               uint64_t* bar_empty, int i0, int j0, int z, int Li, int Lj) {
+  int s = 0, ph = 0;
+  const uint32_t tx_bytes = (uint32_t)(Li + Lj) * TILE_BYTES;
+  const int PSTAGE_BYTES = (Li + Lj) * TILE_BYTES, PNSTAGE = min(MAXSTAGE, 24 / (Li + Lj));
+  for (int it = 0; it < p.n_iters; ++it) {
+    tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ph ^ 1);
+    if (tc::elect_one()) {
+      const uint32_t full = tc::smem_u32(&bar_full[s]);
+      tc::mbar_arrive_expect_tx(full, tx_bytes);
+      const uint32_t base = smem0 + s * PSTAGE_BYTES;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        if (a < Li) tc::tma_load_3d(base + a * TILE_BYTES, tmap, full, i0, it * KS, z * 3 + a);
+        if (a < Lj) tc::tma_load_3d(base + (Li + a) * TILE_BYTES, tmap, full, j0, it * KS, z * 3 + a);
+      }
+    }
+    __syncwarp();
+    if (++s == PNSTAGE) { s = 0; ph ^= 1; }
+  }
+}
+
+__device__ __forceinline__ void gram_issue_p(const GramTcParams& p, uint32_t smem0, uint32_t tmem, uint64_t* bar_full,
+                                             uint64_t* bar_empty, uint64_t* bar_tmem, int Li, int Lj) {
+  constexpr uint32_t idesc = tc::idesc_i8(TM, TN, 1, 1, 1, 1);
+  const uint64_t d0 = tc::smem_desc(smem0, TILE_BYTES, 8 * BOXW, tc::LAYOUT_SW128);
+  const int PSTAGE_BYTES = (Li + Lj) * TILE_BYTES, PNSTAGE = min(MAXSTAGE, 24 / (Li + Lj));
+  const uint32_t b_off = (uint32_t)(Li * TILE_BYTES) >> 4;
+  int s = 0, ph = 0;
+  for (int it = 0; it < p.n_iters; ++it) {
+    tc::mbar_wait(tc::smem_u32(&bar_full[s]), ph);
+    tc::tc_fence_after();
+    const uint64_t ds = d0 + (uint64_t)(s * (PSTAGE_BYTES >> 4));
+#pragma unroll
+    for (int kk = 0; kk < KS / 32; ++kk) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+          if (a < Li && b < Lj) {
+            const uint64_t da = ds + (uint64_t)((a * TILE_BYTES + kk * 32 * BOXW) >> 4);
+            const uint64_t db = ds + (uint64_t)(b_off + ((b * TILE_BYTES + kk * 32 * BOXW) >> 4));
+            // accumulator a + b: its first product of the tile is the pair with the smallest a, a = max(0, a + b - Lj + 1)
+            const int a_first = (a + b) > (Lj - 1) ? (a + b) - (Lj - 1) : 0;
+            const bool first = (it == 0) && (kk == 0) && (a == a_first);
+            if (tc::elect_one()) tc::mma_i8(tmem + (a + b) * TN, da, db, idesc, first ? 0u : 1u);
+          }
+        }
+      }
+    }
+    if (tc::elect_one()) tc::mma_commit(tc::smem_u32(&bar_empty[s]));
+    __syncwarp();
+    if (++s == PNSTAGE) { s = 0; ph ^= 1; }
+  }
+  if (tc::elect_one()) tc::mma_commit(tc::smem_u32(bar_tmem));
+  __syncwarp();
+}
+
 __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmapB,
                                                                const GramTcParams p) {
   const int ti = blockIdx.y, tj = blockIdx.x, z = blockIdx.z;
@@ -203,7 +273,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
   __shared__ uint32_t tmem_base_s;
 
   const int warp = tc::uniform_warp_id(), lane = threadIdx.x & 31;
-  const int L = p.nlimb[z];
+  int L = p.nlimb[z], Li = L, Lj = L;           // dual: one digit count per candidate
+  if (!p.dual) {                                 // primal: per tile, from the 32-feature group counts
+    Li = 1; Lj = 1;
+    const int32_t* g = p.nl32 + (long long)z * p.G32;
+#pragma unroll
+    for (int q = 0; q < TM / 32; ++q) if (i0 / 32 + q < p.G32) Li = max(Li, g[i0 / 32 + q]);
+#pragma unroll
+    for (int q = 0; q < TN / 32; ++q) if (j0 / 32 + q < p.G32) Lj = max(Lj, g[j0 / 32 + q]);
+  }
   const uint32_t smem0 = tc::smem_u32(smem);
 
   if (warp == 0 && lane == 0) {
@@ -221,26 +299,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (p.dual) {
-      if (L == 1) gram_produce<1, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-      else if (L == 2) gram_produce<2, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-      else gram_produce<3, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-    } else {
-      if (L == 1) gram_produce<1, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-      else if (L == 2) gram_produce<2, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-      else gram_produce<3, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
-    }
+    if (!p.dual) gram_produce_p(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z, Li, Lj);
+    else if (L == 1) gram_produce<1, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+    else if (L == 2) gram_produce<2, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+    else gram_produce<3, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (p.dual) {
-      if (L == 1) gram_issue<1, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-      else if (L == 2) gram_issue<2, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-      else gram_issue<3, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-    } else {
-      if (L == 1) gram_issue<1, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-      else if (L == 2) gram_issue<2, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-      else gram_issue<3, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
-    }
+    if (!p.dual) gram_issue_p(p, smem0, tmem, bar_full, bar_empty, &bar_tmem, Li, Lj);
+    else if (L == 1) gram_issue<1, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    else if (L == 2) gram_issue<2, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    else gram_issue<3, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp % 4) .. +31 =====
     const int q = warp & 3;
@@ -248,7 +316,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
     tc::tc_fence_after();
     const int i = i0 + q * 32 + lane;
     double* Arow = p.A + (long long)z * p.a_stride + (long long)i * p.ld;
-    const int nacc = 2 * L - 1;
+    const int nacc = Li + Lj - 1;
     for (int c0 = 0; c0 < TN; c0 += 16) {
       uint32_t r[5][16];
 #pragma unroll
@@ -310,7 +378,8 @@ bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal) {
 }
 
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {
-  return (size_t)lb_align_up((int64_t)n_cand * 3 * n * lb_gram_tc_fp(F, c_aug), 256) + (size_t)lb_align_up((int64_t)n_cand * 4, 256);
+  const int64_t Fp = lb_gram_tc_fp(F, c_aug);
+  return (size_t)lb_align_up((int64_t)n_cand * 3 * n * Fp, 256) + (size_t)lb_align_up((int64_t)n_cand * (1 + (Fp + 31) / 32) * 4, 256);
 }
 
 // A[z] (lower triangle, fp64, leading dimension ld) = U[z]^T U[z] + lam I for integer-valued U, |U| < 2^23 (primal), or
@@ -324,12 +393,15 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   const int64_t Fp = lb_gram_tc_fp(F, c_aug);
   int8_t* planes = reinterpret_cast<int8_t*>(ws);
   int32_t* nlimb = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + lb_align_up((int64_t)n_cand * 3 * n * Fp, 256));
-  fill_i32_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(nlimb, n_cand, 1);
+  const int G32 = (int)((Fp + 31) / 32);
+  int32_t* nl32 = nlimb + n_cand;                  // [n_cand][G32] right behind the per-candidate counts
+  const int n_counts = n_cand * (1 + G32);
+  fill_i32_kernel<<<(n_counts + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1);
   h->launches += 1;
   {
     const long long work = n * (Fp / 8);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
-    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb);
+    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32);
     h->launches += 1;
     if (c_aug) {
       dim3 g1((unsigned)((n * c_aug + 255) / 256), (unsigned)n_cand);
@@ -356,7 +428,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
       return LBCNN_ERR_CUDA;
   }
   GramTcParams p{};
-  p.nlimb = nlimb; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
+  p.nlimb = nlimb; p.nl32 = nl32; p.G32 = G32; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
   const int64_t odim = primal ? F + c_aug : n, ocols = primal ? F : n;
   p.Fcols = (int)ocols;
   p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
