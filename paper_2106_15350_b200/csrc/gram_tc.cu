@@ -299,13 +299,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
 
   if (warp == 0) {
     // ===== TMA producer =====
-    if (!p.dual) gram_produce_p(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z, Li, Lj);
+    if (!p.dual && Li != Lj) gram_produce_p(&tmap, p, smem0, bar_full, bar_empty, i0, j0, z, Li, Lj);
+    else if (!p.dual) {               // equal digit counts (the common case): the fully specialised loops
+      if (Li == 1) gram_produce<1, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else if (Li == 2) gram_produce<2, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+      else gram_produce<3, false>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
+    }
     else if (L == 1) gram_produce<1, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
     else if (L == 2) gram_produce<2, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
     else gram_produce<3, true>(&tmap, &tmapB, p, smem0, bar_full, bar_empty, i0, j0, z);
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (!p.dual) gram_issue_p(p, smem0, tmem, bar_full, bar_empty, &bar_tmem, Li, Lj);
+    if (!p.dual && Li != Lj) gram_issue_p(p, smem0, tmem, bar_full, bar_empty, &bar_tmem, Li, Lj);
+    else if (!p.dual) {
+      if (Li == 1) gram_issue<1, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else if (Li == 2) gram_issue<2, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+      else gram_issue<3, false>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    }
     else if (L == 1) gram_issue<1, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
     else if (L == 2) gram_issue<2, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
     else gram_issue<3, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
