@@ -292,7 +292,7 @@ def run_cuda(args):
                                                "HBM copy GB/s" if roofline["bound"] == "hbm" else
                                                "bf16 %s / 2 (TF32 nominal ratio) / 3 (3xTF32 = fp32-accurate)"
                                                % ("sustained" if total_s > 2.0 else "burst"))
-        prof = os.path.join(ROOT, "profiles", "traffic_%s.json" % w.name)
+        prof = os.path.join(ROOT, "profiles", "traffic_%s.txt" % w.name)   # JSON text written from the ncu capture
         if os.path.exists(prof):      # dram bytes per launch from the committed ncu --set full capture
             with open(prof) as f:
                 roofline["traffic"] = json.load(f).get(dominant)
