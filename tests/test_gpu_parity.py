@@ -302,6 +302,61 @@ def test_search_chunked_equals_unchunked(handle):
     assert e.value.status == lb.ERR_WORKSPACE
 
 
+def test_search_degenerate_sizes(handle):
+    """one candidate (best = worst = 0), a single test sample (accuracy 0 or 1), a single train image
+    per class-less corner: one image through the expander."""
+    w = _small("mnist", 300, 1, 1)
+    got, ref = _search_both(handle, w)
+    assert int(got["best"][0]) == 0 and int(got["best"][1]) == 0
+    assert got["acc"][0] in (0.0, 1.0) and got["acc"][0] == ref["acc"][0]
+    assert _fro(got["W_best"].astype(np.float64), ref["W"][0]) <= TOL_W_FRO
+    # one image, one candidate: every CTA of the tensor-core expander is a ragged batch
+    w1 = _small("gtsrb", 50, 4, 1)
+    x = synth.make_dataset(w1)[0][:1]
+    ker = synth.make_kernels(w1, 1)
+    H = handle.expand(lb.arch_of(w1, 1.0), _dev(x), _dev(ker)).cpu().numpy()
+    assert np.array_equal(H[0].astype(np.int64), orc.expand(_orc_arch(w1), x, ker[0]))
+
+
+def test_argument_errors_on_the_device_path(handle):
+    w = _small("tiny_mnist", 64, 16, 2)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    handle.set_workspace(None)
+    with pytest.raises(lb.LbcnnError) as e:          # no workspace at all
+        handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    assert e.value.status == lb.ERR_WORKSPACE
+    handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+    for bad_C in (0.0, -1.0):                        # C <= 0 (SPEC.md:140)
+        with pytest.raises(lb.LbcnnError) as e:
+            handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, bad_C, _dev(ker))
+        assert e.value.status == lb.ERR_INVALID_ARG
+    with pytest.raises(lb.LbcnnError) as e:          # fewer than two classes
+        handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), 1, w.C, _dev(ker))
+    assert e.value.status == lb.ERR_INVALID_ARG
+    bad = lb.make_arch(8, 8, 1, [(lb.CONV_FULL, 4, 4, 0, 2, 2, 0, 0)], 1.0)      # even kernel size
+    with pytest.raises(lb.LbcnnError) as e:
+        handle.expand(bad, _dev(trx[:, :8, :8]), _dev(ker))
+    assert e.value.status == lb.ERR_INVALID_ARCH
+
+
+def test_host_buffer_entry_equals_device_entry(handle):
+    """lbcnn_search_candidates_host (bench.py's e2e leg) = the device-pointer entry on the same bytes."""
+    w = _small("mnist", 500, 200, 6)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    full, _ = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)
+    handle.set_workspace(None)
+    handle.ensure_workspace(full + lb.host_staging_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand))
+    dev = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a))
+    host = handle.search_candidates_host(arch, t(trx), t(try_), t(tex), t(tey), w.n_classes, w.C, t(ker))
+    for k in ("acc", "correct", "info", "best", "W_best"):
+        assert np.array_equal(dev[k].cpu().numpy(), host[k].numpy()), k
+
+
 def test_staged_calls_replay_the_search(handle):
     """expand -> fit -> score through the three stand-alone entry points reproduces the driver's numbers
     (replay of the best kernels, PAPER.md:94 `use_stored`), and labels agree with the oracle's one by one."""
