@@ -416,6 +416,56 @@ def test_full_size_bench_config_sampled(handle):
             assert _fro(out["W_best"].cpu().numpy().astype(np.float64), Wo) <= TOL_W_FRO
 
 
+def test_full_size_orl_config_sampled(handle):
+    """BASELINE.json configs[3] at FULL size (1024 candidates, dual branch, 120 test samples: a single flipped label
+    would break the 99.9 % / 0.2 pp tolerances) in the launch configuration bench.py times; eight candidates spread over
+    the batch, the best and the worst are checked whole against the oracle -- every predicted label count must be equal."""
+    w = synth.WORKLOADS["orl"]
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    full, _ = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, int(100 * (1 << 30)))
+    handle.set_workspace(None)
+    handle.ensure_workspace(full)
+    out = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    correct = out["correct"].cpu().numpy()
+    acc = out["acc"].cpu().numpy()
+    assert (out["info"].cpu().numpy() == 0).all()
+    best, worst = int(out["best"][0]), int(out["best"][1])
+    assert best == int(np.argmax(correct)) and worst == int(np.argmin(correct))
+    oa = _orc_arch(w)
+    s = float(np.float32(w.feature_scale))
+    for k in sorted({0, 1, 127, 128, 511, 777, 1023, best, worst}):
+        Htr = orc.expand(oa, trx, ker[k]).astype(np.float64) * s
+        Hte = orc.expand(oa, tex, ker[k]).astype(np.float64) * s
+        Wo, inf, _ = orc.elm_fit(Htr, try_, w.n_classes, w.C)
+        po, co, _ = orc.elm_score(Hte, Wo, tey)
+        assert inf == 0
+        assert co == int(correct[k]), (k, co, int(correct[k]))
+        assert abs(co / w.n_test - acc[k]) * 100.0 <= TOL_ACC_PP
+        if k == best:
+            assert _fro(out["W_best"].cpu().numpy().astype(np.float64), Wo) <= TOL_W_FRO
+    handle.set_workspace(None)
+
+
+@pytest.mark.parametrize("name", ["gtsrb", "vggface"])
+def test_full_size_expand_sampled(handle, name):
+    """configs[2] / configs[4]: the expander at the FULL train-set size (the grid, batch and candidate split bench.py
+    times); sampled rows -- first, last, around CTA batch boundaries -- of two candidates must equal the oracle's integers."""
+    w = synth.WORKLOADS[name]
+    trx = synth.make_dataset(w)[0]
+    K0 = w.n_cand - 2
+    ker = synth.make_kernels(w)[K0:]
+    H = handle.expand(lb.arch_of(w, 1.0), _dev(trx), _dev(ker))
+    n = w.n_train
+    rows = np.array([0, 1, 2, 3, 5, 6, 7, n // 2, n // 2 + 1, n - 2, n - 1])
+    Hs = H[:, torch.from_numpy(rows).cuda()].cpu().numpy()
+    del H
+    oa = _orc_arch(w)
+    for j in range(2):
+        assert np.array_equal(Hs[j].astype(np.int64), orc.expand(oa, trx[rows], ker[j])), (name, j)
+
+
 # ---- exact integer Gram on the tensor cores (gram_tc.cu) -------------------------------------------------
 TC_CASES = [  # n, F, c, max_abs, K : digits 1 / 2 / 3, ragged n (not a multiple of 64) and F (not of 16 / 96 / 128)
     (300, 70, 5, 100, 2), (1000, 200, 7, 30000, 3), (777, 333, 4, 900000, 2), (2049, 129, 3, 8000000, 1),
