@@ -10,19 +10,20 @@
  * Conventions (all entry points)
  *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch allocations); pointers
  *     named h_* and all struct / out-parameter pointers are HOST pointers.  The library never
- *     allocates, frees or retains device memory; scratch comes from the caller-provided workspace
- *     (lbcnn_set_workspace).  One exception, owned by the handle: the tensor-core expander keeps a small
- *     stream-ordered scratch buffer (cudaMallocAsync on the call's stream, grown on demand, freed by
- *     lbcnn_destroy) holding the +-1 kernel sets re-laid-out as MMA operands (about 10 KB per candidate).
- *     `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *     allocates, frees or retains device memory; ALL scratch comes from the caller-provided workspace
+ *     (lbcnn_set_workspace), and a call whose scratch does not fit returns LBCNN_ERR_WORKSPACE.
+ *     `stream` is a cudaStream_t passed as void* (NULL = default stream).  The handle's device must be the
+ *     calling thread's current device for every call that takes a stream (lbcnn_create does not change it).
  *   - Every call returns an int status (LBCNN_OK = 0 ...) and only ENQUEUES work on `stream`; it
  *     never synchronises.  Numerical failure is not a status: a non-positive Cholesky pivot j
- *     writes d_info[k] = j + 1 (LAPACK convention) for candidate k and the batch continues.
+ *     writes d_info[k] = j + 1 (LAPACK convention) for candidate k and the batch continues;
+ *     d_info[k] = -1 says candidate k's features broke the LBCNN_H_INTEGER promise (see the flag).
  *   - Layouts: images uint8 NHWC "channels last"; kernel sets int8 with entries
  *     -1/+1, per candidate the layers concatenated, layer l = [n_kernels][Cin_l][k][k]; bias int32
  *     per candidate, layers concatenated, layer l = [Cout_l]; H = features, row-major
  *     [candidate][sample][F] with the C,H,W flatten order f = (o*Hout + i)*Wout + j; W = output
- *     weights row-major [candidate][F][n_classes]; labels int32 in [0, n_classes).
+ *     weights row-major [candidate][F][n_classes]; labels int32 in [0, n_classes) (a label outside
+ *     that range is not an error: its sample gets an all-zero target row and is never counted correct).
  *   - H here is samples x features, the transpose of the listing's H (features x samples,
  *     PAPER.md:66); the listing's H.H^T is H^T H here.
  *   - There is no CPU fallback: without a CUDA device lbcnn_create fails with LBCNN_ERR_CUDA.
@@ -46,14 +47,15 @@ enum {
   LBCNN_ERR_INVALID_ARCH = 2, /* a spatial size < 1, even kernel size, pooling window with no real cell, too large for one SM's shared memory */
   LBCNN_ERR_SHAPE = 3,        /* F / channel mismatch */
   LBCNN_ERR_WORKSPACE = 4,    /* workspace absent or too small (never a hidden allocation) */
-  LBCNN_ERR_CUDA = 5          /* no device / launch or driver error */
+  LBCNN_ERR_CUDA = 5,         /* no device / launch or driver error */
+  LBCNN_ERR_NOMEM = 6         /* host allocation failed (lbcnn_create) */
 };
 
 enum { LBCNN_CONV_FULL = 0, LBCNN_CONV_DEPTHWISE = 1 };
 enum { LBCNN_ACT_NONE = 0, LBCNN_ACT_RELU = 1 };
 
 /* flags of lbcnn_elm_fit */
-#define LBCNN_H_INTEGER 1u /* stored H values are integers with abs < 2^23 (the expander's output with feature_scale = 1): the Gram is then computed exactly on the tensor cores */
+#define LBCNN_H_INTEGER 1u /* stored H values are integers with abs <= 8355711 = 127 (1 + 2^8 + 2^16), three balanced radix-256 int8 digits (the expander's output with feature_scale = 1): the Gram is then computed exactly on the tensor cores.  A candidate holding a value outside that range, or a non-integer, gets d_info[k] = -1 and no W */
 #define LBCNN_FORCE_PRIMAL 2u /* testing: take the F x F branch whatever F and n are */
 #define LBCNN_FORCE_DUAL 4u   /* testing: take the n x n branch */
 
@@ -85,9 +87,21 @@ const char* lbcnn_version(void);
 const char* lbcnn_status_string(int status);
 
 /* Create / destroy a handle bound to CUDA device `device`.  Fails with LBCNN_ERR_CUDA when no
- * such device exists (there is no CPU path). */
+ * such device exists (there is no CPU path), LBCNN_ERR_NOMEM when the host allocation fails.  The
+ * calling thread's current device is not changed. */
 int lbcnn_create(lbcnn_handle_t* h, int device);
 int lbcnn_destroy(lbcnn_handle_t h);
+
+/* Options (testing and measurement; the defaults are the product path).
+ *   LBCNN_OPT_FORCE_SIMT_EXPAND  1: lbcnn_expand always takes the exact int32 SIMT kernel
+ *   LBCNN_OPT_SOLVER             LBCNN_SOLVER_AUTO: F3 picks per system size; _FP64: blocked fp64 Cholesky only;
+ *                                _MIXED: tensor-core (tcgen05) factorisation of split operands + fp64-residual
+ *                                iterative refinement whenever the system is large enough to have a trailing update
+ *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
+ *                                captured CUDA graph (default 1) */
+enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2 };
+enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
+int lbcnn_set_option(lbcnn_handle_t h, int option, int value);
 
 /* Host-only shape arithmetic ("feature vector with size 15680"; Tables II-V).
  * F = Cout_last * Hout * Wout; out_hwc = {Hout, Wout, Cout} of the last layer (may be NULL). */
@@ -96,19 +110,24 @@ int lbcnn_feature_dim(const lbcnn_arch_t* arch, int64_t* F, int32_t out_hwc[3]);
 int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t* n_bias);
 
 /* Workspace.  lbcnn_workspace_bytes gives the size with which lbcnn_search_candidates processes
- * min(n_cand, as many candidates as fit in `budget_bytes`) candidates per chunk (budget 0 = no cap)
- * -- and which is also enough for lbcnn_elm_fit on n_train samples and n_cand candidates.
- * min_bytes (may be NULL) = the size for one candidate per chunk.  The workspace stays owned by the
- * caller and must outlive every call enqueued with it. */
+ * min(n_cand, as many candidates as fit in `budget_bytes`) candidates per chunk (budget 0 = no cap).
+ * min_bytes (may be NULL) = the size for one candidate per chunk.  `h` may be NULL (pure host arithmetic
+ * for a B200).  The stand-alone calls have their own queries: lbcnn_fit_workspace_bytes for
+ * lbcnn_elm_fit with the SAME flags, lbcnn_expand_workspace_bytes for lbcnn_expand.  The workspace
+ * stays owned by the caller and must outlive every call enqueued with it. */
 int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
                           int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes);
 int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
 /* Workspace a stand-alone lbcnn_elm_fit(n, F, n_classes, n_cand, flags) needs (host-only arithmetic). */
 int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes);
+/* Workspace lbcnn_expand needs for n_cand candidates of this architecture: the +-1 kernel sets re-laid-out as
+ * tensor-core operands (about 10 KB per candidate); 0 when the architecture takes the SIMT kernel. */
+int lbcnn_expand_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int32_t n_cand, int32_t has_bias, size_t* bytes);
 
 /* Expander: d_H[k][i][:] = feature_scale * flatten(layers(image i; kernel set k)).
  * The integer feature is exact (signed adds of uint8 pixels, abs < 2^24); the only rounding is the
- * one fp32 multiply by feature_scale.  d_bias may be NULL (= 0).  Needs no workspace. */
+ * one fp32 multiply by feature_scale.  d_bias may be NULL (= 0).  Scratch: the first
+ * lbcnn_expand_workspace_bytes() bytes of the workspace (LBCNN_ERR_WORKSPACE when absent or too small). */
 int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_images /*[n][H][W][C]*/, int64_t n,
                  const int8_t* d_kernels /*[n_cand][n_weights]*/, const int32_t* d_bias /*[n_cand][n_bias] or NULL*/,
                  int32_t n_cand, float* d_H /*[n_cand][n][F]*/, void* stream);

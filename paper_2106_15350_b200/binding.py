@@ -13,17 +13,19 @@ from typing import Optional, Sequence, Tuple
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liblbcnn.so")
 
-OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA = range(6)
+OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA, ERR_NOMEM = range(7)
 CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 EXPAND_SIMT, EXPAND_TENSOR = 0, 1
+OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH = 0, 1, 2
+SOLVER_AUTO, SOLVER_FP64, SOLVER_MIXED = 0, 1, 2
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
-           "lbcnn_get_phase_times")
+           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -198,6 +200,15 @@ class Handle:
             self._ws = None
             self.set_workspace(torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % self.device))
 
+    def set_option(self, option: int, value: int):
+        _check(lib().lbcnn_set_option(self._h, C.c_int(option), C.c_int(value)), "lbcnn_set_option")
+
+    def expand_workspace_bytes(self, arch: Arch, n_cand: int, has_bias: bool = False) -> int:
+        b = C.c_size_t()
+        _check(lib().lbcnn_expand_workspace_bytes(self._h, C.byref(arch), C.c_int32(n_cand), C.c_int32(int(has_bias)),
+                                                  C.byref(b)), "lbcnn_expand_workspace_bytes")
+        return b.value
+
     def expand_path(self, arch: Arch, has_bias: bool = False) -> int:
         """EXPAND_TENSOR (tcgen05 kernel) or EXPAND_SIMT (exact int32 kernel) for this architecture."""
         p = C.c_int32()
@@ -227,6 +238,9 @@ class Handle:
         n, K = images.shape[0], kernels.shape[0]
         if out is None:
             out = torch.empty((K, n, F), dtype=torch.float32, device=images.device)
+        need = self.expand_workspace_bytes(arch, K, bias is not None)
+        if need:
+            self.ensure_workspace(need)
         _check(lib().lbcnn_expand(self._h, C.byref(arch), _ptr(images, torch.uint8), C.c_int64(n),
                                   _ptr(kernels, torch.int8), _ptr(bias, torch.int32, True), C.c_int32(K),
                                   _ptr(out, torch.float32), _stream()), "lbcnn_expand")

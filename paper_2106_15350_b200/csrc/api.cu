@@ -2,7 +2,6 @@
 // planning and the search driver.  All compute is in expand.cu / fit.cu / score.cu; there is no CPU path.
 #include "internal.h"
 #include <new>
-#include <stdlib.h>
 
 // ---- host shape logic -------------------------------------------------------------------------
 // pooling output size (PAPER.md:54 max_pooling_2d(ksize, stride, pad, cover_all=True); PAPER.md:104 28->14->7)
@@ -66,6 +65,7 @@ const char* lbcnn_status_string(int status) {
     case LBCNN_ERR_SHAPE: return "shape mismatch";
     case LBCNN_ERR_WORKSPACE: return "workspace absent or too small";
     case LBCNN_ERR_CUDA: return "CUDA error (no device, launch or driver failure)";
+    case LBCNN_ERR_NOMEM: return "host allocation failed";
     default: return "unknown status";
   }
 }
@@ -75,17 +75,29 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   *h = nullptr;
   int count = 0;
   if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return LBCNN_ERR_CUDA;
-  LB_CUDA_OK(cudaSetDevice(device));
+  // the attributes are queried by device ordinal: the calling thread's current device is left as it was
+  int n_sm = 0, smem_optin = 0;
+  LB_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
+  LB_CUDA_OK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
   lbcnn_handle_s* p = new (std::nothrow) lbcnn_handle_s();
-  if (!p) return LBCNN_ERR_INVALID_ARG;
-  p->device = device;
-  LB_CUDA_OK(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device));
-  LB_CUDA_OK(cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
-  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0; p->xw = nullptr; p->xw_bytes = 0;
-  const char* fs = getenv("LBCNN_FORCE_SIMT_EXPAND");
-  p->force_simt_expand = (fs && fs[0] == '1') ? 1 : 0;
+  if (!p) return LBCNN_ERR_NOMEM;
+  p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
+  p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1;
   *h = p;
   return LBCNN_OK;
+}
+
+int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
+  if (!h) return LBCNN_ERR_INVALID_ARG;
+  switch (option) {
+    case LBCNN_OPT_FORCE_SIMT_EXPAND: h->force_simt_expand = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_SOLVER:
+      if (value != LBCNN_SOLVER_AUTO && value != LBCNN_SOLVER_FP64 && value != LBCNN_SOLVER_MIXED) return LBCNN_ERR_INVALID_ARG;
+      h->solver = value; return LBCNN_OK;
+    case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
+    default: return LBCNN_ERR_INVALID_ARG;
+  }
 }
 
 int lbcnn_set_profiling(lbcnn_handle_t h, int enable) {
@@ -112,7 +124,6 @@ int lbcnn_get_phase_times(lbcnn_handle_t h, float* h_ms, int32_t* h_count) {
 int lbcnn_destroy(lbcnn_handle_t h) {
   if (!h) return LBCNN_ERR_INVALID_ARG;
   for (LbPhaseRec& r : h->recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
-  if (h->xw) cudaFree(h->xw);
   delete h;
   return LBCNN_OK;
 }
@@ -158,31 +169,43 @@ int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes) {
 namespace {
 struct SearchPlan {
   FitPlan fit;
-  size_t fit_off, htr_off, hte_off, w_off, total;
+  size_t xw_off, fit_off, htr_off, hte_off, w_off, total;
 };
-void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, SearchPlan* p) {
+// xw1 = expander scratch per candidate (lb_expand_ws_bytes(.., 1)); kc = candidates per chunk
+void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, SearchPlan* p) {
   lb_fit_plan(n_train, F, c, kc, flags, &p->fit);
   size_t off = 0;
+  p->xw_off = off;  off += (size_t)lb_align_up((int64_t)(xw1 * (size_t)kc), 256);
   p->fit_off = off; off += p->fit.total;
   p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * n_train * F * 4, 256);
   p->hte_off = off; off += (size_t)lb_align_up((int64_t)kc * n_test * F * 4, 256);
   p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
   p->total = off;
 }
-// the driver's features are exact integers; below 2^23 the fit may use the exact tensor-core Gram
-uint32_t search_fit_flags(const ArchShape& s) { return s.max_abs < (1LL << 23) ? LBCNN_H_INTEGER : 0u; }
+// The driver's features are exact integers; inside the digit envelope of the exact tensor-core Gram (three balanced
+// radix-256 digits hold |u| <= 8355711) the fit may use it.  A bias is an arbitrary int32 and is not part of the bound,
+// so a search with bias keeps the general fp64 Gram.
+uint32_t search_fit_flags(const ArchShape& s, bool has_bias) {
+  return (!has_bias && s.max_abs <= LB_H_INTEGER_MAX) ? LBCNN_H_INTEGER : 0u;
+}
 // largest chunk size whose plan fits in `bytes` (0 if none)
-int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t bytes) {
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, size_t bytes) {
   SearchPlan p;
-  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, &p);
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, &p);
   if (p.total <= bytes) return n_cand;
   int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
   while (hi - lo > 1) {
     const int mid = lo + (hi - lo) / 2;
-    plan_search(F, n_train, n_test, c, n_cand, mid, flags, &p);
+    plan_search(F, n_train, n_test, c, n_cand, mid, flags, xw1, &p);
     if (p.total <= bytes) lo = mid; else hi = mid;
   }
   return lo;
+}
+// expander scratch per candidate; a NULL handle (pure host arithmetic) assumes the B200's 227 KB of shared memory
+size_t expand_ws_per_cand(lbcnn_handle_t h, const ArchShape& s, bool has_bias) {
+  lbcnn_handle_s tmp{};
+  tmp.max_smem_optin = 232448;
+  return lb_expand_ws_bytes(h ? h : &tmp, s, has_bias, 1);
 }
 }  // namespace
 
@@ -190,24 +213,32 @@ extern "C" {
 
 int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
                           int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes) {
-  (void)h;   // pure host arithmetic: a NULL handle is accepted
   if (!bytes || n_train < 1 || n_test < 0 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   ArchShape s;
   const int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
+  const uint32_t flags = search_fit_flags(s, false);     // the bias-free plan is the larger one (digit planes)
+  const size_t xw1 = expand_ws_per_cand(h, s, false);
   SearchPlan p1;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, search_fit_flags(s), &p1);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, &p1);
   if (min_bytes) *min_bytes = p1.total;
   int kc = n_cand;
   if (budget_bytes) {
-    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, search_fit_flags(s), budget_bytes);
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, budget_bytes);
     if (kc < 1) kc = 1;
   }
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, search_fit_flags(s), &p);
-  FitPlan fp;   // a stand-alone lbcnn_elm_fit over all n_cand candidates (flags = 0) must fit as well
-  lb_fit_plan(n_train, s.F, n_classes, n_cand, 0, &fp);
-  *bytes = p.total > fp.total ? p.total : fp.total;
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, &p);
+  *bytes = p.total;
+  return LBCNN_OK;
+}
+
+int lbcnn_expand_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int32_t n_cand, int32_t has_bias, size_t* bytes) {
+  if (!h || !bytes || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  ArchShape s;
+  const int rc = lb_arch_shape(arch, &s);
+  if (rc) return rc;
+  *bytes = lb_expand_ws_bytes(h, s, has_bias != 0, n_cand);
   return LBCNN_OK;
 }
 
@@ -217,7 +248,8 @@ int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_im
   ArchShape s;
   const int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
-  return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, (cudaStream_t)stream);
+  return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, h->ws, h->ws_bytes,
+                          (cudaStream_t)stream);
 }
 
 int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes) {
@@ -242,7 +274,7 @@ int lbcnn_elm_fit(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, floa
                   void* stream) {
   if (!h || !d_H || !d_labels || !d_W || !d_info || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   if (!(C > 0.0f) || !(h_scale > 0.0f)) return LBCNN_ERR_INVALID_ARG;
-  if (n > 2147483647LL || F > 2147483647LL) return LBCNN_ERR_INVALID_ARG;
+  if (n > 2147483647LL || F > 2147483647LL || n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
   FitPlan p;
   lb_fit_plan(n, F, n_classes, n_cand, flags, &p);
   if (!h->ws || h->ws_bytes < p.total) return LBCNN_ERR_WORKSPACE;
@@ -274,12 +306,15 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   ArchShape s;
   int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
+  if (n_cand > 65535 * 64) return LBCNN_ERR_INVALID_ARG;
   if (!ws) return LBCNN_ERR_WORKSPACE;
-  const uint32_t fflags = search_fit_flags(s);
-  const int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, ws_bytes);
+  const uint32_t fflags = search_fit_flags(s, d_bias != nullptr);
+  const size_t xw1 = lb_expand_ws_bytes(h, s, d_bias != nullptr, 1);
+  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, ws_bytes);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
+  if (kc > 65535) kc = 65535;                          // grid.y / grid.z of the batched kernels
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, &p);
   char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
@@ -292,9 +327,9 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
     const int8_t* ker = d_kernels + (int64_t)k0 * s.n_weights;
     const int32_t* bias = d_bias ? d_bias + (int64_t)k0 * s.n_bias : nullptr;
     // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale
-    rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, st);
+    rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st);
     if (rc) return rc;
-    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, st);
+    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, base + p.xw_off, xw1 * (size_t)kn, st);
     if (rc) return rc;
     FitPlan fp;
     lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp);

@@ -31,8 +31,6 @@
 // layers, wide layers) takes the exact SIMT kernel in expand.cu.
 #include "internal.h"
 #include "tc_common.cuh"
-#include <stdio.h>
-#include <stdlib.h>
 
 namespace {
 
@@ -54,18 +52,8 @@ struct XtcParams {
   int off_img, off_a1, off_w1, off_w2, off_pl, off_tab1, off_tab2, plane_bytes, plbuf_bytes;
   // TMEM column offsets
   int tm_r1, tm_r2;
-  long long* trace;   // debug builds (-DXTC_TRACE) only
 };
 
-#ifdef XTC_TRACE
-#define XT_TRACE(ev) do { if (tr && (threadIdx.x & 31) == 0 && trn < 8190) tr[trn++] = ((long long)clock64() << 8) | (ev); } while (0)
-#define XT_TRACE_ARGS , long long* tr, int& trn
-#define XT_TRACE_PASS , tr, trn
-#else
-#define XT_TRACE(ev) do { } while (0)
-#define XT_TRACE_ARGS
-#define XT_TRACE_PASS
-#endif
 
 // barrier slots
 enum { W1_FULL = 0, W1_EMPTY = 2, W2_FULL = 4, W2_EMPTY = 7, R1_FULL = 10, R1_EMPTY = 14, PL_FULL = 18, PL_EMPTY = 20,
@@ -138,7 +126,7 @@ __device__ __forceinline__ uint32_t pack4(uint32_t a, uint32_t b, uint32_t c, ui
 
 template <int NPH, bool RELU>
 __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, const uint64_t* bars, uint32_t tmem,
-                                             int set, int quad, int lane, int n_cta_cand XT_TRACE_ARGS) {
+                                             int set, int quad, int lane, int n_cta_cand) {
   constexpr int CPG = 16 / NPH;          // channels per 16-column group
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
   // loop invariants in registers (the asm statements' memory clobbers would otherwise re-read the parameters)
@@ -160,7 +148,6 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
       const uint32_t taddr = taddr0 + slot * N1;
       tc::mbar_wait(bar_full0 + 8 * slot, (n1 >> lg_slot) & 1);
       tc::tc_fence_after();
-      XT_TRACE(6);
       int mx[16];
 #pragma unroll
       for (int e = 0; e < 16; ++e) mx[e] = 0;
@@ -180,8 +167,7 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
       tc::tc_fence_before();
       __syncwarp();
       if (lane == 0) tc::mbar_arrive(bar_empty0 + 8 * slot);               // accumulator slot free again
-      XT_TRACE(7);
-      if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; XT_TRACE(8); }
+      if (!waited) { tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1); waited = true; }
       const int32_t off = tab1[t1 * 128];
       if (off >= 0) {
         // v = 64 (v >> 6) + (v & 63): both digits fit an int8; four channels per word, words past the real channels stay 0
@@ -200,13 +186,11 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
         *reinterpret_cast<uint4*>(dst) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
         *reinterpret_cast<uint4*>(dst + hi_off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
       }
-      XT_TRACE(9);
     }
     if (!waited) tc::mbar_wait(bar_addr(bars, PL_EMPTY + buf), (use & 1) ^ 1);   // never run ahead of the buffer's phase
     tc::fence_proxy_async();                 // generic-proxy plane writes -> visible to the MMA's async proxy
     __syncwarp();
     if (lane == 0) tc::mbar_arrive(bar_addr(bars, PL_FULL + buf));
-    XT_TRACE(10);
   }
 }
 
@@ -214,7 +198,7 @@ __device__ __forceinline__ void e1_two_layer(const XtcParams& p, uint8_t* smem, 
 // tab1[m] = b*F + i*Wo + j of pooled position m (flatten C,H,W adds o*Ho*Wo), -1 = none
 template <int NPH, bool RELU, bool UNIT>
 __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem,
-                                          int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0 XT_TRACE_ARGS) {
+                                          int set, int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
   constexpr int CPG = 16 / NPH;
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
   // loop invariants in registers (the asm statements' memory clobbers would otherwise re-read the parameters)
@@ -295,7 +279,7 @@ __device__ __forceinline__ void e2_store16(float* __restrict__ Hb, uint32_t idx,
 
 template <bool RELU, bool UNIT>
 __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, const uint64_t* bars, uint32_t tmem, int set,
-                                       int quad, int lane, int c_begin, int n_cta_cand, long long img0 XT_TRACE_ARGS) {
+                                       int quad, int lane, int c_begin, int n_cta_cand, long long img0) {
   const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
   const int32_t* tab2 = reinterpret_cast<const int32_t*>(smem + p.off_tab2);
   const int nph2 = p.nph2, N2 = p.N2, cout2 = p.Cout2, T2 = p.T2;
@@ -310,7 +294,6 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
       if ((n2 & 1) != set) continue;
       tc::mbar_wait(bar_addr(bars, R2_FULL + set), (n2 >> 1) & 1);
       tc::tc_fence_after();
-      XT_TRACE(11);
       const int32_t off = tab2[t2 * 128 + quad * 32 + lane];
       for (int c0 = 0; c0 < cout2; c0 += 16) {
         int mx[16];
@@ -335,7 +318,6 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
       tc::tc_fence_before();
       __syncwarp();
       if (lane == 0) tc::mbar_arrive(bar_addr(bars, R2_EMPTY + set));
-      XT_TRACE(12);
     }
   }
 }
@@ -508,11 +490,6 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = tmem_base_s;
-#ifdef XTC_TRACE
-  long long* tr = (p.trace && blockIdx.x == gridDim.x / 2 && blockIdx.y == 0) ? p.trace + warp * 8192 + 1 : nullptr;
-  int trn = 0;
-  XT_TRACE(0);
-#endif
 
   if (warp == 0) {
     // ===== layer-1 issuer =====
@@ -547,13 +524,11 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         const int slot = n1 & (nslot1 - 1);
         tc::mbar_wait(bar_empty0 + 8 * slot, ((n1 >> lg) & 1) ^ 1);
         tc::tc_fence_after();
-        XT_TRACE(1);
         const uint32_t d = d_base + slot * n1cols;
         const uint64_t da_t = da_base + (uint64_t)(t1 * 128);
         for (int ks = 0; ks < nks; ++ks)
           if (tc::elect_one()) tc::mma_i8(d, da_t + (uint64_t)(ks * a_ks), db_c + (uint64_t)(ks * b_ks), idesc1, ks > 0);
         if (tc::elect_one()) tc::mma_commit(bar_full0 + 8 * slot);
-        XT_TRACE(2);
       }
       if (tc::elect_one()) tc::mma_commit(bar_addr(bars, W1_EMPTY + (ci & 1)));
       __syncwarp();
@@ -585,14 +560,12 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
         const int buf = (p.NPB == 2) ? (ci & 1) : 0;
         const int use = (p.NPB == 2) ? (ci >> 1) : ci;
         tc::mbar_wait(bar_addr(bars, PL_FULL + buf), use & 1);
-        XT_TRACE(3);
         const uint32_t pl_base = s_base + p.off_pl + buf * p.plbuf_bytes;
         const uint32_t b_base = s_base + p.off_w2 + wslot * p.w2_bytes;
         for (int t2 = 0; t2 < p.T2; ++t2, ++n2) {
           const int slot = n2 & 1;
           tc::mbar_wait(bar_addr(bars, R2_EMPTY + slot), ((n2 >> 1) & 1) ^ 1);
           tc::tc_fence_after();
-          XT_TRACE(4);
           const uint32_t d0 = tmem + p.tm_r2 + slot * acc_cols;
           const uint32_t row0 = (uint32_t)(p.base0 + t2 * 128) * 16;
           const uint64_t da0 = tc::smem_desc(pl_base + row0, lbo_a, 128, tc::LAYOUT_NONE);
@@ -602,7 +575,6 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
           else l2_issue_tile<0, 0>(p, half, d0, da0, db0, idesc2);
           if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R2_FULL + slot));
           __syncwarp();
-          XT_TRACE(5);
         }
         if (tc::elect_one()) {
           tc::mma_commit(bar_addr(bars, PL_EMPTY + buf));
@@ -615,21 +587,21 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
     const int set = (warp - 2) >> 2, quad = warp & 3;
     if (p.n_layers == 2) {
       const bool relu1 = p.act1 == LBCNN_ACT_RELU;
-      if (p.nph1 == 4 && !relu1) e1_two_layer<4, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else if (p.nph1 == 4) e1_two_layer<4, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else if (p.nph1 == 1 && !relu1) e1_two_layer<1, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else if (p.nph1 == 1) e1_two_layer<1, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else if (!relu1) e1_two_layer<16, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
-      else e1_two_layer<16, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand XT_TRACE_PASS);
+      if (p.nph1 == 4 && !relu1) e1_two_layer<4, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else if (p.nph1 == 4) e1_two_layer<4, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else if (p.nph1 == 1 && !relu1) e1_two_layer<1, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else if (p.nph1 == 1) e1_two_layer<1, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else if (!relu1) e1_two_layer<16, false>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
+      else e1_two_layer<16, true>(p, smem, bars, tmem, set, quad, lane, n_cta_cand);
     } else {
       // the search driver's case (no relu, scale 1) is specialised; everything else takes the general instantiation
       const bool plain = p.act1 != LBCNN_ACT_RELU && p.scale == 1.0f;
 #define XT_E1S(NPH)                                                                                                      \
   do {                                                                                                                   \
-    if (plain) e1_single<NPH, false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS); \
+    if (plain) e1_single<NPH, false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0); \
     else if (p.act1 == LBCNN_ACT_RELU)                                                                                   \
-      e1_single<NPH, true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);         \
-    else e1_single<NPH, false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);     \
+      e1_single<NPH, true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);         \
+    else e1_single<NPH, false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);     \
   } while (0)
       if (p.nph1 == 1) XT_E1S(1);
       else if (p.nph1 == 4) XT_E1S(4);
@@ -640,17 +612,13 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
     const int set = (warp - 2 - n_e1_warps) >> 2, quad = warp & 3;
     const bool relu = p.act2 == LBCNN_ACT_RELU, unit = p.scale == 1.0f;
     if (relu) {
-      if (unit) e2_run<true, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
-      else e2_run<true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      if (unit) e2_run<true, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+      else e2_run<true, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
     } else {
-      if (unit) e2_run<false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
-      else e2_run<false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0 XT_TRACE_PASS);
+      if (unit) e2_run<false, true>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
+      else e2_run<false, false>(p, smem, bars, tmem, set, quad, lane, c_begin, n_cta_cand, img0);
     }
   }
-#ifdef XTC_TRACE
-  XT_TRACE(13);
-  if (tr && lane == 0) tr[-1] = trn;
-#endif
   tc::tc_fence_before();
   __syncthreads();
   if (warp == 0) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, 512); }
@@ -756,34 +724,36 @@ bool lb_expand_tc_usable(const lbcnn_handle_s* h, const ArchShape& s, bool has_b
   return plan_xtc(h, s, has_bias, &q, &sm);
 }
 
+// bytes of caller workspace the tensor-core expander needs for n_cand candidates: the +-1 kernel sets re-laid-out as the
+// shared-memory images of the B operands (0 when the architecture takes the SIMT kernel)
+size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand) {
+  XtcParams q; size_t sm;
+  if (!plan_xtc(h, s, has_bias, &q, &sm)) return 0;
+  return (size_t)lb_align_up((int64_t)n_cand * q.blob_bytes, 256);
+}
+
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
-                        const int8_t* d_kernels, int n_cand, float* d_H, cudaStream_t st) {
+                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st) {
   XtcParams p; size_t smem = 0;
   if (!plan_xtc(h, s, false, &p, &smem)) return LBCNN_ERR_INVALID_ARCH;
-  LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
-  // handle-owned scratch for the re-laid-out kernel sets (stream-ordered allocation, grown on demand)
+  if (n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
+  // scratch for the re-laid-out kernel sets comes from the caller's workspace (never a hidden allocation)
   const size_t need = (size_t)n_cand * p.blob_bytes;
-  if (need > h->xw_bytes) {
-    if (h->xw) LB_CUDA_OK(cudaFreeAsync(h->xw, st));
-    h->xw = nullptr; h->xw_bytes = 0;
-    const size_t cap = (need + ((size_t)1 << 20) - 1) >> 20 << 20;
-    LB_CUDA_OK(cudaMallocAsync(&h->xw, cap, st));
-    h->xw_bytes = cap;
-  }
+  if (!xw || xw_bytes < need) return LBCNN_ERR_WORKSPACE;
+  LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
   {
     PrepParams w{};
-    w.ker = d_kernels; w.n_weights = (int)s.n_weights; w.blob = reinterpret_cast<uint8_t*>(h->xw);
+    w.ker = d_kernels; w.n_weights = (int)s.n_weights; w.blob = reinterpret_cast<uint8_t*>(xw);
     w.blob_bytes = p.blob_bytes; w.w1_bytes = p.w1_bytes; w.n_layers = p.n_layers;
     w.k1 = p.k1; w.P1 = p.P1; w.nph1 = p.nph1; w.Cout1 = p.Cout1; w.N1 = p.N1; w.K1 = p.K1; w.K1p = p.K1p; w.Pk1 = p.Pk1;
     w.Cin1 = p.C; w.w1_off = (int)s.L[0].w_off;
     if (p.n_layers == 2) { w.k2 = p.k2; w.Cout2 = p.Cout2; w.N2 = p.N2; w.w2_off = (int)s.L[1].w_off; }
-    if (n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
     dim3 grid((unsigned)((p.blob_bytes + 1023) / 1024 < 1 ? 1 : (p.blob_bytes + 1023) / 1024), (unsigned)n_cand);
     xtc_prep_kernel<<<grid, 256, 0, st>>>(w);
     h->launches += 1;
     LB_CUDA_OK(cudaGetLastError());
   }
-  p.img = d_images; p.n_img = n; p.wblob = reinterpret_cast<const uint8_t*>(h->xw); p.n_cand = n_cand;
+  p.img = d_images; p.n_img = n; p.wblob = reinterpret_cast<const uint8_t*>(xw); p.n_cand = n_cand;
   p.Hout = d_H; p.F = s.F; p.scale = feature_scale;
   const long long batches = (n + p.B - 1) / p.B;
   // candidates per CTA: as many as possible (they share the staged images and A1) while the grid still
@@ -797,28 +767,9 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
   // one CTA per SM (it owns all 512 TMEM columns): ask for more than half of the SM's shared memory
   if (smem < 120 * 1024) smem = 120 * 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(expand_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  if (getenv("LBCNN_DEBUG"))
-    fprintf(stderr, "[xtc] B=%d T1=%d T2=%d N1=%d K1p=%d N2=%d NPB=%d nslot1=%d smem=%zu cpc=%d grid=%lld x %d blob=%d\n", p.B, p.T1,
-            p.T2, p.N1, p.K1p, p.N2, p.NPB, 1 << p.lg_nslot1, smem, cpc, batches, gy, p.blob_bytes);
   dim3 grid((unsigned)batches, (unsigned)gy);
-  p.trace = nullptr;
-#ifdef XTC_TRACE
-  static long long* d_trace = nullptr;
-  const size_t trace_bytes = (size_t)XT_WARPS * 8192 * 8;
-  if (!d_trace) cudaMalloc(&d_trace, trace_bytes);
-  cudaMemsetAsync(d_trace, 0, trace_bytes, st);
-  p.trace = d_trace;
-#endif
   expand_tc_kernel<<<grid, XT_THREADS, smem, st>>>(p);
   h->launches += 1;
   LB_CUDA_OK(cudaGetLastError());
-#ifdef XTC_TRACE
-  {
-    cudaStreamSynchronize(st);
-    std::vector<long long> hb(XT_WARPS * 8192);
-    cudaMemcpy(hb.data(), d_trace, trace_bytes, cudaMemcpyDeviceToHost);
-    if (FILE* fp = fopen("gpurun_out/xtc_trace.bin", "wb")) { fwrite(hb.data(), 8, hb.size(), fp); fclose(fp); }
-  }
-#endif
   return LBCNN_OK;
 }

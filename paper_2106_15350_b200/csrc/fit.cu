@@ -73,7 +73,9 @@ __global__ void label_perm_kernel(const int32_t* __restrict__ y, int n, int c, i
   extern __shared__ int cnt[];
   for (int t = threadIdx.x; t <= c; t += blockDim.x) cnt[t] = 0;
   __syncthreads();
-  for (int i = threadIdx.x; i < n; i += blockDim.x) atomicAdd(&cnt[y[i] + 1], 1);
+  // a label outside [0, c) belongs to no class: its sample contributes an all-zero target row (include/lbcnn.h)
+  for (int i = threadIdx.x; i < n; i += blockDim.x)
+    if ((unsigned)y[i] < (unsigned)c) atomicAdd(&cnt[y[i] + 1], 1);
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int t = 1; t <= c; ++t) cnt[t] += cnt[t - 1];
@@ -276,7 +278,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, d_labels, c, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, d_labels, c, d_info, st);
       if (rc) return rc;
     } else {
     GemmP g{};
@@ -301,7 +303,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, nullptr, 0, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, nullptr, 0, d_info, st);
       if (rc) return rc;
     } else {
     GemmP g{};

@@ -1,7 +1,7 @@
 // gram_tc.cu -- K2 on the tensor pipe: the EXACT Gram matrix of integer-valued features (F1, PAPER.md:66-70
 // `cp.dot(H,H.T)`), A = U^T U + lam I, with tcgen05.mma kind::i8 and int32 accumulators in TMEM.
 //
-// The expander's features are exact integers (R14).  Every integer u with |u| < 2^23 is written
+// The expander's features are exact integers (R14).  Every integer u with |u| <= 8355711 is written
 // as balanced radix-256 digits  u = d0 + 256 d1 + 65536 d2,  d in [-128, 127]  (1, 2 or 3 digits, chosen
 // per candidate from the data), so
 //     G[i][j] = sum_n u[n][i] u[n][j] = sum_s 256^s P_s[i][j],   P_s = sum_{a+b=s} D_a^T D_b
@@ -57,11 +57,12 @@ __device__ __forceinline__ uint32_t pack_bytes(uint32_t a, uint32_t b, uint32_t 
 }
 __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
                                                     int8_t* __restrict__ planes, int32_t* __restrict__ nlimb,
-                                                    int32_t* __restrict__ nl32, int G32) {
+                                                    int32_t* __restrict__ nl32, int G32, int32_t* __restrict__ info) {
   const int z = blockIdx.y;
   const long long oct_per_row = Fp / 8;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   uint32_t or2 = 0, or3 = 0;
+  bool bad = false;          // a value outside the three-digit envelope, or not an integer: the LBCNN_H_INTEGER promise is broken
   if (t < n * oct_per_row) {
     const long long row = t / oct_per_row;
     const int f0 = (int)(t % oct_per_row) * 8;
@@ -72,9 +73,15 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
       const float4 y = __ldcs(reinterpret_cast<const float4*>(src) + 1);
       v[0] = (int)x.x; v[1] = (int)x.y; v[2] = (int)x.z; v[3] = (int)x.w;
       v[4] = (int)y.x; v[5] = (int)y.y; v[6] = (int)y.z; v[7] = (int)y.w;
+      bad = !((float)v[0] == x.x && (float)v[1] == x.y && (float)v[2] == x.z && (float)v[3] == x.w &&
+              (float)v[4] == y.x && (float)v[5] == y.y && (float)v[6] == y.z && (float)v[7] == y.w);
     } else {
 #pragma unroll
-      for (int q = 0; q < 8; ++q) v[q] = (f0 + q < F) ? (int)src[q] : 0;
+      for (int q = 0; q < 8; ++q) {
+        const float x = (f0 + q < F) ? src[q] : 0.0f;
+        v[q] = (int)x;
+        bad = bad || !((float)v[q] == x);
+      }
     }
     uint32_t t1[8], t2[8];
 #pragma unroll
@@ -83,7 +90,9 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
       t2[q] = (uint32_t)(v[q] + 32896);
       or2 |= t1[q] & 0xFFFFFF00u;
       or3 |= t2[q] & 0xFFFF0000u;
+      bad = bad || (t2[q] + 0x800000u) >= 0x1000000u;       // third digit (t2 >> 16) outside [-128, 127]
     }
+    if (bad) info[z] = -1;
     uint2 w0, w1, w2;
     w0.x = pack_bytes((uint32_t)v[0], (uint32_t)v[1], (uint32_t)v[2], (uint32_t)v[3], 0);
     w0.y = pack_bytes((uint32_t)v[4], (uint32_t)v[5], (uint32_t)v[6], (uint32_t)v[7], 0);
@@ -396,7 +405,8 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {
 // U U^T + lam I (dual).  Primal with d_labels != NULL: rows F .. F + n_classes - 1 of A[z] additionally receive
 // (U^T T)^T, T the one-hot coding of the labels (the appended right-hand-side rows of the Cholesky layout).
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, cudaStream_t st) {
+                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
+                      cudaStream_t st) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   const int c_aug = (primal && d_labels && lb_gram_tc_fuse_rhs(F, n_classes)) ? n_classes : 0;
@@ -411,7 +421,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   {
     const long long work = n * (Fp / 8);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
-    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32);
+    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32, d_info);
     h->launches += 1;
     if (c_aug) {
       dim3 g1((unsigned)((n * c_aug + 255) / 256), (unsigned)n_cand);

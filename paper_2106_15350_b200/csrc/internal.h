@@ -16,8 +16,9 @@ struct lbcnn_handle_s {
   void* ws;
   size_t ws_bytes;
   int64_t launches;
-  void* xw; size_t xw_bytes;        // handle-owned scratch: kernel sets re-laid-out for the tensor-core expander
-  int force_simt_expand;            // testing: keep the expander on the SIMT kernel (LBCNN_FORCE_SIMT_EXPAND=1)
+  int force_simt_expand;            // testing (lbcnn_set_option): keep the expander on the SIMT kernel
+  int solver;                       // LBCNN_SOLVER_* (lbcnn_set_option)
+  int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
 };
@@ -37,6 +38,9 @@ struct LbPhase {
     if (e__ != cudaSuccess) return LBCNN_ERR_CUDA;        \
   } while (0)
 
+// largest |u| three balanced radix-256 int8 digits represent: 127 + 127*256 + 127*65536
+constexpr int64_t LB_H_INTEGER_MAX = 8355711;
+
 static inline int64_t lb_align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 // ---- host shape logic (api.cu) -------------------------------------------------------------
@@ -55,13 +59,17 @@ int lb_pool_out(int n, int k, int s, int p, int cover_all);
 int lb_arch_shape(const lbcnn_arch_t* a, ArchShape* s);
 
 // ---- expander (expand.cu) ------------------------------------------------------------------
+// xw / xw_bytes: caller scratch of lb_expand_ws_bytes() bytes (the tensor-core kernel's prepared operands)
+size_t lb_expand_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand);
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
-                     const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, cudaStream_t st);
+                     const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, void* xw, size_t xw_bytes,
+                     cudaStream_t st);
 
 // tensor-core expander (expand_tc.cu): FULL convolutions, non-overlapping pooling, 1-2 layers, no bias
 bool lb_expand_tc_usable(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias);
+size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand);
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
-                        const int8_t* d_kernels, int n_cand, float* d_H, cudaStream_t st);
+                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st);
 
 // ---- fit (fit.cu) --------------------------------------------------------------------------
 struct FitPlan {
@@ -83,7 +91,8 @@ bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug);
 bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-hot columns of the Gram's digit plane 0
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
-                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, cudaStream_t st);
+                      long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
+                      cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,

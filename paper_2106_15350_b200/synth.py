@@ -302,9 +302,13 @@ def _gen_faces(w: Workload, n_train: int, n_test: int, seed: int, id_amp: float,
     return X[tr], y[tr], X[te], y[te]
 
 
-# amplitudes frozen after calibration with the oracle ("Input recipe")
-_LOWRANK_AMPS = dict(class_amp=10.0, var_amp=22.0, noise=75.0)
-_FACES_AMPS = dict(id_amp=15.0, var_amp=40.0, noise=25.0)
+# amplitudes per workload, frozen after calibration with the oracle ("Input recipe"): the oracle's
+# accuracies must stay below 100 % and spread by at least 2 percentage points across the candidates
+AMPS: Dict[str, Dict[str, float]] = {
+    "gtsrb": dict(class_amp=7.0, var_amp=22.0, noise=75.0),
+    "vggface": dict(class_amp=4.0, var_amp=22.0, noise=75.0),
+    "orl": dict(id_amp=13.0, var_amp=40.0, noise=25.0),
+}
 
 
 def make_dataset(w: Workload):
@@ -314,9 +318,9 @@ def make_dataset(w: Workload):
     if w.generator == "blobs":
         X, y = _gen_blobs(w, w.n_train + w.n_test, seed)
     elif w.generator == "lowrank":
-        X, y = _gen_lowrank(w, w.n_train + w.n_test, seed, **_LOWRANK_AMPS)
+        X, y = _gen_lowrank(w, w.n_train + w.n_test, seed, **AMPS[w.name])
     elif w.generator == "faces":
-        return _gen_faces(w, w.n_train, w.n_test, seed, **_FACES_AMPS)
+        return _gen_faces(w, w.n_train, w.n_test, seed, **AMPS[w.name])
     else:
         raise ValueError(w.generator)
     nt = w.n_train
