@@ -10,10 +10,15 @@ candidate, scores the held-out set and picks best / worst.  De
 BASELINE.json configs[1] ("MNIST-shaped reduced-subset search": N_train 20000, N_test 10000, 64 candidates).
 
 One JSON line on stdout (rank 0):
-  value        candidates/s, inputs resident in HBM, CUDA events on the launching stream, max over ranks
+  value        candidates/s, inputs resident in HBM, CUDA events on the launching stream, max over ranks; the
+               library's per-phase events are OFF in this pass
+  phases       a second pass of the same steps with per-phase CUDA events ON: time, algorithmic work and roofline
+               fraction of every phase, each against the peak of the pipe its kernels run on
+  roofline     the phase with the largest time (`kernel`), copied from `phases`
   e2e          the same metric through lbcnn_search_candidates_host: HOST (pinned) buffers, host<->device
                copies inside the timed region
-  roofline     dominant kernel of the step: algorithmic work / its CUDA-event time in the timed region
+  per_config   value / ms_per_step / e2e / phases / clocks / accuracy of ALL FIVE BASELINE.json configs measured in
+               this run (north_star: "candidates/sec reported for each config"); the headline stays --workload
   cpu_baseline the oracle (oracle/, as it stands) on this box's host cores on a bounded sample
   gpu_launches kernels liblbcnn enqueued inside the timed region (counted by the library)
 
@@ -109,37 +114,63 @@ class ClockSampler:
         return dict(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
 
 
-def _phase_rooflines(w, F, n_cand, phase_ms, steps, peaks, sustained: bool):
+# B200 fp64 pipe: DMMA (mma.sync.m8n8k4.f64) 64 FMA/clk/SM x 148 SMs x 1.965 GHz x 2 (measured 64/clk)
+FP64_TFLOPS = 64 * 148 * 1.965e9 * 2 / 1e12
+
+
+def _phase_rooflines(w, F, n_cand, phase_ms, steps, peaks, sustained: bool, stats=None):
     """Algorithmic work per step for each phase (SURVEY.md 8(d) / DESIGN.md "Rooflines") over its measured
-    CUDA-event time per step.  Returns {phase: roofline-dict}."""
+    CUDA-event time per step.  Every phase is divided by the peak of the pipe its kernels actually run on.
+    Returns {phase: roofline-dict}."""
     N, Nte, c = w.n_train, w.n_test, w.n_classes
     px = w.in_h * w.in_w * w.in_c
     primal = F < N
     dim = F if primal else N
     hbm = peaks["hbm_gbs"]
-    # fp32-accurate tensor peak: TF32 dense = bf16 / 2 (guide's nominal ratio 1.1 / 2.25 PF), three TF32 passes
     bf16 = peaks["bf16_sustained"] if sustained else peaks["bf16_burst"]
+    which = "sustained" if sustained else "burst"
+    # fp32-accurate tensor peak (north_star's Gram denominator): TF32 dense = bf16 / 2 (guide's nominal ratio
+    # 1.1 / 2.25 PF), three TF32 passes.  The kernels themselves run int8 digit products: int8 dense = 2 x bf16.
     tens = bf16 / 2.0 / 3.0
+    int8 = 2.0 * bf16
+    stats = stats or {}
+    gram_flop = n_cand * (float(N) * F * (F + 1) if primal else float(F) * N * (N + 1))
+    solve_flop = n_cand * (dim ** 3 / 3.0 + 2.0 * dim * dim * c + (0 if primal else 2.0 * N * F * c))
     work = {
         # H written once (4 F bytes per image per candidate) + every image read once per launch
-        "expand": ("hbm", "GB/s", hbm, (n_cand * (N + Nte) * F * 4.0 + (N + Nte) * px) / 1e9),
+        "expand": ("hbm", "GB/s", hbm, (n_cand * (N + Nte) * F * 4.0 + (N + Nte) * px) / 1e9, "HBM copy GB/s"),
         # symmetric half of the Gram: N dim (dim + 1) flop per candidate (primal), F N (N + 1) (dual)
-        "gram": ("tensor", "TFLOP/s", tens, n_cand * (float(N) * F * (F + 1) if primal else float(F) * N * (N + 1)) / 1e12),
-        "rhs": ("hbm", "GB/s", hbm, (n_cand * float(N) * F * 4.0 if primal else n_cand * float(N) * c * 8.0) / 1e9),
+        "gram": ("tensor", "TFLOP/s", tens, gram_flop / 1e12,
+                 "bf16 %s / 2 (TF32 nominal ratio) / 3 (3xTF32 = fp32-accurate)" % which),
+        "rhs": ("hbm", "GB/s", hbm, (n_cand * float(N) * F * 4.0 if primal else n_cand * float(N) * c * 8.0) / 1e9,
+                "HBM copy GB/s"),
         # Cholesky dim^3/3 + two triangular solves with c right-hand sides 2 dim^2 c (+ dual back-projection 2 N F c)
-        "solve": ("tensor", "TFLOP/s", tens,
-                  n_cand * (dim ** 3 / 3.0 + 2.0 * dim * dim * c + (0 if primal else 2.0 * N * F * c)) / 1e12),
+        "solve": ("fp64", "TFLOP/s", FP64_TFLOPS, solve_flop / 1e12,
+                  "fp64 DMMA pipe: 64 FMA/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md section 7)"),
         # test features read once + W
-        "score": ("hbm", "GB/s", hbm, n_cand * (float(Nte) * F * 4.0 + F * c * 4.0) / 1e9),
+        "score": ("hbm", "GB/s", hbm, n_cand * (float(Nte) * F * 4.0 + F * c * 4.0) / 1e9, "HBM copy GB/s"),
     }
     out = {}
-    for ph, (bound, unit, peak, amount) in work.items():
+    for ph, (bound, unit, peak, amount, src) in work.items():
         ms = phase_ms.get(ph, (0.0, 0))[0] / max(steps, 1)
         if ms <= 0:
             continue
         ach = amount / (ms * 1e-3)
         out[ph] = dict(bound=bound, achieved=round(ach, 3), peak=round(peak, 1), unit=unit, frac=round(ach / peak, 4),
-                       traffic=None, ms_per_step=round(ms, 4), work_per_step=round(amount, 4))
+                       traffic=None, ms_per_step=round(ms, 4), work_per_step=round(amount, 4),
+                       peak_source="%s (%s)" % (peaks["source"], src))
+    if "gram" in out and stats.get("gram_int8_tmac_per_step"):
+        # the pipe in use: executed int8 multiply-adds (counted by the kernel: digit products actually issued,
+        # tile padding included) against the int8 dense peak = 2 x bf16
+        tops = 2.0 * stats["gram_int8_tmac_per_step"] / (out["gram"]["ms_per_step"] * 1e-3)
+        out["gram"]["int8_pipe"] = dict(achieved=round(tops, 1), peak=round(int8, 1), unit="TOP/s",
+                                        frac=round(tops / int8, 4),
+                                        note="kernel-counted int8 MACs of gram_tc_kernel x 2 / whole Gram phase time")
+    if "solve" in out and stats.get("solve_int8_tmac_per_step"):
+        tops = 2.0 * stats["solve_int8_tmac_per_step"] / (out["solve"]["ms_per_step"] * 1e-3)
+        out["solve"]["int8_pipe"] = dict(achieved=round(tops, 1), peak=round(int8, 1), unit="TOP/s",
+                                         frac=round(tops / int8, 4),
+                                         note="kernel-counted int8 MACs of the trailing updates x 2 / whole solve phase time")
     return out
 
 
@@ -191,6 +222,149 @@ def _config(w, n_cand, l2_note):
                 l2=l2_note)
 
 
+def _git_head_of(paths):
+    """hash of the last commit that touched `paths` (None outside a git checkout, e.g. on the GPU box's snapshot)."""
+    try:
+        r = subprocess.run(["git", "-C", ROOT, "log", "-1", "--format=%H", "--"] + list(paths), capture_output=True,
+                           text=True, timeout=10)
+        return r.stdout.strip() or None
+    except Exception:
+        return None
+
+
+def _traffic(name, phase):
+    """dram bytes per step of `phase` from the committed ncu --set full capture (profiles/traffic_<workload>.txt, JSON
+    text stamped with the commit of csrc/ it was captured at).  Dropped (None) when csrc/ has changed since -- a stale
+    capture must not label a newer kernel; kept when git is unavailable and the stamp cannot be checked."""
+    prof = os.path.join(ROOT, "profiles", "traffic_%s.txt" % name)
+    if not os.path.exists(prof):
+        return None
+    with open(prof) as f:
+        d = json.load(f)
+    head = _git_head_of(["paper_2106_15350_b200/csrc"])
+    if head is not None and d.get("csrc_commit") not in (None, head):
+        return None
+    return d.get(phase)
+
+
+def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, world, rank, local, n_cand=0,
+             with_e2e=True):
+    """one workload: `warmup` untimed steps, `steps` timed steps with profiling OFF (value), the same number of steps
+    again with per-phase events ON (phases), then the host-buffer entry (e2e).  Returns the pieces of the JSON line."""
+    w = synth.WORKLOADS[name]
+    if n_cand:
+        w = synth.scaled(w, n_cand=n_cand)
+    K = w.n_cand
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w, K, first=replicas.first_candidate(rank, K))   # every rank searches its own K candidates
+    arch = lb.arch_of(w)
+    F, _ = lb.feature_dim(arch)
+    dev = torch.device("cuda", local)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_in = [pin(trx), pin(try_), pin(tex), pin(tey), pin(ker)]
+    d_in = [t.to(dev) for t in h_in]
+
+    h = lb.Handle(local)
+    stage = lb.host_staging_bytes(arch, w.n_train, w.n_test, w.n_classes, K)
+    budget = int(ws_gb * (1 << 30))
+    ws_bytes, ws_min = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, budget)
+    h.ensure_workspace(ws_bytes + stage)
+    l2_note = "inputs exceed L2: workspace %.2f GB of features/Gram streams through the 126 MB L2 every step" % (ws_bytes / 1e9)
+    if ws_bytes < 2 * 126e6:
+        l2_note = "workspace %.3f GB; L2 flushed by writing a 256 MB buffer between timed steps" % (ws_bytes / 1e9)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    else:
+        flush = None
+
+    def step(out=None):
+        return h.search_candidates(arch, d_in[0], d_in[1], d_in[2], d_in[3], w.n_classes, w.C, d_in[4], out=out)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps):
+        """CUDA events on the launching (current) stream around each step; the L2 flush sits between the brackets"""
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        barrier()
+        for a, b in evs:
+            if flush is not None:
+                flush.fill_(1)
+            a.record()
+            step(out)
+            b.record()
+        barrier()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    out = step()
+    for _ in range(max(warmup - 1, 0)):
+        step(out)
+    barrier()
+    # ---- timed region: device-resident inputs, per-phase events OFF ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = h.launch_count()
+    ms = timed(steps)
+    launches = h.launch_count() - n0
+    clocks = sampler.stop()
+    ms = replicas.max_over_ranks(ms, dev)
+    # ---- second pass, per-phase CUDA events ON: where the time goes (not part of `value`) ----
+    h.set_profiling(True)
+    timed(steps)
+    phase_ms = h.phase_times()
+    h.set_profiling(False)
+    stats = h.op_stats() if hasattr(h, "op_stats") else {}
+    acc = out["acc"].cpu().numpy()
+    info = out["info"].cpu().numpy()
+    if (info != 0).any() or not np.isfinite(acc).all():
+        raise RuntimeError("fit failed for some candidate: info=%s" % info.tolist())
+
+    res = dict(w=w, K=K, F=F, ms=ms, launches=launches, clocks=clocks, phase_ms=phase_ms, stats=stats, acc=acc,
+               best=int(out["best"][0].item()), l2_note=l2_note, data=(trx, try_, tex, tey), e2e=None)
+    if with_e2e:
+        # ---- e2e: host (pinned) buffers through lbcnn_search_candidates_host, copies inside the timed region ----
+        hout = h.search_candidates_host(arch, *h_in[:4], w.n_classes, w.C, h_in[4])
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            h.search_candidates_host(arch, *h_in[:4], w.n_classes, w.C, h_in[4], out=hout)   # synchronises inside
+        barrier()
+        e2e_s = replicas.max_over_ranks(time.perf_counter() - t0, dev)
+        if not np.array_equal(hout["correct"].numpy(), out["correct"].cpu().numpy()):
+            raise RuntimeError("host-buffer path and device-buffer path disagree")
+        h2d = sum(t.numel() * t.element_size() for t in h_in)
+        d2h = sum(t.numel() * t.element_size() for t in hout.values() if t is not None)
+        res["e2e"] = dict(value=replicas.job_throughput(world, K, steps, e2e_s), unit=UNIT, h2d_bytes_per_step=h2d,
+                          d2h_bytes_per_step=d2h)
+    h.close()
+    del d_in, out, flush
+    torch.cuda.empty_cache()
+    return res
+
+
+DTYPE = ("int8 x int8 -> int32 tensor-core expander, Gram and Cholesky trailing updates (exact digit products), "
+         "f64 Cholesky panels and logits, f32 features/weights")
+
+
+def _summary(res, steps, world, replicas, peaks):
+    total_s = res["ms"] * 1e-3
+    w = res["w"]
+    stats = {k: v / (2.0 * steps) for k, v in res["stats"].items()}     # counters ran over both passes
+    roofs = _phase_rooflines(w, res["F"], res["K"], res["phase_ms"], steps, peaks, sustained=total_s > 2.0, stats=stats)
+    for ph in roofs:
+        roofs[ph]["traffic"] = _traffic(w.name, ph)
+    dominant = max(roofs, key=lambda p: roofs[p]["ms_per_step"]) if roofs else None
+    roofline = dict(roofs[dominant]) if dominant else None
+    if roofline:
+        roofline["kernel"] = dominant
+    acc = res["acc"]
+    return dict(value=replicas.job_throughput(world, res["K"], steps, total_s), ms_per_step=res["ms"] / steps,
+                e2e=res["e2e"], gpu_launches=int(res["launches"]), clocks=res["clocks"], roofline=roofline, phases=roofs,
+                accuracy=dict(best=float(acc.max()), worst=float(acc.min()), best_index=res["best"]),
+                config=_config(w, res["K"], res["l2_note"]))
+
+
 def run_cuda(args):
     import numpy as np
     import torch
@@ -208,103 +382,39 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     lb.lib()   # raises ImportError if liblbcnn.so is not built
 
-    w = synth.WORKLOADS[args.workload]
-    if args.n_cand:
-        w = synth.scaled(w, n_cand=args.n_cand)
-    K = w.n_cand
-    trx, try_, tex, tey = synth.make_dataset(w)
-    ker = synth.make_kernels(w, K, first=replicas.first_candidate(rank, K))   # every rank searches its own K candidates
-    arch = lb.arch_of(w)
-    F, _ = lb.feature_dim(arch)
-    dev = torch.device("cuda", local)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    h_in = [pin(trx), pin(try_), pin(tex), pin(tey), pin(ker)]
-    d_in = [t.to(dev) for t in h_in]
-
-    h = lb.Handle(local)
-    stage = lb.host_staging_bytes(arch, w.n_train, w.n_test, w.n_classes, K)
-    budget = int(args.ws_gb * (1 << 30))
-    ws_bytes, ws_min = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, budget)
-    h.ensure_workspace(ws_bytes + stage)
-    l2_note = "inputs exceed L2: workspace %.2f GB of features/Gram streams through the 126 MB L2 every step" % (ws_bytes / 1e9)
-
-    def step(out=None):
-        return h.search_candidates(arch, d_in[0], d_in[1], d_in[2], d_in[3], w.n_classes, w.C, d_in[4], out=out)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    out = step()
-    for _ in range(max(args.warmup - 1, 0)):
-        step(out)
-    barrier()
-    # ---- timed region: device-resident inputs, CUDA events on the launching (current) stream ----
-    sampler = ClockSampler(local)
-    sampler.start()
-    h.set_profiling(True)
-    n0 = h.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        step(out)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = h.launch_count() - n0
-    phase_ms = h.phase_times()
-    h.set_profiling(False)
-    clocks = sampler.stop()
-    ms = replicas.max_over_ranks(ms, dev)
-    acc = out["acc"].cpu().numpy()
-    info = out["info"].cpu().numpy()
-    if (info != 0).any() or not np.isfinite(acc).all():
-        raise RuntimeError("fit failed for some candidate: info=%s" % info.tolist())
-
-    # ---- e2e: host (pinned) buffers through lbcnn_search_candidates_host, copies inside the timed region ----
-    hout = h.search_candidates_host(arch, *h_in[:4], w.n_classes, w.C, h_in[4])
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        h.search_candidates_host(arch, *h_in[:4], w.n_classes, w.C, h_in[4], out=hout)   # synchronises inside
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = replicas.max_over_ranks(e2e_s, dev)
-    if not np.array_equal(hout["correct"].numpy(), out["correct"].cpu().numpy()):
-        raise RuntimeError("host-buffer path and device-buffer path disagree")
-    h2d = sum(t.numel() * t.element_size() for t in h_in)
-    d2h = sum(t.numel() * t.element_size() for t in hout.values() if t is not None)
+    common = (lb, replicas, synth, torch, np, dist)
+    res = _measure(*common, args.workload, args.steps, args.warmup, args.ws_gb, world, rank, local, n_cand=args.n_cand)
+    peaks = _peaks()
+    main = _summary(res, args.steps, world, replicas, peaks)
+    # ---- the other configs of BASELINE.json (north_star: "candidates/sec reported for each config"), same process,
+    #      same rules (warm-up, events, clocks), fewer timed steps; the headline stays the --workload line ----
+    per_config = {}
+    if not args.no_per_config and not args.n_cand:
+        for name in ("tiny_mnist", "mnist", "gtsrb", "orl", "vggface"):
+            if name == args.workload:
+                per_config[name] = {k: main[k] for k in ("value", "ms_per_step", "e2e", "gpu_launches", "clocks", "phases", "accuracy", "config")}
+                continue
+            r = _measure(*common, name, args.per_config_steps, 3, args.ws_gb, world, rank, local)
+            sm = _summary(r, args.per_config_steps, world, replicas, peaks)
+            sm["steps"] = args.per_config_steps
+            del sm["roofline"]
+            per_config[name] = sm
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
-    peaks = _peaks()
-    total_s = ms * 1e-3
-    roofs = _phase_rooflines(w, F, K, phase_ms, args.steps, peaks, sustained=total_s > 2.0)
-    dominant = max(roofs, key=lambda p: roofs[p]["ms_per_step"]) if roofs else None
-    roofline = dict(roofs[dominant]) if dominant else None
-    if roofline:
-        roofline["kernel"] = dominant
-        roofline["peak_source"] = "%s (%s)" % (peaks["source"],
-                                               "HBM copy GB/s" if roofline["bound"] == "hbm" else
-                                               "bf16 %s / 2 (TF32 nominal ratio) / 3 (3xTF32 = fp32-accurate)"
-                                               % ("sustained" if total_s > 2.0 else "burst"))
-        prof = os.path.join(ROOT, "profiles", "traffic_%s.txt" % w.name)   # JSON text written from the ncu capture
-        if os.path.exists(prof):      # dram bytes per launch from the committed ncu --set full capture
-            with open(prof) as f:
-                roofline["traffic"] = json.load(f).get(dominant)
-    line = dict(metric=METRIC, value=replicas.job_throughput(world, K, args.steps, total_s), unit=UNIT, n_gpus=world, steps=args.steps,
-                warmup=args.warmup, ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak",
-                vs_baseline=None, dtype="int8 x int8 -> int32 tensor-core expander and Gram (exact), f64 Cholesky and logits, f32 features/weights",
-                data="synthetic", config=_config(w, K, l2_note), clocks=clocks,
-                e2e=dict(value=replicas.job_throughput(world, K, args.steps, e2e_s), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
-                gpu_launches=int(launches), roofline=roofline, phases=roofs,
-                accuracy=dict(best=float(acc.max()), worst=float(acc.min()), best_index=int(out["best"][0].item())))
+    w, K, acc = res["w"], res["K"], res["acc"]
+    line = dict(metric=METRIC, value=main["value"], unit=UNIT, n_gpus=world, steps=args.steps,
+                warmup=args.warmup, ms_per_step=main["ms_per_step"], higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype=DTYPE, data="synthetic", config=main["config"], clocks=main["clocks"],
+                e2e=main["e2e"], gpu_launches=main["gpu_launches"], roofline=main["roofline"], phases=main["phases"],
+                accuracy=main["accuracy"])
+    if per_config:
+        line["per_config"] = per_config
     if not args.no_cpu_baseline:
         # bounded sample (about 10-30 s of host work): (candidates, N_train, N_test) of the same workload
+        trx, try_, tex, tey = res["data"]
         nc, ntr, nte = CPU_SAMPLE.get(w.name, (1, w.n_train, w.n_test))
         if args.ref_cands_baseline:
             nc = args.ref_cands_baseline
@@ -337,6 +447,8 @@ def main():
     ap.add_argument("--ref-cands", type=int, default=1, help="--impl reference: candidates per step")
     ap.add_argument("--ref-cands-baseline", type=int, default=0, help="cpu_baseline sample size (candidates); 0 = per workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
+    ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")
     args = ap.parse_args()
     if args.warmup < 1 or args.steps < 1:
         ap.error("--steps and --warmup must be >= 1")

@@ -197,9 +197,12 @@ def search(arch: _Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: 
         correct[k] = corr
         acc[k] = corr / float(len(test_y))
         Ws.append(W); preds.append(pred)
-    best = int(np.argmax(acc))          # first index of the maximum (R13)
-    worst = int(np.argmin(acc))
-    out = dict(acc=acc, correct=correct, info=info, best=best, worst=worst, W_best=Ws[best])
+    # first index of the maximum / of the minimum; failed fits (acc = -1) take part in neither (R13:
+    # "lowest candidate index; failed fits are excluded").  All failed: 0 / 0.
+    okk = np.nonzero(info == 0)[0]
+    best = int(okk[np.argmax(acc[okk])]) if len(okk) else 0
+    worst = int(okk[np.argmin(acc[okk])]) if len(okk) else 0
+    out = dict(acc=acc, correct=correct, info=info, best=best, worst=worst, W_best=Ws[best])   # None if every fit failed
     if keep:
         out["W"], out["pred"] = Ws, preds
     return out

@@ -444,6 +444,26 @@ def test_elm_bad_arguments():
         orc.elm_fit(H, np.array([0, 1, 0], dtype=np.int32), 2, 0.0)     # C must be > 0
 
 
+def test_elm_failure_return_is_first_bad_pivot():
+    """Cholesky without jitter (R11): the return value is (index of the first pivot that is not > 0) + 1,
+    LAPACK's convention.  Pinned by construction: a NaN in feature f poisons row / column f of H^T H only, so pivots
+    0..f-1 are untouched and pivot f is the first to fail (primal); in the dual the same holds for the sample index."""
+    rng = np.random.default_rng(5)
+    y = rng.integers(0, 3, size=40).astype(np.int32)
+    for f_bad, n_bad in ((2, 3), (0, 0), (7, 39)):
+        H = rng.standard_normal((40, 8))
+        H[n_bad, f_bad] = np.nan
+        W, info, br = orc.elm_fit(H, y, 3, 1.0)
+        assert br == 1 and info == f_bad + 1
+        W, info, br = orc.elm_fit(H, y, 3, 1.0, force_branch=2)
+        assert br == 2 and info == n_bad + 1
+    # an indefinite system the ridge cannot repair: none exists for C > 0 with finite H (H^T H + I/C is SPD), and indeed
+    # every finite instance factors
+    for _ in range(20):
+        H = rng.standard_normal((6, 9)) * 1e-8
+        assert orc.elm_fit(H, np.arange(6, dtype=np.int32) % 3, 3, 1e12)[1] == 0
+
+
 # ------------------------------------------------------------------------------------------------
 # score
 # ------------------------------------------------------------------------------------------------
@@ -489,3 +509,31 @@ def test_search_best_worst_and_replay():
     cy = np.zeros(20, dtype=np.int32)
     r2 = orc.search(arch, cx, cy, cx, cy, 2, 10.0, ker[:2], w.feature_scale)
     assert np.all(r2["acc"] == 1.0)
+
+
+def test_search_failed_fit_is_excluded(monkeypatch):
+    """a candidate whose fit fails gets accuracy -1 and info = pivot + 1, takes part in neither best nor worst
+    (R13), and the other candidates' results are what a search over them alone gives."""
+    from paper_2106_15350_b200 import synth
+    w = synth.scaled(synth.WORKLOADS["tiny_mnist"], 250, 100, 4)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    arch = orc.make_arch(w.in_h, w.in_w, w.in_c, w.layers)
+    ker = synth.make_kernels(w)
+    real_fit = orc.elm_fit
+    calls = []
+
+    def poisoned_fit(H, labels, n_classes, Creg, force_branch=0):
+        calls.append(1)
+        if len(calls) == 2:                    # the second candidate's features carry a NaN in feature 5
+            H = H.copy()
+            H[7, 5] = np.nan
+        return real_fit(H, labels, n_classes, Creg, force_branch)
+
+    monkeypatch.setattr(orc, "elm_fit", poisoned_fit)
+    r = orc.search(arch, trx, try_, tex, tey, w.n_classes, w.C, ker, w.feature_scale, keep=True)
+    monkeypatch.setattr(orc, "elm_fit", real_fit)
+    assert r["info"].tolist() == [0, 6, 0, 0] and r["acc"][1] == -1.0 and r["W"][1] is None
+    others = orc.search(arch, trx, try_, tex, tey, w.n_classes, w.C, ker[[0, 2, 3]], w.feature_scale)
+    assert np.array_equal(r["acc"][[0, 2, 3]], others["acc"])
+    assert r["best"] == [0, 2, 3][others["best"]] and r["worst"] == [0, 2, 3][others["worst"]]
+    assert r["best"] != 1 and r["worst"] != 1
