@@ -298,12 +298,21 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
         return sum(a.elapsed_time(b) for a, b in evs)
 
     out = step()
-    for _ in range(max(warmup - 1, 0)):
+    for _ in range(max(warmup - 2, 0)):
         step(out)
     barrier()
-    # ---- timed region: device-resident inputs, per-phase events OFF ----
+    # nvidia-smi needs ~100 ms to deliver its first sample: start it one warm-up step early so that short timed
+    # regions (configs[0], [3]) still get samples under load
     sampler = ClockSampler(local)
     sampler.start()
+    t_w = time.perf_counter()
+    while True:
+        step(out)
+        torch.cuda.synchronize()
+        if warmup < 2 or time.perf_counter() - t_w > 0.25:
+            break
+    barrier()
+    # ---- timed region: device-resident inputs, per-phase events OFF ----
     n0 = h.launch_count()
     ms = timed(steps)
     launches = h.launch_count() - n0

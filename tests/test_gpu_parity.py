@@ -365,6 +365,23 @@ def test_search_with_bias_matches_oracle(handle):
     assert info_i[1] == -1 and info_i[0] == 0 and info_i[2] == 0 and info_i[3] == 0
 
 
+def test_search_is_deterministic_run_to_run(handle):
+    """the tensor-core kernels carry hand-rolled mbarrier pipelines and generic -> async proxy hand-offs; a race would
+    show as run-to-run differences.  Five runs of configs[0] and of a reduced configs[1] must be bit-identical."""
+    for w in (synth.WORKLOADS["tiny_mnist"], _small("mnist", 900, 333, 9)):
+        trx, try_, tex, tey = synth.make_dataset(w)
+        ker = synth.make_kernels(w)
+        arch = lb.arch_of(w)
+        handle.set_workspace(None)
+        handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+        args = (arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+        first = {k: v.clone() for k, v in handle.search_candidates(*args).items()}
+        for _ in range(4):
+            again = handle.search_candidates(*args)
+            for k in first:
+                assert torch.equal(first[k], again[k]), k
+
+
 def test_search_chunked_equals_unchunked(handle):
     w = _small("mnist", 400, 150, 7)
     arch = lb.arch_of(w)
