@@ -265,6 +265,8 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     d_in = [t.to(dev) for t in h_in]
 
     h = lb.Handle(local)
+    for opt, val in OPTIONS:
+        h.set_option(opt, val)
     stage = lb.host_staging_bytes(arch, w.n_train, w.n_test, w.n_classes, K)
     budget = int(ws_gb * (1 << 30))
     ws_bytes, ws_min = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, budget)
@@ -319,11 +321,12 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     clocks = sampler.stop()
     ms = replicas.max_over_ranks(ms, dev)
     # ---- second pass, per-phase CUDA events ON: where the time goes (not part of `value`) ----
+    h.op_stats()                      # reset the device-side int8 operation counters
     h.set_profiling(True)
     timed(steps)
     phase_ms = h.phase_times()
     h.set_profiling(False)
-    stats = h.op_stats() if hasattr(h, "op_stats") else {}
+    stats = h.op_stats()
     acc = out["acc"].cpu().numpy()
     info = out["info"].cpu().numpy()
     if (info != 0).any() or not np.isfinite(acc).all():
@@ -352,6 +355,8 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     return res
 
 
+OPTIONS = []       # (option, value) pairs from --solver / --panel (measurement switches; default = the product path)
+
 DTYPE = ("int8 x int8 -> int32 tensor-core expander, Gram and Cholesky trailing updates (exact digit products), "
          "f64 Cholesky panels and logits, f32 features/weights")
 
@@ -359,7 +364,7 @@ DTYPE = ("int8 x int8 -> int32 tensor-core expander, Gram and Cholesky trailing 
 def _summary(res, steps, world, replicas, peaks):
     total_s = res["ms"] * 1e-3
     w = res["w"]
-    stats = {k: v / (2.0 * steps) for k, v in res["stats"].items()}     # counters ran over both passes
+    stats = {k + "_per_step": v / float(steps) for k, v in res["stats"].items()}     # counted over the phase pass
     roofs = _phase_rooflines(w, res["F"], res["K"], res["phase_ms"], steps, peaks, sustained=total_s > 2.0, stats=stats)
     for ph in roofs:
         roofs[ph]["traffic"] = _traffic(w.name, ph)
@@ -390,6 +395,10 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     lb.lib()   # raises ImportError if liblbcnn.so is not built
+    if args.solver:
+        OPTIONS.append((lb.OPT_SOLVER, {"auto": lb.SOLVER_AUTO, "fp64": lb.SOLVER_FP64, "mixed": lb.SOLVER_MIXED}[args.solver]))
+    if args.panel:
+        OPTIONS.append((lb.OPT_PANEL, args.panel))
 
     common = (lb, replicas, synth, torch, np, dist)
     res = _measure(*common, args.workload, args.steps, args.warmup, args.ws_gb, world, rank, local, n_cand=args.n_cand)
@@ -456,6 +465,8 @@ def main():
     ap.add_argument("--ref-cands", type=int, default=1, help="--impl reference: candidates per step")
     ap.add_argument("--ref-cands-baseline", type=int, default=0, help="cpu_baseline sample size (candidates); 0 = per workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--solver", default="", choices=["", "auto", "fp64", "mixed"], help="LBCNN_OPT_SOLVER (measurement)")
+    ap.add_argument("--panel", type=int, default=0, help="LBCNN_OPT_PANEL (measurement)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
     ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")
     args = ap.parse_args()

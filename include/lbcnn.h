@@ -95,11 +95,15 @@ int lbcnn_destroy(lbcnn_handle_t h);
 /* Options (testing and measurement; the defaults are the product path).
  *   LBCNN_OPT_FORCE_SIMT_EXPAND  1: lbcnn_expand always takes the exact int32 SIMT kernel
  *   LBCNN_OPT_SOLVER             LBCNN_SOLVER_AUTO: F3 picks per system size; _FP64: blocked fp64 Cholesky only;
- *                                _MIXED: tensor-core (tcgen05) factorisation of split operands + fp64-residual
- *                                iterative refinement whenever the system is large enough to have a trailing update
+ *                                _MIXED: the trailing updates of the blocked factorisation run on tcgen05 as int8 digit
+ *                                products of the row-scaled panel (four balanced radix-256 digits, ten of the sixteen digit
+ *                                products: ~2^-27 relative, against 2^-24 of an fp32 factorisation) whenever the system has
+ *                                a trailing update; the matrix, the diagonal blocks and the panel solves stay fp64
  *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
- *                                captured CUDA graph (default 1) */
-enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2 };
+ *                                captured CUDA graph (default 1)
+ *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 512) of the blocked Cholesky when its trailing
+ *                                updates run on the tensor pipe (measurement) */
+enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
 int lbcnn_set_option(lbcnn_handle_t h, int option, int value);
 
@@ -117,6 +121,8 @@ int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t*
  * stays owned by the caller and must outlive every call enqueued with it. */
 int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
                           int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes);
+/* d_ws: 256-byte aligned, at least 256 bytes (its first 256 bytes are zeroed on the default stream: the
+ * measurement counters of lbcnn_get_op_stats), or NULL with bytes = 0 to detach. */
 int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
 /* Workspace a stand-alone lbcnn_elm_fit(n, F, n_classes, n_cand, flags) needs (host-only arithmetic). */
 int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes);
@@ -191,6 +197,12 @@ int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch,
                                  const int8_t* h_kernels, const int32_t* h_bias /*or NULL*/, int32_t n_cand,
                                  float* h_acc /*[n_cand]*/, int32_t* h_correct /*[n_cand]*/, int32_t* h_info /*[n_cand]*/,
                                  int32_t* h_best /*[2]*/, float* h_W_best /*[F][n_classes] or NULL*/, void* stream);
+
+/* Measurement: int8 multiply-adds the tensor-core kernels have issued since the last call (or since
+ * lbcnn_set_workspace), counted on the device in the first 256 bytes of the workspace (every size query above
+ * includes them): h_counts[0] = the exact Gram (F1), h_counts[1] = the Cholesky trailing updates (F3).
+ * Copies two words back, resets them and SYNCHRONISES the device -- call it outside timed regions. */
+int lbcnn_get_op_stats(lbcnn_handle_t h, uint64_t h_counts[2]);
 
 /* Number of kernel launches the library has enqueued through this handle since creation (for
  * bench.py's gpu_launches claim). */

@@ -18,14 +18,14 @@ CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 EXPAND_SIMT, EXPAND_TENSOR = 0, 1
-OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH = 0, 1, 2
+OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH, OPT_PANEL = 0, 1, 2, 3
 SOLVER_AUTO, SOLVER_FP64, SOLVER_MIXED = 0, 1, 2
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
-           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes")
+           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -229,6 +229,13 @@ class Handle:
         cnt = (C.c_int32 * len(PHASES))()
         _check(lib().lbcnn_get_phase_times(self._h, ms, cnt), "lbcnn_get_phase_times")
         return {p: (float(ms[i]), int(cnt[i])) for i, p in enumerate(PHASES)}
+
+    def op_stats(self):
+        """int8 multiply-adds (in units of 1e12) the tensor-core Gram / Cholesky trailing updates issued since the last
+        call; synchronises and resets the device counters."""
+        cnt = (C.c_uint64 * 2)()
+        _check(lib().lbcnn_get_op_stats(self._h, cnt), "lbcnn_get_op_stats")
+        return {"gram_int8_tmac": cnt[0] / 1e12, "solve_int8_tmac": cnt[1] / 1e12}
 
     # ---- the four calls of the path ----------------------------------------------------------
     def expand(self, arch: Arch, images, kernels, bias=None, out=None):

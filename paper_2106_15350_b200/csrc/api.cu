@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512;
   *h = p;
   return LBCNN_OK;
 }
@@ -96,6 +96,9 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
       if (value != LBCNN_SOLVER_AUTO && value != LBCNN_SOLVER_FP64 && value != LBCNN_SOLVER_MIXED) return LBCNN_ERR_INVALID_ARG;
       h->solver = value; return LBCNN_OK;
     case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_PANEL:
+      if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
+      h->panel = value; return LBCNN_OK;
     default: return LBCNN_ERR_INVALID_ARG;
   }
 }
@@ -159,7 +162,20 @@ int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes) {
   if (!h) return LBCNN_ERR_INVALID_ARG;
   if ((d_ws == nullptr) != (bytes == 0)) return LBCNN_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0) return LBCNN_ERR_INVALID_ARG;
+  if (d_ws && bytes < LB_WS_HEAD) return LBCNN_ERR_INVALID_ARG;
   h->ws = d_ws; h->ws_bytes = bytes;
+  if (d_ws) LB_CUDA_OK(cudaMemsetAsync(d_ws, 0, LB_WS_HEAD, 0));     // the measurement counters at the head of the workspace
+  return LBCNN_OK;
+}
+
+int lbcnn_get_op_stats(lbcnn_handle_t h, uint64_t* h_counts) {
+  if (!h || !h_counts) return LBCNN_ERR_INVALID_ARG;
+  h_counts[0] = 0; h_counts[1] = 0;
+  if (!h->ws) return LBCNN_OK;
+  unsigned long long tmp[2] = {0ull, 0ull};
+  LB_CUDA_OK(cudaMemcpy(tmp, h->ws, sizeof(tmp), cudaMemcpyDeviceToHost));      // synchronises: a measurement call
+  LB_CUDA_OK(cudaMemset(h->ws, 0, sizeof(tmp)));
+  h_counts[0] = tmp[0]; h_counts[1] = tmp[1];
   return LBCNN_OK;
 }
 
@@ -224,12 +240,13 @@ int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_
   if (min_bytes) *min_bytes = p1.total;
   int kc = n_cand;
   if (budget_bytes) {
-    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, budget_bytes);
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0);
     if (kc < 1) kc = 1;
   }
   SearchPlan p;
   plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, &p);
-  *bytes = p.total;
+  if (min_bytes) *min_bytes += LB_WS_HEAD;
+  *bytes = p.total + LB_WS_HEAD;
   return LBCNN_OK;
 }
 
@@ -239,6 +256,7 @@ int lbcnn_expand_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int
   const int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
   *bytes = lb_expand_ws_bytes(h, s, has_bias != 0, n_cand);
+  if (*bytes) *bytes += LB_WS_HEAD;
   return LBCNN_OK;
 }
 
@@ -248,7 +266,7 @@ int lbcnn_expand(lbcnn_handle_t h, const lbcnn_arch_t* arch, const uint8_t* d_im
   ArchShape s;
   const int rc = lb_arch_shape(arch, &s);
   if (rc) return rc;
-  return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, h->ws, h->ws_bytes,
+  return lb_launch_expand(h, s, arch->feature_scale, d_images, n, d_kernels, d_bias, n_cand, d_H, lb_ws_base(h), lb_ws_avail(h),
                           (cudaStream_t)stream);
 }
 
@@ -256,7 +274,7 @@ int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n
   if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   FitPlan p;
   lb_fit_plan(n, F, n_classes, n_cand, flags, &p);
-  *bytes = p.total;
+  *bytes = p.total + LB_WS_HEAD;
   return LBCNN_OK;
 }
 
@@ -277,8 +295,8 @@ int lbcnn_elm_fit(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, floa
   if (n > 2147483647LL || F > 2147483647LL || n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
   FitPlan p;
   lb_fit_plan(n, F, n_classes, n_cand, flags, &p);
-  if (!h->ws || h->ws_bytes < p.total) return LBCNN_ERR_WORKSPACE;
-  return lb_launch_fit(h, h->ws, p, d_H, n, F, h_scale, d_labels, n_classes, C, n_cand, d_W, d_info, (cudaStream_t)stream);
+  if (!h->ws || lb_ws_avail(h) < p.total) return LBCNN_ERR_WORKSPACE;
+  return lb_launch_fit(h, lb_ws_base(h), p, d_H, n, F, h_scale, d_labels, n_classes, C, n_cand, d_W, d_info, (cudaStream_t)stream);
 }
 
 int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
@@ -375,7 +393,7 @@ int lbcnn_search_candidates(lbcnn_handle_t h, const lbcnn_arch_t* arch, const ui
                             const int8_t* d_kernels, const int32_t* d_bias, int32_t n_cand, float* d_acc,
                             int32_t* d_correct, int32_t* d_info, int32_t* d_best, float* d_W_best, void* stream) {
   if (!h) return LBCNN_ERR_INVALID_ARG;
-  return search_impl(h, h->ws, h->ws_bytes, arch, d_train, d_train_labels, n_train, d_test, d_test_labels, n_test,
+  return search_impl(h, lb_ws_base(h), lb_ws_avail(h), arch, d_train, d_train_labels, n_train, d_test, d_test_labels, n_test,
                      n_classes, C, d_kernels, d_bias, n_cand, d_acc, d_correct, d_info, d_best, d_W_best, stream);
 }
 
@@ -405,8 +423,8 @@ int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch, con
   if (rc) return rc;
   HostStage p;
   plan_host_stage(s, n_train, n_test, n_classes, n_cand, h_bias != nullptr, &p);
-  if (!h->ws || h->ws_bytes <= p.total) return LBCNN_ERR_WORKSPACE;
-  char* base = reinterpret_cast<char*>(h->ws);
+  if (!h->ws || lb_ws_avail(h) <= p.total) return LBCNN_ERR_WORKSPACE;
+  char* base = lb_ws_base(h);
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t px = (int64_t)s.L[0].hin * s.L[0].win * s.L[0].cin;
   LB_CUDA_OK(cudaMemcpyAsync(base + p.train, h_train, (size_t)(n_train * px), cudaMemcpyHostToDevice, st));
@@ -421,7 +439,7 @@ int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch, con
   int32_t* d_info = reinterpret_cast<int32_t*>(base + p.info);
   int32_t* d_best = reinterpret_cast<int32_t*>(base + p.best);
   float* d_wb = h_W_best ? reinterpret_cast<float*>(base + p.wbest) : nullptr;
-  rc = search_impl(h, base + p.total, h->ws_bytes - p.total, arch, reinterpret_cast<const uint8_t*>(base + p.train),
+  rc = search_impl(h, base + p.total, lb_ws_avail(h) - p.total, arch, reinterpret_cast<const uint8_t*>(base + p.train),
                    reinterpret_cast<const int32_t*>(base + p.train_y), n_train,
                    reinterpret_cast<const uint8_t*>(base + p.test), reinterpret_cast<const int32_t*>(base + p.test_y),
                    n_test, n_classes, C, reinterpret_cast<const int8_t*>(base + p.ker),

@@ -253,6 +253,10 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->tc_off = off;   p->fuse_rhs = (p->use_tc && primal && lb_gram_tc_fuse_rhs(F, n_classes)) ? 1 : 0;
   if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand, p->fuse_rhs ? n_classes : 0);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
+  // digit planes + row scales of the tensor-core trailing updates (chol_tc.cu), for systems large enough to have them
+  p->stc_kmax = (p->dim >= LB_STC_MIN_DIM) ? LB_STC_KMAX : 0;
+  p->stc_off = off;
+  if (p->stc_kmax) off += lb_chol_tc_ws_bytes(p->rows, n_cand, p->stc_kmax);
   p->total = off;
 }
 
@@ -331,7 +335,15 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   // 64-column steps (factor the diagonal block and invert it; panel rows X = A21 L11^-T as a product; update the
   // REST OF THE PANEL only) touch a narrow strip; the wide trailing matrix is updated once per panel with K = NBO,
   // which cuts its read-modify-write traffic by NBO / NB.
-  constexpr int NBO = 256;
+  // With the tensor-core trailing update (chol_tc.cu) the wide update costs ~1/10 of its fp64 time, so the panel is made
+  // wider (its read-modify-write traffic on the trailing matrix falls with 1/NBO).
+  const bool tc_solve = pl.stc_kmax > 0 && (h->solver == LBCNN_SOLVER_MIXED || (h->solver == LBCNN_SOLVER_AUTO && dim >= LB_STC_AUTO_DIM));
+  const int NBO = tc_solve ? h->panel : 256;
+  CholTcCtx tcx;
+  if (tc_solve) {
+    rc = lb_chol_tc_begin(h, base + pl.stc_off, rows, dim, n_cand, pl.stc_kmax, A, a_stride, ld, lb_ws_counter(h, 1), &tcx);
+    if (rc) return rc;
+  }
   const size_t potrf_smem = 2 * NB * (NB + 1) * sizeof(double);
   LB_CUDA_OK(cudaFuncSetAttribute(potrf_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)potrf_smem));
   for (long long J0 = 0; J0 < dim; J0 += NBO) {
@@ -361,7 +373,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
         }
       }
     }
-    if (dim - J1 > 0) {                                                // trailing matrix, K = the whole panel
+    if (dim - J1 > 0 && tc_solve) {                                    // trailing matrix on the tensor pipe
+      rc = lb_chol_tc_update(h, tcx, (int)J1, (int)dim, (int)J0, (int)(J1 - J0), st);
+      if (rc) return rc;
+    } else if (dim - J1 > 0) {                                         // trailing matrix, K = the whole panel
       GemmP g{};
       g.A = A + J1 * ld + J0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
       g.B = A + J1 * ld + J0; g.sBr = ld; g.sBk = 1; g.bB = a_stride;

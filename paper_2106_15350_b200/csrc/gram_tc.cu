@@ -43,6 +43,7 @@ struct GramTcParams {
   int Fcols;           // columns written (primal with fused right-hand side: F features of F + c output rows)
   int dual;            // 0: A = U^T U (operands MN-major: the feature index is contiguous); 1: A = U U^T (K-major)
   double lam;
+  unsigned long long* ops;   // int8 multiply-adds issued (measurement)
 };
 
 // ---- digit split ----------------------------------------------------------------------------------
@@ -328,6 +329,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
     else if (L == 1) gram_issue<1, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
     else if (L == 2) gram_issue<2, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
     else gram_issue<3, true>(p, smem0, tmem, bar_full, bar_empty, &bar_tmem);
+    if (p.ops && lane == 0)
+      atomicAdd(p.ops, (unsigned long long)p.n_iters * (p.dual ? 4 : KS / 32) * (unsigned long long)(Li * Lj) * (TM * TN * 32));
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp % 4) .. +31 =====
     const int q = warp & 3;
@@ -450,7 +453,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   GramTcParams p{};
   p.nlimb = nlimb; p.nl32 = nl32; p.G32 = G32; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
   const int64_t odim = primal ? F + c_aug : n, ocols = primal ? F : n;
-  p.Fcols = (int)ocols;
+  p.Fcols = (int)ocols; p.ops = lb_ws_counter(h, 0);
   p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
   const size_t smem = (size_t)RING_BYTES + 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -18,6 +18,7 @@ struct lbcnn_handle_s {
   int64_t launches;
   int force_simt_expand;            // testing (lbcnn_set_option): keep the expander on the SIMT kernel
   int solver;                       // LBCNN_SOLVER_* (lbcnn_set_option)
+  int panel;                        // panel width of the blocked Cholesky when its trailing updates run on tcgen05
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
@@ -37,6 +38,15 @@ struct LbPhase {
     cudaError_t e__ = (expr);                             \
     if (e__ != cudaSuccess) return LBCNN_ERR_CUDA;        \
   } while (0)
+
+// The first LB_WS_HEAD bytes of the caller's workspace hold the library's measurement counters (zeroed by
+// lbcnn_set_workspace): [0] int8 multiply-adds issued by the Gram kernel, [1] by the Cholesky trailing updates.
+constexpr size_t LB_WS_HEAD = 256;
+static inline char* lb_ws_base(const lbcnn_handle_s* h) { return h->ws ? reinterpret_cast<char*>(h->ws) + LB_WS_HEAD : nullptr; }
+static inline size_t lb_ws_avail(const lbcnn_handle_s* h) { return h->ws_bytes > LB_WS_HEAD ? h->ws_bytes - LB_WS_HEAD : 0; }
+static inline unsigned long long* lb_ws_counter(const lbcnn_handle_s* h, int i) {
+  return h->ws ? reinterpret_cast<unsigned long long*>(h->ws) + i : nullptr;
+}
 
 // largest |u| three balanced radix-256 int8 digits represent: 127 + 127*256 + 127*65536
 constexpr int64_t LB_H_INTEGER_MAX = 8355711;
@@ -77,7 +87,8 @@ struct FitPlan {
   int64_t dim;           // system dimension
   int64_t rows;          // dim + n_classes (right-hand sides appended as rows)
   size_t a_bytes;        // per candidate: rows * dim doubles
-  size_t perm_off, off_off, a_off, tc_off, linv_off, total; // offsets inside the fit workspace
+  size_t perm_off, off_off, a_off, tc_off, linv_off, stc_off, total; // offsets inside the fit workspace
+  int stc_kmax;          // widest panel the tensor-core trailing update is planned for (0: no scratch reserved)
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
   int fuse_rhs;          // ... which then also produces the right-hand side (one-hot label columns)
 };
@@ -93,6 +104,22 @@ bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
                       long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
                       cudaStream_t st);
+
+constexpr int LB_STC_KMAX = 1024;      // widest panel (digit-plane pitch)
+constexpr int LB_STC_MIN_DIM = 512;    // systems below this never reserve the scratch
+constexpr int LB_STC_AUTO_DIM = 1024;  // LBCNN_SOLVER_AUTO takes the tensor-core updates from this dimension on
+// ---- Cholesky trailing updates on tcgen05 (chol_tc.cu) ------------------------------------------------
+struct CholTcCtx {
+  alignas(64) unsigned char tmap[128];   // CUtensorMap of the digit planes
+  int8_t* planes; double* rscale; int pitch;
+  int64_t rows, dim; int n_cand;
+  double* A; long long a_stride, ld;
+  unsigned long long* ops;
+};
+size_t lb_chol_tc_ws_bytes(int64_t rows, int n_cand, int kmax);
+int lb_chol_tc_begin(lbcnn_handle_s* h, void* ws, int64_t rows, int64_t dim, int n_cand, int kmax, double* A,
+                     long long a_stride, long long ld, unsigned long long* ops, CholTcCtx* ctx);
+int lb_chol_tc_update(lbcnn_handle_s* h, const CholTcCtx& ctx, int r0, int c1, int k0, int K, cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,

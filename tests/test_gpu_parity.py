@@ -196,6 +196,45 @@ def test_fit_matches_oracle_general_fp32(handle, n, F, c, flags):
         assert _fro(W[k], Wo) <= 1e-5     # what the fp64 path actually delivers (fp32 rounding of W)
 
 
+@pytest.mark.parametrize("n,F,c,panel,integer", [(1500, 700, 5, 128, False), (2100, 1100, 12, 256, True),
+                                                  (900, 2000, 7, 192, False), (1300, 577, 3, 64, True)])
+def test_fit_tensor_core_solver(handle, n, F, c, panel, integer):
+    """LBCNN_SOLVER_MIXED: the trailing updates of the blocked Cholesky as int8 digit products on tcgen05 (chol_tc.cu).
+    Ragged dimensions (not multiples of 64 / 128 / the panel), primal and dual, well- and ill-conditioned (integer
+    features with a common mode, cond ~ 1e6 like the expander's output): W against the oracle within north_star's
+    1e-3 and against the all-fp64 solver within 1e-4."""
+    rng = np.random.default_rng(n + F)
+    K = 2
+    if integer:
+        base = rng.integers(0, 4000, size=(K, 1, F))
+        H = (base + rng.integers(-300, 300, size=(K, n, F))).astype(np.float32)
+        s, Creg, flags = 1.0 / 255.0, 1e4, lb.H_INTEGER
+    else:
+        H = rng.standard_normal((K, n, F)).astype(np.float32)
+        s, Creg, flags = 1.0, 10.0, 0
+    y = rng.integers(0, c, size=n).astype(np.int32)
+    Hd, yd = _dev(H), _dev(y)
+    handle.set_workspace(None)
+    handle.ensure_workspace(lb.fit_workspace_bytes(n, F, c, K, flags))
+    try:
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_MIXED)
+        handle.set_option(lb.OPT_PANEL, panel)
+        W_tc, info_tc = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=flags)
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_FP64)
+        W_64, info_64 = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=flags)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_AUTO)
+        handle.set_option(lb.OPT_PANEL, 512)
+    assert (info_tc.cpu().numpy() == 0).all() and (info_64.cpu().numpy() == 0).all()
+    sc = float(np.float32(s))
+    for k in range(K):
+        a, b = W_tc[k].cpu().numpy().astype(np.float64), W_64[k].cpu().numpy().astype(np.float64)
+        assert _fro(a, b) <= 1e-4, _fro(a, b)
+        Wo, inf, _ = orc.elm_fit(H[k].astype(np.float64) * sc, y, c, Creg)
+        assert inf == 0 and _fro(a, Wo) <= TOL_W_FRO, _fro(a, Wo)
+
+
 def test_fit_worked_example(handle):
     # tests/golden/worked_examples.txt [elm_small]: H=[[1,0],[0,1],[1,1]], labels [0,1,0], C=1 -> W=[[.625,-.125],[.125,.375]]
     H = np.array([[[1, 0], [0, 1], [1, 1]]], dtype=np.float32)
