@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 1; p->deflate = 1;
   *h = p;
   return LBCNN_OK;
 }
@@ -96,6 +96,8 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
       if (value != LBCNN_SOLVER_AUTO && value != LBCNN_SOLVER_FP64 && value != LBCNN_SOLVER_MIXED) return LBCNN_ERR_INVALID_ARG;
       h->solver = value; return LBCNN_OK;
     case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_INNER_TC: h->inner_tc = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_DEFLATE: h->deflate = value ? 1 : 0; return LBCNN_OK;
     case LBCNN_OPT_PANEL:
       if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
       h->panel = value; return LBCNN_OK;

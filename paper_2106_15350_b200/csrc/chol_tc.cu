@@ -188,16 +188,34 @@ __global__ void __launch_bounds__(NTHREADS, 1) syrk_tc_kernel(const __grid_const
       }
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");                // the eight epilogue warps
-    for (int rr = 0; rr < TM / 8; ++rr) {
-      const int r = ew * (TM / 8) + rr;
-      const long long i = (long long)i0 + r;
-      if (i >= p.rows) break;
-      const long long jmax = (i < p.dim) ? i : (long long)p.c1 - 1;      // last column this row stores
-      double* Arow = p.A + (long long)z * p.a_stride + i * p.ld;
+    // 8 rows x 128 columns per batch: all 32 loads of a lane are issued before the first subtract, so a warp keeps
+    // 8 KB in flight (the per-SM share of HBM needs tens of KB in flight; a load-subtract-store chain per row does not)
+#pragma unroll 1
+    for (int rb = 0; rb < TM / 8; rb += 8) {
+      double v[8][TN / 32];
 #pragma unroll
-      for (int t = 0; t < TN / 32; ++t) {
-        const long long j = (long long)j0 + lane + 32 * t;
-        if (j < p.c1 && j <= jmax) Arow[j] -= S[r * SP + lane + 32 * t];
+      for (int rr = 0; rr < 8; ++rr) {
+        const int r = ew * (TM / 8) + rb + rr;
+        const long long i = (long long)i0 + r;
+        const long long jmax = (i < p.dim) ? i : (long long)p.c1 - 1;      // last column this row stores
+        const double* Arow = p.A + (long long)z * p.a_stride + i * p.ld;
+#pragma unroll
+        for (int t = 0; t < TN / 32; ++t) {
+          const long long j = (long long)j0 + lane + 32 * t;
+          v[rr][t] = (i < p.rows && j < p.c1 && j <= jmax) ? __ldcs(Arow + j) : 0.0;
+        }
+      }
+#pragma unroll
+      for (int rr = 0; rr < 8; ++rr) {
+        const int r = ew * (TM / 8) + rb + rr;
+        const long long i = (long long)i0 + r;
+        const long long jmax = (i < p.dim) ? i : (long long)p.c1 - 1;
+        double* Arow = p.A + (long long)z * p.a_stride + i * p.ld;
+#pragma unroll
+        for (int t = 0; t < TN / 32; ++t) {
+          const long long j = (long long)j0 + lane + 32 * t;
+          if (i < p.rows && j < p.c1 && j <= jmax) Arow[j] = v[rr][t] - S[r * SP + lane + 32 * t];
+        }
       }
     }
     tc::tc_fence_before();

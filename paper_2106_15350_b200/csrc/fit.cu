@@ -362,7 +362,23 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
         g.M = (int)(rows - j1); g.N = nbj; g.K = nbj; g.alpha = 1.0; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
         rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
         if (rc) return rc;
-        if (J1 - j1 > 0) {                                             // rest of the panel: columns j1 .. J1-1
+        // The very first block column carries the features' common mode (all features are positive: L's first column
+        // is 10-100x larger than the rest of its row).  Inside a row-scaled int8 slice it would cost the other columns
+        // that many bits, so its update of the WHOLE trailing matrix stays on the fp64 path and the tensor-core update of
+        // panel 0 starts at column 64.
+        const bool deflate = tc_solve && h->deflate && j0 == 0;
+        if (deflate && dim - j1 > 0) {
+          GemmP u{};
+          u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
+          u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
+          u.C = A + j1 * ld + j1; u.ldc = ld; u.bC = a_stride;
+          u.M = (int)(rows - j1); u.N = (int)(dim - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
+          rc = launch_gemm<double, double, double, true, true>(h, u, n_cand, st);
+          if (rc) return rc;
+        } else if (J1 - j1 > 0 && tc_solve && h->inner_tc) {           // rest of the panel on the tensor pipe (K = 64)
+          rc = lb_chol_tc_update(h, tcx, (int)j1, (int)J1, (int)j0, nbj, st);
+          if (rc) return rc;
+        } else if (J1 - j1 > 0) {                                      // rest of the panel: columns j1 .. J1-1
           GemmP u{};
           u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
           u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
@@ -374,7 +390,8 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
       }
     }
     if (dim - J1 > 0 && tc_solve) {                                    // trailing matrix on the tensor pipe
-      rc = lb_chol_tc_update(h, tcx, (int)J1, (int)dim, (int)J0, (int)(J1 - J0), st);
+      const long long K0 = (h->deflate && J0 == 0) ? ((NB < J1) ? NB : J1) : J0;      // block column 0 was applied in fp64
+      rc = lb_chol_tc_update(h, tcx, (int)J1, (int)dim, (int)K0, (int)(J1 - K0), st);
       if (rc) return rc;
     } else if (dim - J1 > 0) {                                         // trailing matrix, K = the whole panel
       GemmP g{};

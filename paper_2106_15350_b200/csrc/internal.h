@@ -19,6 +19,8 @@ struct lbcnn_handle_s {
   int force_simt_expand;            // testing (lbcnn_set_option): keep the expander on the SIMT kernel
   int solver;                       // LBCNN_SOLVER_* (lbcnn_set_option)
   int panel;                        // panel width of the blocked Cholesky when its trailing updates run on tcgen05
+  int inner_tc;                     // ... and whether the 64-column steps inside a panel use them too
+  int deflate;                      // ... with the first block column's update kept in fp64 (common-mode deflation)
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
