@@ -103,7 +103,8 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                captured CUDA graph (default 1)
  *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 512) of the blocked Cholesky when its trailing
  *                                updates run on the tensor pipe (measurement)
- *   LBCNN_OPT_INNER_TC           0: the 64-column steps inside a panel keep the fp64 DMMA update (default 1: tensor pipe)
+ *   LBCNN_OPT_INNER_TC           1: the 64-column steps inside a panel use the tensor-pipe update too (default 0: fp64 DMMA;
+ *                                at K = 64 the update is bound by its read-modify-write traffic, measured slower)
  *   LBCNN_OPT_DEFLATE            0: the first block column's trailing update goes through the int8 slices too (default 1: it
  *                                stays fp64 -- it carries the common mode of the all-positive features) */
 enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5 };

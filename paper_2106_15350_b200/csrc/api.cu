@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 1; p->deflate = 1;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 0; p->deflate = 1;
   *h = p;
   return LBCNN_OK;
 }
