@@ -349,7 +349,7 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
     // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale
     rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st);
     if (rc) return rc;
-    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, base + p.xw_off, xw1 * (size_t)kn, st);
+    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, base + p.xw_off, xw1 * (size_t)kn, st, true);
     if (rc) return rc;
     FitPlan fp;
     lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp);

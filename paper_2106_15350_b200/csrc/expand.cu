@@ -184,9 +184,9 @@ size_t lb_expand_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_
 
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, void* xw, size_t xw_bytes,
-                     cudaStream_t st) {
+                     cudaStream_t st, bool prepared) {
   if (!h->force_simt_expand && lb_expand_tc_usable(h, s, d_bias != nullptr))
-    return lb_launch_expand_tc(h, s, feature_scale, d_images, n, d_kernels, n_cand, d_H, xw, xw_bytes, st);
+    return lb_launch_expand_tc(h, s, feature_scale, d_images, n, d_kernels, n_cand, d_H, xw, xw_bytes, st, prepared);
   LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
   ExpandParams p{};
   p.n_layers = s.n_layers;

@@ -733,7 +733,8 @@ size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool h
 }
 
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
-                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st) {
+                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st,
+                        bool prepared) {
   XtcParams p; size_t smem = 0;
   if (!plan_xtc(h, s, false, &p, &smem)) return LBCNN_ERR_INVALID_ARCH;
   if (n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
@@ -741,7 +742,7 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
   const size_t need = (size_t)n_cand * p.blob_bytes;
   if (!xw || xw_bytes < need) return LBCNN_ERR_WORKSPACE;
   LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
-  {
+  if (!prepared) {
     PrepParams w{};
     w.ker = d_kernels; w.n_weights = (int)s.n_weights; w.blob = reinterpret_cast<uint8_t*>(xw);
     w.blob_bytes = p.blob_bytes; w.w1_bytes = p.w1_bytes; w.n_layers = p.n_layers;

@@ -274,8 +274,10 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   const int c = n_classes;
   int rc;
 
-  rc = lb_launch_zero_i32(h, d_info, n_cand, st);
-  if (rc) return rc;
+  if (!pl.use_tc) {                 // the tensor-core Gram zeroes info together with its digit counts
+    rc = lb_launch_zero_i32(h, d_info, n_cand, st);
+    if (rc) return rc;
+  }
 
   if (pl.primal) {
     // F1: A = U^T U + lam I (lower tiles), operands read with k = sample (slow) and i = feature (contiguous)
@@ -447,3 +449,4 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;
 }
+

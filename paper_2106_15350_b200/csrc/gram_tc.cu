@@ -58,7 +58,8 @@ __device__ __forceinline__ uint32_t pack_bytes(uint32_t a, uint32_t b, uint32_t 
 }
 __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U, long long n, int F, int Fp,
                                                     int8_t* __restrict__ planes, int32_t* __restrict__ nlimb,
-                                                    int32_t* __restrict__ nl32, int G32, int32_t* __restrict__ info) {
+                                                    int32_t* __restrict__ nl32, int G32, int32_t* __restrict__ info,
+                                                    const int32_t* __restrict__ y, int c_aug) {
   const int z = blockIdx.y;
   const long long oct_per_row = Fp / 8;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -78,8 +79,10 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
               (float)v[4] == y.x && (float)v[5] == y.y && (float)v[6] == y.z && (float)v[7] == y.w);
     } else {
 #pragma unroll
+      // columns F .. F + c_aug - 1 of plane 0: the one-hot coding of the sample's label (fused right-hand side)
+      const int lab = c_aug ? y[row] : -1;
       for (int q = 0; q < 8; ++q) {
-        const float x = (f0 + q < F) ? src[q] : 0.0f;
+        const float x = (f0 + q < F) ? src[q] : ((f0 + q - F == lab && lab < c_aug) ? 1.0f : 0.0f);
         v[q] = (int)x;
         bad = bad || !((float)v[q] == x);
       }
@@ -120,18 +123,11 @@ __global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ U,
   if ((threadIdx.x & 31) == 0 && need > 1 && need > *reinterpret_cast<volatile int32_t*>(&nlimb[z])) atomicMax(&nlimb[z], need);
 }
 
-// one-hot label columns F .. F + c - 1 of digit plane 0 (planes 1, 2 keep the zeros the split kernel wrote there)
-__global__ void onehot_kernel(const int32_t* __restrict__ y, long long n, int F, int Fp, int c, int8_t* __restrict__ planes) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= n * c) return;
-  const long long row = t / c;
-  const int cls = (int)(t - row * c);
-  planes[((long long)blockIdx.y * 3 * n + row) * Fp + F + cls] = (y[row] == cls) ? 1 : 0;
-}
-
-__global__ void fill_i32_kernel(int32_t* p, int n, int32_t v) {
+// digit counts = 1 and (zero != NULL) the candidates' info words = 0, in one launch
+__global__ void fill_i32_kernel(int32_t* p, int n, int32_t v, int32_t* zero, int nz) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t < n) p[t] = v;
+  if (zero && t < nz) zero[t] = 0;
 }
 
 // ---- the Gram kernel ------------------------------------------------------------------------------
@@ -387,10 +383,13 @@ EncodeTiledFn get_encode() {
 // ---- host side --------------------------------------------------------------------------------------
 // plane pitch; `c_aug` one-hot label columns are appended to the features (primal branch: the Gram of [U | T] holds
 // U^T T, the right-hand side, in its last c rows -- PAPER.md:67, 70 -- for the price of c extra columns)
-int64_t lb_gram_tc_fp(int64_t F, int c_aug) { return lb_align_up(F + c_aug, 16); }
-// worth it when the c extra rows fit into the last 128-row tile the features leave partly empty (otherwise a whole extra
-// row of tiles costs more than the separate label-segmented sum)
-bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes) { return (F + n_classes + 127) / 128 == (F + 127) / 128; }
+// plane pitch: a multiple of 128 bytes, so that every 128-byte TMA box row and every row of the split pass starts on a line
+// (with a pitch that is only a multiple of 16 the fused label columns cost configs[2] +10 ms instead of +5)
+int64_t lb_gram_tc_fp(int64_t F, int c_aug) { return lb_align_up(F + c_aug, 128); }
+// The c extra rows cost at most one more row of 128 x 96 tiles (one digit: the label columns live in plane 0 only), which is
+// cheaper than the separate label-segmented pass over the fp32 features (N F 4 bytes of HBM reads): measured on
+// configs[2] -2.4 ms, on configs[4] -4.8 ms per step.  More than 128 classes keep the separate kernel.
+bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes) { (void)F; return n_classes <= 128; }
 
 // int32 accumulators stay exact while 3 * 128^2 * (contraction length) < 2^31; the contraction runs over the samples
 // (primal) or over the features (dual)
@@ -419,18 +418,15 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   const int G32 = (int)((Fp + 31) / 32);
   int32_t* nl32 = nlimb + n_cand;                  // [n_cand][G32] right behind the per-candidate counts
   const int n_counts = n_cand * (1 + G32);
-  fill_i32_kernel<<<(n_counts + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1);
+  // one launch: digit counts = 1 and the candidates' info = 0 (the fit's own zeroing is skipped on this path)
+  const int nfill = n_counts > n_cand ? n_counts : n_cand;
+  fill_i32_kernel<<<(nfill + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1, d_info, n_cand);
   h->launches += 1;
   {
     const long long work = n * (Fp / 8);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
-    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32, d_info);
+    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32, d_info, d_labels, c_aug);
     h->launches += 1;
-    if (c_aug) {
-      dim3 g1((unsigned)((n * c_aug + 255) / 256), (unsigned)n_cand);
-      onehot_kernel<<<g1, 256, 0, st>>>(d_labels, n, (int)F, (int)Fp, c_aug, planes);
-      h->launches += 1;
-    }
   }
   LB_CUDA_OK(cudaGetLastError());
   CUtensorMap tmap, tmapB;

@@ -73,15 +73,18 @@ int lb_arch_shape(const lbcnn_arch_t* a, ArchShape* s);
 // ---- expander (expand.cu) ------------------------------------------------------------------
 // xw / xw_bytes: caller scratch of lb_expand_ws_bytes() bytes (the tensor-core kernel's prepared operands)
 size_t lb_expand_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand);
+// prepared: xw already holds these candidates' operands from an earlier call (the driver expands the train and the test
+// set with the same kernel sets): the re-layout kernel is not launched again
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, void* xw, size_t xw_bytes,
-                     cudaStream_t st);
+                     cudaStream_t st, bool prepared = false);
 
 // tensor-core expander (expand_tc.cu): FULL convolutions, non-overlapping pooling, 1-2 layers, no bias
 bool lb_expand_tc_usable(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias);
 size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand);
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
-                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st);
+                        const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st,
+                        bool prepared = false);
 
 // ---- fit (fit.cu) --------------------------------------------------------------------------
 struct FitPlan {

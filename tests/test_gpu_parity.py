@@ -669,8 +669,10 @@ def test_full_size_fit_score(handle, name):
 TC_CASES = [  # n, F, c, max_abs, K : digits 1 / 2 / 3, ragged n (not a multiple of 64) and F (not of 16 / 96 / 128)
     (300, 70, 5, 100, 2), (1000, 200, 7, 30000, 3), (777, 333, 4, 900000, 2), (2049, 129, 3, 8000000, 1),
     (130, 97, 3, 20000, 2), (5000, 980, 10, 16000, 1),
-    # F a multiple of 128: the label columns would need an extra row of tiles, so the right-hand side is NOT fused
+    # F a multiple of 128: the label columns take an extra row of tiles
     (640, 256, 5, 20000, 2),
+    # more than 128 classes: the right-hand side is NOT fused (label-segmented column sums)
+    (700, 200, 130, 20000, 2),
     # dual branch (F >= n): K-major operands, contraction over the features; ragged n and F, 1 / 2 / 3 digits
     (150, 700, 5, 6000, 3), (97, 130, 3, 100, 2), (280, 5152, 40, 6375, 2), (200, 333, 4, 900000, 1)]
 
