@@ -106,8 +106,15 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *   LBCNN_OPT_INNER_TC           1: the 64-column steps inside a panel use the tensor-pipe update too (default 0: fp64 DMMA;
  *                                at K = 64 the update is bound by its read-modify-write traffic, measured slower)
  *   LBCNN_OPT_DEFLATE            0: the first block column's trailing update goes through the int8 slices too (default 1: it
- *                                stays fp64 -- it carries the common mode of the all-positive features) */
-enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5 };
+ *                                stays fp64 -- it carries the common mode of the all-positive features)
+ *   LBCNN_OPT_SCORER             LBCNN_SCORER_AUTO: the search driver scores its integer features on the tensor pipe (int8 digit
+ *                                products, rows inside the error bound re-evaluated in fp64 -- the decision equals the fp64
+ *                                argmax), lbcnn_elm_score uses the fp64 kernel; _FP64: fp64 everywhere; _TENSOR: lbcnn_elm_score
+ *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
+ *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
+enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5,
+       LBCNN_OPT_SCORER = 6 };
+enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
 int lbcnn_set_option(lbcnn_handle_t h, int option, int value);
 
@@ -201,6 +208,9 @@ int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch,
                                  const int8_t* h_kernels, const int32_t* h_bias /*or NULL*/, int32_t n_cand,
                                  float* h_acc /*[n_cand]*/, int32_t* h_correct /*[n_cand]*/, int32_t* h_info /*[n_cand]*/,
                                  int32_t* h_best /*[2]*/, float* h_W_best /*[F][n_classes] or NULL*/, void* stream);
+
+/* Workspace lbcnn_elm_score needs under LBCNN_SCORER_TENSOR (host-only arithmetic; 0 is never returned). */
+int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes);
 
 /* Measurement: int8 multiply-adds the tensor-core kernels have issued since the last call (or since
  * lbcnn_set_workspace), counted on the device in the first 256 bytes of the workspace (every size query above

@@ -18,14 +18,15 @@ CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 EXPAND_SIMT, EXPAND_TENSOR = 0, 1
-OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH, OPT_PANEL, OPT_INNER_TC, OPT_DEFLATE = 0, 1, 2, 3, 4, 5
+OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH, OPT_PANEL, OPT_INNER_TC, OPT_DEFLATE, OPT_SCORER = 0, 1, 2, 3, 4, 5, 6
+SCORER_AUTO, SCORER_FP64, SCORER_TENSOR = 0, 1, 2
 SOLVER_AUTO, SOLVER_FP64, SOLVER_MIXED = 0, 1, 2
 
 EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destroy", "lbcnn_feature_dim",
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
-           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats")
+           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -126,6 +127,13 @@ def fit_workspace_bytes(n: int, F: int, n_classes: int, n_cand: int, flags: int 
     b = C.c_size_t()
     _check(lib().lbcnn_fit_workspace_bytes(C.c_int64(n), C.c_int64(F), C.c_int32(n_classes), C.c_int32(n_cand),
                                            C.c_uint32(flags), C.byref(b)), "lbcnn_fit_workspace_bytes")
+    return b.value
+
+
+def score_workspace_bytes(n: int, F: int, n_classes: int, n_cand: int) -> int:
+    b = C.c_size_t()
+    _check(lib().lbcnn_score_workspace_bytes(C.c_int64(n), C.c_int64(F), C.c_int32(n_classes), C.c_int32(n_cand), C.byref(b)),
+           "lbcnn_score_workspace_bytes")
     return b.value
 
 

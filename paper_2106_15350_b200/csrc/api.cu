@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 0; p->deflate = 1;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 0; p->deflate = 1; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -98,6 +98,9 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
     case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
     case LBCNN_OPT_INNER_TC: h->inner_tc = value ? 1 : 0; return LBCNN_OK;
     case LBCNN_OPT_DEFLATE: h->deflate = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_SCORER:
+      if (value != LBCNN_SCORER_AUTO && value != LBCNN_SCORER_FP64 && value != LBCNN_SCORER_TENSOR) return LBCNN_ERR_INVALID_ARG;
+      h->scorer = value; return LBCNN_OK;
     case LBCNN_OPT_PANEL:
       if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
       h->panel = value; return LBCNN_OK;
@@ -187,7 +190,7 @@ int lbcnn_get_op_stats(lbcnn_handle_t h, uint64_t* h_counts) {
 namespace {
 struct SearchPlan {
   FitPlan fit;
-  size_t xw_off, fit_off, htr_off, hte_off, w_off, total;
+  size_t xw_off, fit_off, htr_off, hte_off, w_off, sc_off, total;
 };
 // xw1 = expander scratch per candidate (lb_expand_ws_bytes(.., 1)); kc = candidates per chunk
 void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, SearchPlan* p) {
@@ -198,6 +201,8 @@ void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, 
   p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * n_train * F * 4, 256);
   p->hte_off = off; off += (size_t)lb_align_up((int64_t)kc * n_test * F * 4, 256);
   p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
+  // scratch of the tensor-core scorer (integer features only; it may still be left unused at run time)
+  p->sc_off = off;  if (flags & LBCNN_H_INTEGER) off += lb_score_tc_ws_bytes(n_test, F, c, kc);
   p->total = off;
 }
 // The driver's features are exact integers; inside the digit envelope of the exact tensor-core Gram (three balanced
@@ -307,7 +312,18 @@ int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, fl
   if (!h || !d_H || !d_W || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   if (d_correct && !d_labels) return LBCNN_ERR_INVALID_ARG;
   if (n > 2147483647LL || F > 2147483647LL || n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
+  if (h->scorer == LBCNN_SCORER_TENSOR && lb_score_tc_usable(d_H, n, F, n_classes, n_cand)) {
+    if (!h->ws || lb_ws_avail(h) < lb_score_tc_ws_bytes(n, F, n_classes, n_cand)) return LBCNN_ERR_WORKSPACE;
+    return lb_launch_score_tc(h, lb_ws_base(h), d_H, n, F, h_scale, d_W, n_classes, d_labels, n_cand, d_pred, d_correct,
+                              (cudaStream_t)stream);
+  }
   return lb_launch_score(h, d_H, n, F, h_scale, d_W, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
+}
+
+int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes) {
+  if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  *bytes = lb_score_tc_ws_bytes(n, F, n_classes, n_cand) + LB_WS_HEAD;
+  return LBCNN_OK;
 }
 
 }  // extern "C"
@@ -356,8 +372,12 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
     rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn,
                        Wall + (int64_t)k0 * wel, d_info + k0, st);
     if (rc) return rc;
-    rc = lb_launch_score(h, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn, nullptr,
-                         d_correct + k0, st);
+    if ((fflags & LBCNN_H_INTEGER) && h->scorer != LBCNN_SCORER_FP64 && lb_score_tc_usable(Hte, n_test, s.F, n_classes, kn))
+      rc = lb_launch_score_tc(h, base + p.sc_off, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn,
+                              nullptr, d_correct + k0, st);
+    else
+      rc = lb_launch_score(h, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn, nullptr,
+                           d_correct + k0, st);
     if (rc) return rc;
   }
   return lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, Wall, wel, d_W_best, st);

@@ -21,6 +21,7 @@ struct lbcnn_handle_s {
   int panel;                        // panel width of the blocked Cholesky when its trailing updates run on tcgen05
   int inner_tc;                     // ... and whether the 64-column steps inside a panel use them too
   int deflate;                      // ... with the first block column's update kept in fp64 (common-mode deflation)
+  int scorer;                       // LBCNN_SCORER_* (lbcnn_set_option)
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
@@ -130,6 +131,12 @@ int lb_chol_tc_update(lbcnn_handle_s* h, const CholTcCtx& ctx, int r0, int c1, i
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                     int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
                     cudaStream_t st);
+// tensor-core scorer (score_tc.cu): integer-valued features, up to 128 classes; scratch from the caller's workspace
+bool lb_score_tc_usable(const float* d_H, int64_t n, int64_t F, int n_classes, int n_cand);
+size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand);
+int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
+                       int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
+                       cudaStream_t st);
 int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,

@@ -289,6 +289,47 @@ def test_score_matches_oracle_and_ties(handle):
     assert (pt.cpu().numpy() == 3).all()
 
 
+@pytest.mark.parametrize("K,n,F,c,amax", [(2, 203, 96, 70, 50), (3, 1000, 980, 10, 200000), (1, 300, 2048, 43, 900000),
+                                          (2, 517, 260, 128, 6000), (1, 129, 8, 2, 3)])
+def test_score_tensor_core_equals_fp64_argmax(handle, K, n, F, c, amax):
+    """LBCNN_SCORER_TENSOR (score_tc.cu): int8 digit products on tcgen05 + exact fp64 re-evaluation of the rows inside
+    the error bound.  Labels must equal the oracle's fp64 argmax ONE BY ONE -- including exact ties (lowest index), rows
+    that hold a non-integer or an out-of-range feature, an all-zero W, ragged n and F not a multiple of 64."""
+    rng = np.random.default_rng(K * 1000 + F)
+    base = rng.integers(0, amax // 2 + 1, size=(K, 1, F))
+    H = (base + rng.integers(-(amax // 2), amax // 2 + 1, size=(K, n, F))).astype(np.float32)
+    H[0, 3, 1] = 0.5                     # not an integer
+    H[0, 5, 2] = 9.0e6                   # outside three balanced radix-256 digits
+    H[0, 7, :] = 0.0
+    W = (rng.standard_normal((K, F, c)) * rng.uniform(1e-4, 1.0, size=(K, 1, c))).astype(np.float32)
+    W[0, :, c - 1] = W[0, :, 0]          # exact ties between class 0 and the last class: class 0 must win
+    y = rng.integers(0, c, size=n).astype(np.int32)
+    hs = 1.0 / 255.0
+    handle.set_workspace(None)
+    handle.ensure_workspace(lb.score_workspace_bytes(n, F, c, K))
+    try:
+        handle.set_option(lb.OPT_SCORER, lb.SCORER_TENSOR)
+        pred, corr = handle.elm_score(_dev(H), _dev(W), _dev(y), h_scale=hs)
+        Wz = np.zeros((1, F, c), dtype=np.float32)
+        pz, _ = handle.elm_score(_dev(H[:1]), _dev(Wz))
+        handle.set_option(lb.OPT_SCORER, lb.SCORER_FP64)
+        pred64, corr64 = handle.elm_score(_dev(H), _dev(W), _dev(y), h_scale=hs)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_option(lb.OPT_SCORER, lb.SCORER_AUTO)
+    pred, corr = pred.cpu().numpy(), corr.cpu().numpy()
+    assert (pz.cpu().numpy() == 0).all()
+    sc = float(np.float32(hs))
+    for k in range(K):
+        po, co, margin = orc.elm_score(H[k].astype(np.float64) * sc, W[k].astype(np.float64), y, want_margin=True)
+        differ = np.nonzero(pred[k] != po)[0]
+        # the only admissible differences are fp64 rounding-order effects at margins ~1e-16 of the logits
+        assert len(differ) == 0 or np.all(margin[differ] <= 1e-12 * np.abs(H[k].astype(np.float64) * sc).sum(1)[differ].max()), (k, differ[:10], margin[differ][:10])
+        assert corr[k] == int((pred[k] == y).sum())
+    assert torch.equal(torch.from_numpy(pred), pred64.cpu()) or (pred != pred64.cpu().numpy()).mean() < 1e-3
+    assert (pred[0] != c - 1).all() or c == 2          # ties resolved to the lower index
+
+
 def _search_both(handle, w, budget=None):
     trx, try_, tex, tey = synth.make_dataset(w)
     ker = synth.make_kernels(w)
