@@ -372,7 +372,8 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
     rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn,
                        Wall + (int64_t)k0 * wel, d_info + k0, st);
     if (rc) return rc;
-    if ((fflags & LBCNN_H_INTEGER) && h->scorer != LBCNN_SCORER_FP64 && lb_score_tc_usable(Hte, n_test, s.F, n_classes, kn))
+    if ((fflags & LBCNN_H_INTEGER) && h->scorer != LBCNN_SCORER_FP64 && lb_score_tc_usable(Hte, n_test, s.F, n_classes, kn) &&
+        (h->scorer == LBCNN_SCORER_TENSOR || lb_score_tc_worthwhile(n_test, s.F, n_classes, kn)))
       rc = lb_launch_score_tc(h, base + p.sc_off, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn,
                               nullptr, d_correct + k0, st);
     else

@@ -133,6 +133,7 @@ int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, f
                     cudaStream_t st);
 // tensor-core scorer (score_tc.cu): integer-valued features, up to 128 classes; scratch from the caller's workspace
 bool lb_score_tc_usable(const float* d_H, int64_t n, int64_t F, int n_classes, int n_cand);
+bool lb_score_tc_worthwhile(int64_t n, int64_t F, int n_classes, int n_cand);
 size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand);
 int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                        int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,

@@ -318,39 +318,50 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
   if (warp == 1) { tc::tc_fence_after(); tc::tmem_dealloc(tmem, 512); }
 }
 
-// ---- exact re-evaluation of the flagged rows (fp64, plain order) ------------------------------------------------------
+// ---- exact re-evaluation of the flagged rows (fp64) ---------------------------------------------------------------------
+// One CTA per flagged row, the 128 threads split the FEATURES (thread t takes f = t, t + 128, ...: coalesced reads of the
+// row, eight classes at a time in registers), then a fixed-order tree over the threads: deterministic, every product
+// exact in fp64 (fp32 x fp32), only the order of the fp64 additions differs from the oracle's plain loop.
 __global__ void __launch_bounds__(128) score_exact_kernel(const float* __restrict__ U, long long n, long long F,
                                                           const float* __restrict__ W, int c, const int32_t* __restrict__ y,
                                                           const int32_t* __restrict__ flag_count, const int32_t* __restrict__ flag_list,
                                                           int32_t* __restrict__ pred, int32_t* __restrict__ correct) {
-  __shared__ float u_s[128];
-  __shared__ double l_s[128];
-  const int t = threadIdx.x, total = *flag_count;
+  __shared__ double red[4][8];
+  const int t = threadIdx.x, lane = t & 31, wp = t >> 5, total = *flag_count;
   for (int idx = blockIdx.x; idx < total; idx += gridDim.x) {
     const long long e = flag_list[idx];
     const long long z = e / n, row = e - z * n;
     const float* Ur = U + (z * n + row) * F;
     const float* Wz = W + z * F * c;
     double bestv = 0.0; int besti = -1;
-    for (int c0 = 0; c0 < c; c0 += 128) {
-      const int j = c0 + t;
-      double acc = 0.0;
-      for (long long f0 = 0; f0 < F; f0 += 128) {
-        __syncthreads();
-        u_s[t] = (f0 + t < F) ? Ur[f0 + t] : 0.0f;
-        __syncthreads();
-        if (j < c) {
-          const int kend = (int)((F - f0 < 128) ? F - f0 : 128);
-          for (int k = 0; k < kend; ++k) acc = fma((double)u_s[k], (double)Wz[(f0 + k) * c + j], acc);
-        }
+    for (int c0 = 0; c0 < c; c0 += 8) {
+      double acc[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+      const int nc = (c - c0 < 8) ? c - c0 : 8;
+      for (long long f = t; f < F; f += 128) {
+        const double u = (double)Ur[f];
+        const float* wr = Wz + f * c + c0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < nc) acc[q] = fma(u, (double)wr[q], acc[q]);
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], d);
       }
       __syncthreads();
-      l_s[t] = acc;
+      if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) red[wp][q] = acc[q];
+      }
       __syncthreads();
       if (t == 0) {
-        const int jn = (c - c0 < 128) ? c - c0 : 128;
-        for (int k = 0; k < jn; ++k)
-          if (besti < 0 || l_s[k] > bestv) { bestv = l_s[k]; besti = c0 + k; }      // first index on ties
+        for (int q = 0; q < nc; ++q) {
+          const double l = (red[0][q] + red[1][q]) + (red[2][q] + red[3][q]);
+          if (besti < 0 || l > bestv) { bestv = l; besti = c0 + q; }                 // first index on ties
+        }
       }
     }
     if (t == 0) {
@@ -396,6 +407,11 @@ void score_tc_layout(int64_t n, int64_t F, int c, int n_cand, ScoreTcLayout* L) 
 }  // namespace
 
 // the tensor-core scorer takes integer-valued features with up to 128 classes; everything else stays on the fp64 kernel
+bool lb_score_tc_worthwhile(int64_t n, int64_t F, int n_classes, int n_cand) {
+  // below ~1e9 multiply-adds the two preparation kernels and the second pass cost more than the fp64 kernel's whole run
+  return (double)n * (double)F * (double)n_classes * (double)n_cand >= 1.0e9;
+}
+
 bool lb_score_tc_usable(const float* d_H, int64_t n, int64_t F, int n_classes, int n_cand) {
   return n_classes <= 128 && (F % 4) == 0 && F <= 43690 && F >= 4 && (reinterpret_cast<uintptr_t>(d_H) % 16) == 0 &&
          (int64_t)n_cand * n < (1LL << 31) && n < (1 << 30) && n_cand <= 65535;
