@@ -269,7 +269,21 @@ __device__ __forceinline__ void gram_issue_p(const GramTcParams& p, uint32_t sme
 
 __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmapB,
                                                                const GramTcParams p) {
-  const int ti = blockIdx.y, tj = blockIdx.x, z = blockIdx.z;
+  // Tile order.  CTAs are scheduled in linear block order, and one candidate's digit planes (configs[4]: 3 x 166 MB) do
+  // not fit the 126 MB L2.  With the natural order (all column tiles of one row tile, then the next row) the ~148 CTAs
+  // in flight share ONE row operand and stream 86 different column operands: every row of tiles re-reads all planes from
+  // HBM (measured 373 GB per launch, the kernel was HBM-bound at 3.9 TB/s).  Bands of RB row tiles, column-major inside
+  // the band, make the CTAs in flight a ~RB x 12 block of tiles that shares RB row operands and ~12 column operands.
+  constexpr int RB = 12;
+  const int z = blockIdx.z;
+  int ti, tj;
+  {
+    const int lin = blockIdx.y * gridDim.x + blockIdx.x;
+    const int band = lin / (RB * gridDim.x), rem = lin - band * (RB * gridDim.x);
+    const int rows = min(RB, (int)gridDim.y - band * RB);
+    tj = rem / rows;
+    ti = band * RB + (rem - tj * rows);
+  }
   const int i0 = ti * TM, j0 = tj * TN;
   if (j0 > i0 + TM - 1) return;                 // tile entirely above the diagonal
   extern __shared__ __align__(1024) uint8_t smem_raw[];
