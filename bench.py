@@ -405,6 +405,8 @@ def run_cuda(args):
         OPTIONS.append((lb.OPT_PANEL, args.panel))
     if args.inner_tc >= 0:
         OPTIONS.append((lb.OPT_INNER_TC, args.inner_tc))
+    if args.mid_panel >= 0:
+        OPTIONS.append((lb.OPT_MID_PANEL, args.mid_panel))
     if args.scorer:
         OPTIONS.append((lb.OPT_SCORER, {"auto": lb.SCORER_AUTO, "fp64": lb.SCORER_FP64, "tensor": lb.SCORER_TENSOR}[args.scorer]))
 
@@ -476,6 +478,7 @@ def main():
     ap.add_argument("--solver", default="", choices=["", "auto", "fp64", "mixed"], help="LBCNN_OPT_SOLVER (measurement)")
     ap.add_argument("--panel", type=int, default=0, help="LBCNN_OPT_PANEL (measurement)")
     ap.add_argument("--inner-tc", type=int, default=-1, help="LBCNN_OPT_INNER_TC (measurement)")
+    ap.add_argument("--mid-panel", type=int, default=-1, help="LBCNN_OPT_MID_PANEL (measurement)")
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
     ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")

@@ -101,7 +101,9 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                a trailing update; the matrix, the diagonal blocks and the panel solves stay fp64
  *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
  *                                captured CUDA graph (default 1)
- *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 512) of the blocked Cholesky when its trailing
+ *   LBCNN_OPT_MID_PANEL          width (multiple of 64; default 256; 0 = none) of the blocks inside a panel whose 64-column steps
+ *                                run in fp64; a finished block updates the rest of its panel on the tensor pipe
+ *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 1024) of the blocked Cholesky when its trailing
  *                                updates run on the tensor pipe (measurement)
  *   LBCNN_OPT_INNER_TC           1: the 64-column steps inside a panel use the tensor-pipe update too (default 0: fp64 DMMA;
  *                                at K = 64 the update is bound by its read-modify-write traffic, measured slower)
@@ -113,7 +115,7 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
  *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
 enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5,
-       LBCNN_OPT_SCORER = 6 };
+       LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7 };
 enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
 int lbcnn_set_option(lbcnn_handle_t h, int option, int value);

@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 512; p->inner_tc = 0; p->deflate = 1; p->scorer = LBCNN_SCORER_AUTO;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->inner_tc = 0; p->deflate = 1; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -101,6 +101,9 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
     case LBCNN_OPT_SCORER:
       if (value != LBCNN_SCORER_AUTO && value != LBCNN_SCORER_FP64 && value != LBCNN_SCORER_TENSOR) return LBCNN_ERR_INVALID_ARG;
       h->scorer = value; return LBCNN_OK;
+    case LBCNN_OPT_MID_PANEL:
+      if (value != 0 && (value < 64 || value > LB_STC_KMAX || value % 64)) return LBCNN_ERR_INVALID_ARG;
+      h->mid_panel = value; return LBCNN_OK;
     case LBCNN_OPT_PANEL:
       if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
       h->panel = value; return LBCNN_OK;

@@ -341,6 +341,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   // wider (its read-modify-write traffic on the trailing matrix falls with 1/NBO).
   const bool tc_solve = pl.stc_kmax > 0 && (h->solver == LBCNN_SOLVER_MIXED || (h->solver == LBCNN_SOLVER_AUTO && dim >= LB_STC_AUTO_DIM));
   const int NBO = tc_solve ? h->panel : 256;
+  const int NBM = (tc_solve && h->mid_panel >= NB && h->mid_panel < NBO) ? h->mid_panel : NBO;      // mid level (fp64 steps inside)
   CholTcCtx tcx;
   if (tc_solve) {
     rc = lb_chol_tc_begin(h, base + pl.stc_off, rows, dim, n_cand, pl.stc_kmax, A, a_stride, ld, lb_ws_counter(h, 1), &tcx);
@@ -356,6 +357,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
       potrf_diag_kernel<<<n_cand, 256, potrf_smem, st>>>(A, a_stride, ld, (int)j0, nbj, d_info, Lj, linv_stride);
       h->launches += 1;
       const long long j1 = j0 + nbj;
+      const long long M0 = J0 + (j0 - J0) / NBM * NBM, M1 = (M0 + NBM < J1) ? M0 + NBM : J1;     // the mid block of this step
       if (rows - j1 > 0) {
         GemmP g{};                                                     // X = A21 * Linv^T, in place (one column tile)
         g.A = A + j1 * ld + j0; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
@@ -377,16 +379,23 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
           u.M = (int)(rows - j1); u.N = (int)(dim - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
           rc = launch_gemm<double, double, double, true, true>(h, u, n_cand, st);
           if (rc) return rc;
-        } else if (J1 - j1 > 0 && tc_solve && h->inner_tc) {           // rest of the panel on the tensor pipe (K = 64)
+        } else if (J1 - j1 > 0 && tc_solve && h->inner_tc) {           // rest of the panel on the tensor pipe (K = 64; measurement)
           rc = lb_chol_tc_update(h, tcx, (int)j1, (int)J1, (int)j0, nbj, st);
           if (rc) return rc;
-        } else if (J1 - j1 > 0) {                                      // rest of the panel: columns j1 .. J1-1
+        } else if (M1 - j1 > 0) {                                      // rest of the mid block: columns j1 .. M1-1 (fp64)
           GemmP u{};
           u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
           u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
           u.C = A + j1 * ld + j1; u.ldc = ld; u.bC = a_stride;
-          u.M = (int)(rows - j1); u.N = (int)(J1 - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
+          u.M = (int)(rows - j1); u.N = (int)(M1 - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
           rc = launch_gemm<double, double, double, true, true>(h, u, n_cand, st);
+          if (rc) return rc;
+        }
+        // a finished mid block updates the rest of its panel on the tensor pipe (K = NBM): the fp64 steps above then only
+        // ever touch NBM-wide strips, and the wide trailing matrix is read and written once per NBO columns
+        if (j1 == M1 && J1 - M1 > 0 && NBM < NBO && !(h->inner_tc)) {
+          const long long K0 = (h->deflate && M0 == 0) ? ((NB < M1) ? NB : M1) : M0;
+          rc = lb_chol_tc_update(h, tcx, (int)M1, (int)J1, (int)K0, (int)(M1 - K0), st);
           if (rc) return rc;
         }
       }

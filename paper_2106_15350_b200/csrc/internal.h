@@ -22,6 +22,7 @@ struct lbcnn_handle_s {
   int inner_tc;                     // ... and whether the 64-column steps inside a panel use them too
   int deflate;                      // ... with the first block column's update kept in fp64 (common-mode deflation)
   int scorer;                       // LBCNN_SCORER_* (lbcnn_set_option)
+  int mid_panel;                    // width of the fp64-stepped blocks inside a panel (three-level factorisation); 0 = two levels
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;

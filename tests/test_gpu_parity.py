@@ -219,13 +219,15 @@ def test_fit_tensor_core_solver(handle, n, F, c, panel, integer):
     try:
         handle.set_option(lb.OPT_SOLVER, lb.SOLVER_MIXED)
         handle.set_option(lb.OPT_PANEL, panel)
+        handle.set_option(lb.OPT_MID_PANEL, {256: 128, 192: 64}.get(panel, 0))     # three levels on two of the cases
         W_tc, info_tc = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=flags)
         handle.set_option(lb.OPT_SOLVER, lb.SOLVER_FP64)
         W_64, info_64 = handle.elm_fit(Hd, yd, c, Creg, h_scale=s, flags=flags)
         torch.cuda.synchronize()
     finally:
         handle.set_option(lb.OPT_SOLVER, lb.SOLVER_AUTO)
-        handle.set_option(lb.OPT_PANEL, 512)
+        handle.set_option(lb.OPT_PANEL, 1024)
+        handle.set_option(lb.OPT_MID_PANEL, 256)
     assert (info_tc.cpu().numpy() == 0).all() and (info_64.cpu().numpy() == 0).all()
     sc = float(np.float32(s))
     for k in range(K):
