@@ -273,7 +273,7 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
         h.set_option(opt, val)
     stage = lb.host_staging_bytes(arch, w.n_train, w.n_test, w.n_classes, K)
     budget = int(ws_gb * (1 << 30))
-    ws_bytes, ws_min = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, budget)
+    ws_bytes, ws_min = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, budget, handle=h)
     h.ensure_workspace(ws_bytes + stage)
     l2_note = "inputs exceed L2: workspace %.2f GB of features/Gram streams through the 126 MB L2 every step" % (ws_bytes / 1e9)
     if ws_bytes < 2 * 126e6:
@@ -407,6 +407,8 @@ def run_cuda(args):
         OPTIONS.append((lb.OPT_INNER_TC, args.inner_tc))
     if args.mid_panel >= 0:
         OPTIONS.append((lb.OPT_MID_PANEL, args.mid_panel))
+    if args.stream_rows > 0:
+        OPTIONS.append((lb.OPT_STREAM_ROWS, args.stream_rows))
     if args.scorer:
         OPTIONS.append((lb.OPT_SCORER, {"auto": lb.SCORER_AUTO, "fp64": lb.SCORER_FP64, "tensor": lb.SCORER_TENSOR}[args.scorer]))
 
@@ -479,6 +481,7 @@ def main():
     ap.add_argument("--panel", type=int, default=0, help="LBCNN_OPT_PANEL (measurement)")
     ap.add_argument("--inner-tc", type=int, default=-1, help="LBCNN_OPT_INNER_TC (measurement)")
     ap.add_argument("--mid-panel", type=int, default=-1, help="LBCNN_OPT_MID_PANEL (measurement)")
+    ap.add_argument("--stream-rows", type=int, default=0, help="LBCNN_OPT_STREAM_ROWS: streamed search, samples per chunk")
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
     ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")

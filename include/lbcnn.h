@@ -101,6 +101,11 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                a trailing update; the matrix, the diagonal blocks and the panel solves stay fp64
  *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
  *                                captured CUDA graph (default 1)
+ *   LBCNN_OPT_STREAM_ROWS        r > 0: streamed search ("limited GPU-RAM ... reduced fraction of the training
+ *                                set"): the driver expands at most r samples at a time; the exact integer Gram and right-hand side
+ *                                of the chunks add up (bit-identical to the unstreamed result), the test set is scored chunk by
+ *                                chunk, so the features of the whole set never exist and the workspace no longer grows with
+ *                                N_train / N_test.  Takes effect on the primal branch with the exact tensor-core Gram; 0 = off
  *   LBCNN_OPT_MID_PANEL          width (multiple of 64; default 256; 0 = none) of the blocks inside a panel whose 64-column steps
  *                                run in fp64; a finished block updates the rest of its panel on the tensor pipe
  *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 1024) of the blocked Cholesky when its trailing
@@ -115,7 +120,7 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
  *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
 enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5,
-       LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7 };
+       LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7, LBCNN_OPT_STREAM_ROWS = 8 };
 enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
 int lbcnn_set_option(lbcnn_handle_t h, int option, int value);

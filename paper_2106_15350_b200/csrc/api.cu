@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->inner_tc = 0; p->deflate = 1; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->inner_tc = 0; p->deflate = 1; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -104,6 +104,9 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
     case LBCNN_OPT_MID_PANEL:
       if (value != 0 && (value < 64 || value > LB_STC_KMAX || value % 64)) return LBCNN_ERR_INVALID_ARG;
       h->mid_panel = value; return LBCNN_OK;
+    case LBCNN_OPT_STREAM_ROWS:
+      if (value < 0) return LBCNN_ERR_INVALID_ARG;
+      h->stream_rows = value; return LBCNN_OK;
     case LBCNN_OPT_PANEL:
       if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
       h->panel = value; return LBCNN_OK;
@@ -194,10 +197,19 @@ namespace {
 struct SearchPlan {
   FitPlan fit;
   size_t xw_off, fit_off, htr_off, hte_off, w_off, sc_off, total;
+  int stream; int64_t ntr_ws, nte_ws;      // streamed: rows of the train / test features resident at once
 };
 // xw1 = expander scratch per candidate (lb_expand_ws_bytes(.., 1)); kc = candidates per chunk
-void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, SearchPlan* p) {
+// sr: streamed search (LBCNN_OPT_STREAM_ROWS) -- at most sr samples of the train / test set are resident at once
+void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, int64_t sr,
+                 SearchPlan* p) {
   lb_fit_plan(n_train, F, c, kc, flags, &p->fit);
+  p->stream = (sr > 0 && (sr < n_train || sr < n_test) && p->fit.primal && p->fit.use_tc && p->fit.fuse_rhs) ? 1 : 0;
+  if (p->stream) {
+    if (sr < n_train) { lb_fit_plan(n_train, F, c, kc, flags, &p->fit, sr); n_train = sr; }
+    if (sr < n_test) n_test = sr;
+  }
+  p->ntr_ws = n_train; p->nte_ws = n_test;
   size_t off = 0;
   p->xw_off = off;  off += (size_t)lb_align_up((int64_t)(xw1 * (size_t)kc), 256);
   p->fit_off = off; off += p->fit.total;
@@ -215,14 +227,14 @@ uint32_t search_fit_flags(const ArchShape& s, bool has_bias) {
   return (!has_bias && s.max_abs <= LB_H_INTEGER_MAX) ? LBCNN_H_INTEGER : 0u;
 }
 // largest chunk size whose plan fits in `bytes` (0 if none)
-int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, size_t bytes) {
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, int64_t sr, size_t bytes) {
   SearchPlan p;
-  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, &p);
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, sr, &p);
   if (p.total <= bytes) return n_cand;
   int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
   while (hi - lo > 1) {
     const int mid = lo + (hi - lo) / 2;
-    plan_search(F, n_train, n_test, c, n_cand, mid, flags, xw1, &p);
+    plan_search(F, n_train, n_test, c, n_cand, mid, flags, xw1, sr, &p);
     if (p.total <= bytes) lo = mid; else hi = mid;
   }
   return lo;
@@ -245,16 +257,17 @@ int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_
   if (rc) return rc;
   const uint32_t flags = search_fit_flags(s, false);     // the bias-free plan is the larger one (digit planes)
   const size_t xw1 = expand_ws_per_cand(h, s, false);
+  const int64_t sr = h ? h->stream_rows : 0;
   SearchPlan p1;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, &p1);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, sr, &p1);
   if (min_bytes) *min_bytes = p1.total;
   int kc = n_cand;
   if (budget_bytes) {
-    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0);
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, sr, budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0);
     if (kc < 1) kc = 1;
   }
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, &p);
   if (min_bytes) *min_bytes += LB_WS_HEAD;
   *bytes = p.total + LB_WS_HEAD;
   return LBCNN_OK;
@@ -349,11 +362,12 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   if (!ws) return LBCNN_ERR_WORKSPACE;
   const uint32_t fflags = search_fit_flags(s, d_bias != nullptr);
   const size_t xw1 = lb_expand_ws_bytes(h, s, d_bias != nullptr, 1);
-  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, ws_bytes);
+  const int64_t sr = h->stream_rows;
+  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, sr, ws_bytes);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
   if (kc > 65535) kc = 65535;                          // grid.y / grid.z of the batched kernels
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, sr, &p);
   char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
@@ -361,28 +375,47 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   cudaStream_t st = (cudaStream_t)stream;
   const float hs = arch->feature_scale;
   const int64_t wel = s.F * n_classes;
+  const int64_t px = (int64_t)s.L[0].hin * s.L[0].win * s.L[0].cin;      // bytes of one image
   for (int k0 = 0; k0 < n_cand; k0 += kc) {
     const int kn = (n_cand - k0 < kc) ? n_cand - k0 : kc;
     const int8_t* ker = d_kernels + (int64_t)k0 * s.n_weights;
     const int32_t* bias = d_bias ? d_bias + (int64_t)k0 * s.n_bias : nullptr;
-    // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale
-    rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st);
-    if (rc) return rc;
-    rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Hte, base + p.xw_off, xw1 * (size_t)kn, st, true);
-    if (rc) return rc;
+    float* Wk = Wall + (int64_t)k0 * wel;
+    const bool tc_score = (fflags & LBCNN_H_INTEGER) && h->scorer != LBCNN_SCORER_FP64 &&
+                          lb_score_tc_usable(Hte, p.nte_ws, s.F, n_classes, kn) &&
+                          (h->scorer == LBCNN_SCORER_TENSOR || lb_score_tc_worthwhile(n_test, s.F, n_classes, kn));
     FitPlan fp;
-    lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp);
-    rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn,
-                       Wall + (int64_t)k0 * wel, d_info + k0, st);
-    if (rc) return rc;
-    if ((fflags & LBCNN_H_INTEGER) && h->scorer != LBCNN_SCORER_FP64 && lb_score_tc_usable(Hte, n_test, s.F, n_classes, kn) &&
-        (h->scorer == LBCNN_SCORER_TENSOR || lb_score_tc_worthwhile(n_test, s.F, n_classes, kn)))
-      rc = lb_launch_score_tc(h, base + p.sc_off, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn,
-                              nullptr, d_correct + k0, st);
-    else
-      rc = lb_launch_score(h, Hte, n_test, s.F, hs, Wall + (int64_t)k0 * wel, n_classes, d_test_labels, kn, nullptr,
-                           d_correct + k0, st);
-    if (rc) return rc;
+    lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, p.ntr_ws);
+    // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale.
+    // Streamed ("limited GPU-RAM"): the train set passes through in chunks of
+    // ntr_ws samples whose exact integer Grams (and fused right-hand sides) add up in A -- H of the whole set never exists.
+    for (int64_t r0 = 0; r0 < n_train; r0 += p.ntr_ws) {
+      const int64_t nr = (n_train - r0 < p.ntr_ws) ? n_train - r0 : p.ntr_ws;
+      rc = lb_launch_expand(h, s, 1.0f, d_train + r0 * px, nr, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st, r0 > 0);
+      if (rc) return rc;
+      if (p.stream) {
+        const FitStream fs{1, r0 == 0 ? 1 : 0, r0 + nr >= n_train ? 1 : 0};
+        rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, nr, s.F, hs, d_train_labels + r0, n_classes, C, kn, Wk, d_info + k0, st, &fs);
+        if (rc) return rc;
+      }
+    }
+    {
+      const FitStream fs{2, 0, 0};
+      rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn, Wk, d_info + k0, st,
+                         p.stream ? &fs : nullptr);
+      if (rc) return rc;
+    }
+    for (int64_t r0 = 0; r0 < n_test; r0 += p.nte_ws) {
+      const int64_t nr = (n_test - r0 < p.nte_ws) ? n_test - r0 : p.nte_ws;
+      rc = lb_launch_expand(h, s, 1.0f, d_test + r0 * px, nr, ker, bias, kn, Hte, base + p.xw_off, xw1 * (size_t)kn, st, true);
+      if (rc) return rc;
+      if (tc_score)
+        rc = lb_launch_score_tc(h, base + p.sc_off, Hte, nr, s.F, hs, Wk, n_classes, d_test_labels + r0, kn, nullptr, d_correct + k0, st,
+                                r0 > 0);
+      else
+        rc = lb_launch_score(h, Hte, nr, s.F, hs, Wk, n_classes, d_test_labels + r0, kn, nullptr, d_correct + k0, st, r0 > 0);
+      if (rc) return rc;
+    }
   }
   return lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, Wall, wel, d_W_best, st);
 }

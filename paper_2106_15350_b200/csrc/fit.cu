@@ -237,7 +237,8 @@ __global__ void w_from_xt_kernel(const double* __restrict__ A, long long a_strid
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
-void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p) {
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws) {
+  if (n_ws <= 0 || n_ws > n) n_ws = n;
   int primal = (F < n) ? 1 : 0;                       // PAPER.md:68 `if n_inputs<Ntr` ('LLL'), else 'MMM'
   if (flags & LBCNN_FORCE_PRIMAL) primal = 1;
   if (flags & LBCNN_FORCE_DUAL) primal = 0;
@@ -251,7 +252,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
   p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
   p->tc_off = off;   p->fuse_rhs = (p->use_tc && primal && lb_gram_tc_fuse_rhs(F, n_classes)) ? 1 : 0;
-  if (p->use_tc) off += lb_gram_tc_ws_bytes(n, F, n_cand, p->fuse_rhs ? n_classes : 0);
+  if (p->use_tc) off += lb_gram_tc_ws_bytes(n_ws, F, n_cand, p->fuse_rhs ? n_classes : 0);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   // digit planes + row scales of the tensor-core trailing updates (chol_tc.cu), for systems large enough to have them
   p->stc_kmax = (p->dim >= LB_STC_MIN_DIM) ? LB_STC_KMAX : 0;
@@ -262,7 +263,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
 
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d_H, int64_t n, int64_t F, float h_scale,
                   const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
-                  cudaStream_t st) {
+                  cudaStream_t st, const FitStream* fs) {
   char* base = reinterpret_cast<char*>(ws);
   int32_t* perm = reinterpret_cast<int32_t*>(base + pl.perm_off);
   int32_t* off = reinterpret_cast<int32_t*>(base + pl.off_off);
@@ -278,8 +279,18 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     rc = lb_launch_zero_i32(h, d_info, n_cand, st);
     if (rc) return rc;
   }
+  if (fs) {                         // streamed: only the exact tensor-core Gram with the fused right-hand side accumulates
+    if (!(pl.primal && pl.use_tc && pl.fuse_rhs)) return LBCNN_ERR_INVALID_ARG;
+    if (fs->stage == 1) {
+      LbPhase ph(h, LBCNN_PHASE_GRAM, st);
+      return lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, true, d_labels, c, d_info, st,
+                               fs->first_chunk == 0, fs->last_chunk != 0);
+    }
+  }
 
-  if (pl.primal) {
+  if (fs && fs->stage == 2) {
+    // the Gram and the right-hand side are complete in A
+  } else if (pl.primal) {
     // F1: A = U^T U + lam I (lower tiles), operands read with k = sample (slow) and i = feature (contiguous)
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);

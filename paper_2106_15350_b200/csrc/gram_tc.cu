@@ -44,6 +44,8 @@ struct GramTcParams {
   int dual;            // 0: A = U^T U (operands MN-major: the feature index is contiguous); 1: A = U U^T (K-major)
   double lam;
   unsigned long long* ops;   // int8 multiply-adds issued (measurement)
+  int accumulate;            // A += G (a further chunk of samples of a streamed Gram) instead of A = G
+  int add_lam;               // ... + lam I (the last chunk: (G1 + G2 + ..) + lam rounds like the unstreamed G + lam)
 };
 
 // ---- digit split ----------------------------------------------------------------------------------
@@ -365,7 +367,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
             for (int s = 4; s >= 0; --s)
               if (s < nacc) g = g * 256 + (long long)(int32_t)r[s][e];
             double v = (double)g;
-            if (i == j) v += p.lam;
+            if (p.accumulate) v += Arow[j];          // integers below 2^53: the chunked sum is as exact as the whole one
+            if (p.add_lam && i == j) v += p.lam;
             Arow[j] = v;
           }
         }
@@ -422,7 +425,7 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {
 // (U^T T)^T, T the one-hot coding of the labels (the appended right-hand-side rows of the Cholesky layout).
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
                       long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
-                      cudaStream_t st) {
+                      cudaStream_t st, bool accumulate, bool add_lam) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   const int c_aug = (primal && d_labels && lb_gram_tc_fuse_rhs(F, n_classes)) ? n_classes : 0;
@@ -434,7 +437,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   const int n_counts = n_cand * (1 + G32);
   // one launch: digit counts = 1 and the candidates' info = 0 (the fit's own zeroing is skipped on this path)
   const int nfill = n_counts > n_cand ? n_counts : n_cand;
-  fill_i32_kernel<<<(nfill + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1, d_info, n_cand);
+  fill_i32_kernel<<<(nfill + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1, accumulate ? nullptr : d_info, n_cand);
   h->launches += 1;
   {
     const long long work = n * (Fp / 8);
@@ -463,7 +466,7 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   GramTcParams p{};
   p.nlimb = nlimb; p.nl32 = nl32; p.G32 = G32; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
   const int64_t odim = primal ? F + c_aug : n, ocols = primal ? F : n;
-  p.Fcols = (int)ocols; p.ops = lb_ws_counter(h, 0);
+  p.Fcols = (int)ocols; p.ops = lb_ws_counter(h, 0); p.accumulate = accumulate ? 1 : 0; p.add_lam = add_lam ? 1 : 0;
   p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
   const size_t smem = (size_t)RING_BYTES + 1024;
   LB_CUDA_OK(cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -23,6 +23,7 @@ struct lbcnn_handle_s {
   int deflate;                      // ... with the first block column's update kept in fp64 (common-mode deflation)
   int scorer;                       // LBCNN_SCORER_* (lbcnn_set_option)
   int mid_panel;                    // width of the fp64-stepped blocks inside a panel (three-level factorisation); 0 = two levels
+  int64_t stream_rows;              // search driver: samples expanded / accumulated per chunk (0 = all at once)
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
@@ -99,10 +100,13 @@ struct FitPlan {
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
   int fuse_rhs;          // ... which then also produces the right-hand side (one-hot label columns)
 };
-void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p);
+// n_ws: rows of H resident at once (streamed Gram: the digit planes are sized for one chunk of samples); 0 = n
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws = 0);
+// streamed fit: stage 1 = add one chunk of samples to the Gram (+ fused right-hand side), stage 2 = solve
+struct FitStream { int stage; int first_chunk; int last_chunk; };
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_H, int64_t n, int64_t F, float h_scale,
                   const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
-                  cudaStream_t st);
+                  cudaStream_t st, const FitStream* fs = nullptr);
 
 // ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
 bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
@@ -110,7 +114,7 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug);
 bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-hot columns of the Gram's digit plane 0
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
                       long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
-                      cudaStream_t st);
+                      cudaStream_t st, bool accumulate = false, bool add_lam = true);   // streamed: A += this chunk's Gram; ridge with the last chunk
 
 constexpr int LB_STC_KMAX = 1024;      // widest panel (digit-plane pitch)
 constexpr int LB_STC_MIN_DIM = 512;    // systems below this never reserve the scratch
@@ -129,16 +133,17 @@ int lb_chol_tc_begin(lbcnn_handle_s* h, void* ws, int64_t rows, int64_t dim, int
 int lb_chol_tc_update(lbcnn_handle_s* h, const CholTcCtx& ctx, int r0, int c1, int k0, int K, cudaStream_t st);
 
 // ---- score (score.cu) ----------------------------------------------------------------------
+// keep_correct: add to d_correct instead of starting from zero (streamed scoring of test-set chunks)
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                     int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
-                    cudaStream_t st);
+                    cudaStream_t st, bool keep_correct = false);
 // tensor-core scorer (score_tc.cu): integer-valued features, up to 128 classes; scratch from the caller's workspace
 bool lb_score_tc_usable(const float* d_H, int64_t n, int64_t F, int n_classes, int n_cand);
 bool lb_score_tc_worthwhile(int64_t n, int64_t F, int n_classes, int n_cand);
 size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand);
 int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                        int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
-                       cudaStream_t st);
+                       cudaStream_t st, bool keep_correct = false);
 int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,

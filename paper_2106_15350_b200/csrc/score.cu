@@ -157,9 +157,9 @@ __global__ void finish_kernel(const int32_t* __restrict__ correct, const int32_t
 
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                     int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
-                    cudaStream_t st) {
+                    cudaStream_t st, bool keep_correct) {
   LbPhase ph(h, LBCNN_PHASE_SCORE, st);
-  if (d_correct) {
+  if (d_correct && !keep_correct) {
     int rc = lb_launch_zero_i32(h, d_correct, n_cand, st);
     if (rc) return rc;
   }

@@ -425,7 +425,7 @@ size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand) {
 
 int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                        int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
-                       cudaStream_t st) {
+                       cudaStream_t st, bool keep_correct) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   LbPhase ph(h, LBCNN_PHASE_SCORE, st);
@@ -440,7 +440,7 @@ int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n,
   const int N = L.N, c = n_classes;
   const int Fp = (int)L.Fp;
   LB_CUDA_OK(cudaMemsetAsync(base + L.zero0, 0, L.zero_bytes, st));
-  if (d_correct) LB_CUDA_OK(cudaMemsetAsync(d_correct, 0, (size_t)n_cand * 4, st));
+  if (d_correct && !keep_correct) LB_CUDA_OK(cudaMemsetAsync(d_correct, 0, (size_t)n_cand * 4, st));
   {
     dim3 grid((unsigned)(Fp / PF), (unsigned)n_cand);
     score_wmax_kernel<<<grid, 256, 0, st>>>(d_W, (int)F, c, N, wmax);

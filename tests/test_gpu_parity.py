@@ -464,6 +464,38 @@ def test_search_is_deterministic_run_to_run(handle):
                 assert torch.equal(first[k], again[k]), k
 
 
+@pytest.mark.parametrize("name,ntr,nte,K,rows", [("mnist", 1500, 700, 5, 400), ("gtsrb", 2600, 500, 3, 1000),
+                                                  ("tiny_mnist", 2000, 500, 8, 300), ("vggface", 8300, 300, 2, 4096)])
+def test_streamed_search_equals_resident(handle, name, ntr, nte, K, rows):
+    """LBCNN_OPT_STREAM_ROWS ("limited GPU-RAM"): the train set passes through
+    the expander in chunks whose exact integer Grams and right-hand sides add up, the test set is scored chunk by chunk;
+    H of the whole set never exists.  Everything is exact integer arithmetic below 2^53, so the result must be
+    BIT-IDENTICAL to the resident search -- and the workspace must be smaller (ragged last chunks on purpose)."""
+    w = _small(name, ntr, nte, K)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    args = (arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    full = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, handle=handle)[0]
+    handle.set_workspace(None)
+    handle.ensure_workspace(full)
+    a = {k: v.clone() for k, v in handle.search_candidates(*args).items()}
+    try:
+        handle.set_option(lb.OPT_STREAM_ROWS, rows)
+        small = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, handle=handle)[0]
+        assert small < full
+        handle.set_workspace(None)
+        handle.ensure_workspace(small)
+        b = handle.search_candidates(*args)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_option(lb.OPT_STREAM_ROWS, 0)
+    for k in a:
+        assert torch.equal(a[k], b[k]), k
+    assert (b["info"].cpu().numpy() == 0).all()
+    handle.set_workspace(None)
+
+
 def test_search_chunked_equals_unchunked(handle):
     w = _small("mnist", 400, 150, 7)
     arch = lb.arch_of(w)
