@@ -216,6 +216,22 @@ int lbcnn_search_candidates_host(lbcnn_handle_t h, const lbcnn_arch_t* arch,
                                  float* h_acc /*[n_cand]*/, int32_t* h_correct /*[n_cand]*/, int32_t* h_info /*[n_cand]*/,
                                  int32_t* h_best /*[2]*/, float* h_W_best /*[F][n_classes] or NULL*/, void* stream);
 
+/* <= 8-bit fixed-point output layer ("weights represented as 8 bits integers"; Cell 12, PAPER.md:94, 98;
+ * the scheme is not stated -- reading DESIGN.md R16): per candidate ONE symmetric scale,
+ *   q[f][c] = clip(rint(W[f][c] * (qmax / max|W|)), -qmax, qmax),  qmax = 2^(bits-1) - 1,  2 <= bits <= 8,
+ * the product taken in fp64 and rounded half to even; d_scale[k] = max|W_k| / qmax (so W ~ d_scale[k] * q).  No workspace. */
+int lbcnn_quantize_output_layer(lbcnn_handle_t h, const float* d_W /*[n_cand][F][n_classes]*/, int64_t F, int32_t n_classes,
+                                int32_t n_cand, int32_t bits, int8_t* d_Wq /*[n_cand][F][n_classes]*/,
+                                float* d_scale /*[n_cand]*/, void* stream);
+/* Score with the quantised layer: pred = argmax_c sum_f H[n][f] * q[f][c] (first index on ties); the common positive scale
+ * cannot change the argmax.  For integer-valued H (the expander's output with feature_scale = 1) the logits are EXACT
+ * integers (int8 digit products on the tensor pipe, int64 recombination); a row holding a non-integer or out-of-range
+ * value, and exact ties, are evaluated in fp64.  Needs lbcnn_score_workspace_bytes of workspace; n_classes <= 128,
+ * F a multiple of 4 and <= 43690, d_H 16-byte aligned (else LBCNN_ERR_SHAPE). */
+int lbcnn_elm_score_q(lbcnn_handle_t h, const float* d_H /*[n_cand][n][F]*/, int64_t n, int64_t F,
+                      const int8_t* d_Wq /*[n_cand][F][n_classes]*/, int32_t n_classes, const int32_t* d_labels /*[n] or NULL*/,
+                      int32_t n_cand, int32_t* d_pred /*[n_cand][n] or NULL*/, int32_t* d_correct /*[n_cand] or NULL*/, void* stream);
+
 /* Workspace lbcnn_elm_score needs under LBCNN_SCORER_TENSOR (host-only arithmetic; 0 is never returned). */
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes);
 

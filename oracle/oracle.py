@@ -206,3 +206,33 @@ def search(arch: _Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: 
     if keep:
         out["W"], out["pred"] = Ws, preds
     return out
+
+
+# ---- <= 8-bit fixed-point output layer ------------------------------------------------------------------
+def quantize_output_layer(W: np.ndarray, bits: int = 8):
+    """"weights represented as 8 bits integers" (Cell 12 "quantization with fixed-point ... maximum 8 bits",
+    PAPER.md:94, 98).  The paper does not state the scheme; reading DESIGN.md R16: ONE symmetric scale per output layer,
+        q = clip(rint(W * (qmax / max|W|)), -qmax, qmax),   qmax = 2^(bits-1) - 1,
+    W taken as the fp32 numbers the fit returned, the product formed in fp64, rint = round half to even.
+    Returns (q int8 [F][classes], scale float32 = max|W| / qmax), so that W ~ scale * q."""
+    if not 2 <= bits <= 8:
+        raise ValueError("bits must be 2..8")
+    W32 = np.ascontiguousarray(W, dtype=np.float32)
+    qmax = 2 ** (bits - 1) - 1
+    m = float(np.max(np.abs(W32)))
+    sf = (float(qmax) / m) if m > 0.0 else 0.0
+    q = np.rint(W32.astype(np.float64) * sf)
+    q = np.clip(q, -qmax, qmax).astype(np.int8)
+    return q, np.float32(m / float(qmax))
+
+
+def elm_score_q(U: np.ndarray, q: np.ndarray, labels: Optional[np.ndarray] = None):
+    """Predict with the quantised layer on the INTEGER features U [n][F]: logits = U q in exact integer
+    arithmetic, class = first index of the maximum (R12); the common positive scale cannot change the argmax.
+    Returns (pred int32 [n], correct or None, logits int64 [n][classes])."""
+    U = np.ascontiguousarray(U, dtype=np.int64)
+    q = np.ascontiguousarray(q, dtype=np.int64)
+    logits = U @ q
+    pred = np.argmax(logits, axis=1).astype(np.int32)          # numpy returns the first maximum
+    corr = None if labels is None else int((pred == np.asarray(labels)).sum())
+    return pred, corr, logits

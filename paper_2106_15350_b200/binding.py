@@ -26,7 +26,8 @@ EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destro
            "lbcnn_kernel_set_size", "lbcnn_workspace_bytes", "lbcnn_set_workspace", "lbcnn_expand", "lbcnn_elm_fit",
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
-           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes")
+           "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes",
+           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -282,6 +283,29 @@ class Handle:
         _check(lib().lbcnn_elm_score(self._h, _ptr(H, torch.float32), C.c_int64(n), C.c_int64(F), C.c_float(h_scale),
                                      _ptr(W, torch.float32), C.c_int32(c), _ptr(labels, torch.int32, True), C.c_int32(K),
                                      _ptr(pred, None, True), _ptr(corr, None, True), _stream()), "lbcnn_elm_score")
+        return pred, corr
+
+    def quantize_output_layer(self, W, bits: int = 8):
+        """W f32 [K][F][c] -> (Wq i8 [K][F][c], scale f32 [K]); W ~ scale * Wq (include/lbcnn.h)."""
+        import torch
+        K, F, c = W.shape
+        Wq = torch.empty((K, F, c), dtype=torch.int8, device=W.device)
+        scale = torch.empty((K,), dtype=torch.float32, device=W.device)
+        _check(lib().lbcnn_quantize_output_layer(self._h, _ptr(W, torch.float32), C.c_int64(F), C.c_int32(c), C.c_int32(K),
+                                                 C.c_int32(bits), _ptr(Wq), _ptr(scale), _stream()), "lbcnn_quantize_output_layer")
+        return Wq, scale
+
+    def elm_score_q(self, H, Wq, labels=None, want_pred: bool = True):
+        """returns (pred i32 [K][n] or None, correct i32 [K] or None) with the int8 output layer."""
+        import torch
+        K, n, F = H.shape
+        c = Wq.shape[2]
+        self.ensure_workspace(score_workspace_bytes(n, F, c, K))
+        pred = torch.empty((K, n), dtype=torch.int32, device=H.device) if want_pred else None
+        corr = torch.empty((K,), dtype=torch.int32, device=H.device) if labels is not None else None
+        _check(lib().lbcnn_elm_score_q(self._h, _ptr(H, torch.float32), C.c_int64(n), C.c_int64(F), _ptr(Wq, torch.int8),
+                                       C.c_int32(c), _ptr(labels, torch.int32, True), C.c_int32(K), _ptr(pred, None, True),
+                                       _ptr(corr, None, True), _stream()), "lbcnn_elm_score_q")
         return pred, corr
 
     def search_candidates(self, arch: Arch, train_x, train_y, test_x, test_y, n_classes: int, Creg: float, kernels,

@@ -336,6 +336,22 @@ int lbcnn_elm_score(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, fl
   return lb_launch_score(h, d_H, n, F, h_scale, d_W, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
 }
 
+int lbcnn_quantize_output_layer(lbcnn_handle_t h, const float* d_W, int64_t F, int32_t n_classes, int32_t n_cand, int32_t bits,
+                                int8_t* d_Wq, float* d_scale, void* stream) {
+  if (!h || !d_W || !d_Wq || !d_scale || F < 1 || n_classes < 2 || n_cand < 1 || n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
+  if (bits < 2 || bits > 8) return LBCNN_ERR_INVALID_ARG;
+  return lb_launch_quantize_w(h, d_W, F, n_classes, n_cand, bits, d_Wq, d_scale, (cudaStream_t)stream);
+}
+
+int lbcnn_elm_score_q(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, const int8_t* d_Wq, int32_t n_classes,
+                      const int32_t* d_labels, int32_t n_cand, int32_t* d_pred, int32_t* d_correct, void* stream) {
+  if (!h || !d_H || !d_Wq || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
+  if (d_correct && !d_labels) return LBCNN_ERR_INVALID_ARG;
+  if (!lb_score_tc_usable(d_H, n, F, n_classes, n_cand)) return LBCNN_ERR_SHAPE;
+  if (!h->ws || lb_ws_avail(h) < lb_score_tc_ws_bytes(n, F, n_classes, n_cand)) return LBCNN_ERR_WORKSPACE;
+  return lb_launch_score_q8(h, lb_ws_base(h), d_H, n, F, d_Wq, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
+}
+
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes) {
   if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   *bytes = lb_score_tc_ws_bytes(n, F, n_classes, n_cand) + LB_WS_HEAD;

@@ -144,6 +144,11 @@ size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand);
 int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                        int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
                        cudaStream_t st, bool keep_correct = false);
+// <= 8-bit output layer (score_tc.cu): per-candidate symmetric quantisation of W, and S1 with exact integer logits
+int lb_launch_quantize_w(lbcnn_handle_s* h, const float* d_W, int64_t F, int n_classes, int n_cand, int bits, int8_t* d_Wq,
+                         float* d_scale, cudaStream_t st);
+int lb_launch_score_q8(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, const int8_t* d_Wq, int n_classes,
+                       const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct, cudaStream_t st);
 int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,

@@ -128,11 +128,40 @@ __global__ void __launch_bounds__(256) score_quant_kernel(const float* __restric
   }
 }
 
+// int8 output layer q[F][c] -> the single digit plane Wd[cand][N][Fp] (class-major), cscale = 1
+__global__ void __launch_bounds__(256) score_q8_prep_kernel(const int8_t* __restrict__ Wq, int F, int c, int N, int Fp,
+                                                            int8_t* __restrict__ Wd, double* __restrict__ cscale) {
+  extern __shared__ int8_t sq8[];                             // [PF][c + 1]
+  const int z = blockIdx.y, f0 = blockIdx.x * PF, t = threadIdx.x;
+  const int8_t* Wz = Wq + (long long)z * F * c + (long long)f0 * c;
+  const int rows = min(PF, F - f0), pitch = c + 1;
+  for (int e = t; e < PF * c; e += 256) {
+    const int r = e / c, cls = e - r * c;
+    sq8[r * pitch + cls] = (r < rows) ? Wz[e] : (int8_t)0;
+  }
+  if (blockIdx.x == 0)
+    for (int cls = t; cls < N; cls += 256) cscale[(long long)z * N + cls] = 1.0;
+  __syncthreads();
+  for (int e = t; e < N * (PF / 4); e += 256) {
+    const int cls = e / (PF / 4), g = (e - cls * (PF / 4)) * 4;
+    uint32_t w = 0u;
+    if (cls < c) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) w |= (uint32_t)(uint8_t)sq8[(g + q) * pitch + cls] << (8 * q);
+    }
+    *reinterpret_cast<uint32_t*>(Wd + ((long long)z * N + cls) * Fp + f0 + g) = w;
+  }
+}
+
 // ---- the scoring kernel -----------------------------------------------------------------------------------------------
 constexpr int MAXSTAGE = 4;
 
+// NW digit planes of W, diagonals SMIN .. NDU + NW - 2 issued: <4, 2> = fp32 W as four column-scaled digits (nine of the
+// twelve products, error-bounded); <1, 0> = an int8 output layer (lbcnn_elm_score_q): all three products, EXACT integer logits
+template <int NW, int SMIN>
 __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_constant__ CUtensorMap tmapU,
                                                                const __grid_constant__ CUtensorMap tmapW, const ScoreTcParams p) {
+  constexpr int NACC = NDU + NW - 1 - SMIN;      // accumulators (diagonals kept)
   const int z = blockIdx.y;
   const int i0 = blockIdx.x * TM;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -166,7 +195,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
   if (warp == 0) {
     // ===== TMA producer =====
     int s = 0, ph = 0;
-    const uint32_t tx = (uint32_t)(UF32_BYTES + NDW * w_tile);
+    const uint32_t tx = (uint32_t)(UF32_BYTES + NW * w_tile);
     for (int it = 0; it < p.n_iters; ++it) {
       tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ph ^ 1);
       if (tc::elect_one()) {
@@ -175,13 +204,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
         const uint32_t base = smem0 + s * stage_bytes;
         tc::tma_load_3d(base, &tmapU, full, it * KC, i0, z);
 #pragma unroll
-        for (int b = 0; b < NDW; ++b) tc::tma_load_3d(base + off_w + b * w_tile, &tmapW, full, it * KC, 0, z * NDW + b);
+        for (int b = 0; b < NW; ++b) tc::tma_load_3d(base + off_w + b * w_tile, &tmapW, full, it * KC, 0, z * NW + b);
       }
       __syncwarp();
       if (++s == nstage) { s = 0; ph ^= 1; }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: diagonals s = a + b = 2..5 into accumulators 0..3 =====
+    // ===== MMA issuer: diagonals s = a + b = SMIN .. into accumulators 0 .. NACC-1 =====
     const uint32_t idesc = tc::idesc_i8(TM, N, 1, 1, 0, 0);
     const uint64_t d0 = tc::smem_desc(smem0, 16, 8 * KC, LAYOUT_SW64);
     int s = 0, ph = 0;
@@ -193,16 +222,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
 #pragma unroll
       for (int kk = 0; kk < KC / 32; ++kk) {
 #pragma unroll
-        for (int sd = 2; sd <= NDU + NDW - 2; ++sd) {
+        for (int sd = SMIN; sd <= NDU + NW - 2; ++sd) {
 #pragma unroll
           for (int a = 0; a < NDU; ++a) {
             const int b = sd - a;
-            if (b >= 0 && b < NDW) {
+            if (b >= 0 && b < NW) {
               const uint64_t da = ds + (uint64_t)((off_ud + a * UD_BYTES + kk * 32) >> 4);
               const uint64_t db = ds + (uint64_t)((off_w + b * w_tile + kk * 32) >> 4);
-              const int a_first = (sd - (NDW - 1)) > 0 ? sd - (NDW - 1) : 0;           // smallest a of this diagonal
+              const int a_first = (sd - (NW - 1)) > 0 ? sd - (NW - 1) : 0;             // smallest a of this diagonal
               const bool first = (kk == 0) && (a == a_first);
-              if (tc::elect_one()) tc::mma_i8(tmem + (sd - 2) * N, da, db, idesc, (first && it == 0) ? 0u : 1u);
+              if (tc::elect_one()) tc::mma_i8(tmem + (sd - SMIN) * N, da, db, idesc, (first && it == 0) ? 0u : 1u);
             }
           }
         }
@@ -274,9 +303,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
       double best = 0.0, second = 0.0, cs_max = 0.0;
       int bidx = -1, have2 = 0;
       for (int c0 = 0; c0 < N; c0 += 16) {
-        uint32_t acc[4][16];
+        uint32_t acc[NACC][16];
 #pragma unroll
-        for (int sd = 0; sd < 4; ++sd) tc::tmem_ld16(tmem + ((uint32_t)(q * 32) << 16) + sd * N + c0, acc[sd]);
+        for (int sd = 0; sd < NACC; ++sd) tc::tmem_ld16(tmem + ((uint32_t)(q * 32) << 16) + sd * N + c0, acc[sd]);
         tc::tmem_ld_wait();
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
@@ -284,7 +313,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
           if (j < p.c) {
             long long g = 0;
 #pragma unroll
-            for (int sd = 3; sd >= 0; --sd) g = g * 256 + (long long)(int32_t)acc[sd][e];
+            for (int sd = NACC - 1; sd >= 0; --sd) g = g * 256 + (long long)(int32_t)acc[sd][e];
             const double csj = cs[j];
             const double l = (double)g * csj;
             cs_max = fmax(cs_max, csj);
@@ -300,7 +329,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
         // what the issued diagonals leave out, in the units of l (= true logit / (65536 hs)): the dropped diagonals 0 and 1
         // (|d q| <= 128 |d|) and the rounding of w (half a unit of its last digit per feature)
         const double s0 = (double)row_s[r][0], s1 = (double)row_s[r][1], s2 = (double)row_s[r][2];
-        const double E = cs_max * ((128.0 * 257.0 * s0 + 32768.0 * s1) + 0.5 * (s0 + 256.0 * s1 + 65536.0 * s2)) * (1.0 / 65536.0);
+        const double E = (SMIN == 0) ? 0.0 :       // all diagonals and integer weights: the logits are exact, only ties go on
+            cs_max * ((128.0 * 257.0 * s0 + 32768.0 * s1) + 0.5 * (s0 + 256.0 * s1 + 65536.0 * s2)) * (1.0 / 65536.0);
         const bool exact = row_s[r][3] != 0 || !(best - second > 2.0 * E);
         if (exact) {
           const int slot = atomicAdd(p.flag_count, 1);
@@ -322,8 +352,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
 // One CTA per flagged row, the 128 threads split the FEATURES (thread t takes f = t, t + 128, ...: coalesced reads of the
 // row, eight classes at a time in registers), then a fixed-order tree over the threads: deterministic, every product
 // exact in fp64 (fp32 x fp32), only the order of the fp64 additions differs from the oracle's plain loop.
+template <typename TW>
 __global__ void __launch_bounds__(128) score_exact_kernel(const float* __restrict__ U, long long n, long long F,
-                                                          const float* __restrict__ W, int c, const int32_t* __restrict__ y,
+                                                          const TW* __restrict__ W, int c, const int32_t* __restrict__ y,
                                                           const int32_t* __restrict__ flag_count, const int32_t* __restrict__ flag_list,
                                                           int32_t* __restrict__ pred, int32_t* __restrict__ correct) {
   __shared__ double red[4][8];
@@ -332,7 +363,7 @@ __global__ void __launch_bounds__(128) score_exact_kernel(const float* __restric
     const long long e = flag_list[idx];
     const long long z = e / n, row = e - z * n;
     const float* Ur = U + (z * n + row) * F;
-    const float* Wz = W + z * F * c;
+    const TW* Wz = W + z * F * c;
     double bestv = 0.0; int besti = -1;
     for (int c0 = 0; c0 < c; c0 += 8) {
       double acc[8];
@@ -341,7 +372,7 @@ __global__ void __launch_bounds__(128) score_exact_kernel(const float* __restric
       const int nc = (c - c0 < 8) ? c - c0 : 8;
       for (long long f = t; f < F; f += 128) {
         const double u = (double)Ur[f];
-        const float* wr = Wz + f * c + c0;
+        const TW* wr = Wz + f * c + c0;
 #pragma unroll
         for (int q = 0; q < 8; ++q)
           if (q < nc) acc[q] = fma(u, (double)wr[q], acc[q]);
@@ -423,9 +454,11 @@ size_t lb_score_tc_ws_bytes(int64_t n, int64_t F, int n_classes, int n_cand) {
   return L.total;
 }
 
-int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
-                       int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
-                       cudaStream_t st, bool keep_correct) {
+namespace {
+// d_Wq != NULL: int8 output layer (one digit plane, exact integer logits); else fp32 d_W as four column-scaled digit planes
+int launch_score_common(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
+                        const int8_t* d_Wq, int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred,
+                        int32_t* d_correct, cudaStream_t st, bool keep_correct) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   LbPhase ph(h, LBCNN_PHASE_SCORE, st);
@@ -437,16 +470,21 @@ int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n,
   uint32_t* wmax = reinterpret_cast<uint32_t*>(base + L.wmax);
   int32_t* flag_count = reinterpret_cast<int32_t*>(base + L.flag_count);
   int32_t* flag_list = reinterpret_cast<int32_t*>(base + L.flag_list);
-  const int N = L.N, c = n_classes;
+  const int N = L.N, c = n_classes, NW = d_Wq ? 1 : NDW;
   const int Fp = (int)L.Fp;
   LB_CUDA_OK(cudaMemsetAsync(base + L.zero0, 0, L.zero_bytes, st));
   if (d_correct && !keep_correct) LB_CUDA_OK(cudaMemsetAsync(d_correct, 0, (size_t)n_cand * 4, st));
   {
     dim3 grid((unsigned)(Fp / PF), (unsigned)n_cand);
-    score_wmax_kernel<<<grid, 256, 0, st>>>(d_W, (int)F, c, N, wmax);
-    const size_t sm = (size_t)PF * (c + 1) * 4;
-    score_quant_kernel<<<grid, 256, sm, st>>>(d_W, (int)F, c, N, Fp, wmax, Wd, cscale);
-    h->launches += 2;
+    if (d_Wq) {
+      score_q8_prep_kernel<<<grid, 256, (size_t)PF * (c + 1), st>>>(d_Wq, (int)F, c, N, Fp, Wd, cscale);
+      h->launches += 1;
+    } else {
+      score_wmax_kernel<<<grid, 256, 0, st>>>(d_W, (int)F, c, N, wmax);
+      const size_t sm = (size_t)PF * (c + 1) * 4;
+      score_quant_kernel<<<grid, 256, sm, st>>>(d_W, (int)F, c, N, Fp, wmax, Wd, cscale);
+      h->launches += 2;
+    }
     LB_CUDA_OK(cudaGetLastError());
   }
   CUtensorMap tmapU, tmapW;
@@ -460,7 +498,7 @@ int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n,
       return LBCNN_ERR_CUDA;
   }
   {
-    const cuuint64_t gdim[3] = {(cuuint64_t)Fp, (cuuint64_t)N, (cuuint64_t)n_cand * NDW};
+    const cuuint64_t gdim[3] = {(cuuint64_t)Fp, (cuuint64_t)N, (cuuint64_t)n_cand * NW};
     const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)N * Fp};
     const cuuint32_t box[3] = {KC, (cuuint32_t)N, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
@@ -470,17 +508,85 @@ int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n,
   }
   ScoreTcParams p{};
   p.n = (int)n; p.F = (int)F; p.c = c; p.N = N; p.n_iters = Fp / KC; p.hs = (double)h_scale;
-  p.stage_bytes = UF32_BYTES + NDU * UD_BYTES + NDW * N * KC;
+  p.stage_bytes = UF32_BYTES + NDU * UD_BYTES + NW * N * KC;
   p.nstage = (int)((size_t)(h->max_smem_optin - 2048) / (size_t)p.stage_bytes);
   if (p.nstage > MAXSTAGE) p.nstage = MAXSTAGE;
   if (p.nstage < 2) return LBCNN_ERR_INVALID_ARG;
   p.cscale = cscale; p.y = d_labels; p.pred = d_pred; p.correct = d_correct; p.flag_count = flag_count; p.flag_list = flag_list;
   const size_t smem = (size_t)p.nstage * p.stage_bytes + 1024;
-  LB_CUDA_OK(cudaFuncSetAttribute(score_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   dim3 grid((unsigned)((n + TM - 1) / TM), (unsigned)n_cand);
-  score_tc_kernel<<<grid, NTHREADS, smem, st>>>(tmapU, tmapW, p);
-  score_exact_kernel<<<2 * h->n_sm, 128, 0, st>>>(d_H, n, F, d_W, c, d_labels, flag_count, flag_list, d_pred, d_correct);
+  if (d_Wq) {
+    LB_CUDA_OK(cudaFuncSetAttribute(score_tc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    score_tc_kernel<1, 0><<<grid, NTHREADS, smem, st>>>(tmapU, tmapW, p);
+    score_exact_kernel<int8_t><<<2 * h->n_sm, 128, 0, st>>>(d_H, n, F, d_Wq, c, d_labels, flag_count, flag_list, d_pred, d_correct);
+  } else {
+    LB_CUDA_OK(cudaFuncSetAttribute(score_tc_kernel<NDW, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    score_tc_kernel<NDW, 2><<<grid, NTHREADS, smem, st>>>(tmapU, tmapW, p);
+    score_exact_kernel<float><<<2 * h->n_sm, 128, 0, st>>>(d_H, n, F, d_W, c, d_labels, flag_count, flag_list, d_pred, d_correct);
+  }
   h->launches += 2;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}
+}  // namespace
+
+int lb_launch_score_tc(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
+                       int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,
+                       cudaStream_t st, bool keep_correct) {
+  return launch_score_common(h, ws, d_H, n, F, h_scale, d_W, nullptr, n_classes, d_labels, n_cand, d_pred, d_correct, st, keep_correct);
+}
+
+// S1 with an int8 output layer ("weights represented as 8 bits integers"): exact integer logits
+int lb_launch_score_q8(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, const int8_t* d_Wq, int n_classes,
+                       const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct, cudaStream_t st) {
+  return launch_score_common(h, ws, d_H, n, F, 1.0f, nullptr, d_Wq, n_classes, d_labels, n_cand, d_pred, d_correct, st, false);
+}
+
+// ---- <= 8-bit fixed-point output layer (PAPER.md:94, 98 Cell 12, 131; R16) ------------------------------------------
+namespace {
+__global__ void __launch_bounds__(256) wq_max_kernel(const float* __restrict__ W, long long per_cand, uint32_t* __restrict__ mx_bits) {
+  const long long z = blockIdx.y;
+  const float* Wz = W + z * per_cand;
+  uint32_t m = 0u;
+  for (long long e = (long long)blockIdx.x * 256 + threadIdx.x; e < per_cand; e += (long long)gridDim.x * 256)
+    m = max(m, __float_as_uint(fabsf(Wz[e])));
+  m = __reduce_max_sync(0xffffffffu, m);
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(&mx_bits[z], m);
+}
+// q = clip(rint(w * (qmax / max|W|)), -qmax, qmax): the product in fp64, round half to even -- the oracle does the same
+__global__ void __launch_bounds__(256) wq_quant_kernel(const float* __restrict__ W, long long per_cand, const uint32_t* __restrict__ mx_bits,
+                                                       int qmax, int8_t* __restrict__ Wq) {
+  const long long z = blockIdx.y;
+  const float m = __uint_as_float(mx_bits[z]);
+  const double sf = (m > 0.0f) ? (double)qmax / (double)m : 0.0;
+  for (long long e = (long long)blockIdx.x * 256 + threadIdx.x; e < per_cand; e += (long long)gridDim.x * 256) {
+    int q = __double2int_rn((double)W[z * per_cand + e] * sf);
+    q = max(-qmax, min(qmax, q));
+    Wq[z * per_cand + e] = (int8_t)q;
+  }
+}
+// scale[z] = max|W| / qmax (fp32, one rounding of the fp64 quotient), in place over the bit pattern of the maximum
+__global__ void wq_scale_kernel(uint32_t* __restrict__ mx_bits, int n_cand, int qmax) {
+  const int z = blockIdx.x * blockDim.x + threadIdx.x;
+  if (z < n_cand) {
+    const float m = __uint_as_float(mx_bits[z]);
+    reinterpret_cast<float*>(mx_bits)[z] = (float)((double)m / (double)qmax);
+  }
+}
+}  // namespace
+
+int lb_launch_quantize_w(lbcnn_handle_s* h, const float* d_W, int64_t F, int n_classes, int n_cand, int bits, int8_t* d_Wq,
+                         float* d_scale, cudaStream_t st) {
+  const int qmax = (1 << (bits - 1)) - 1;
+  const long long per = (long long)F * n_classes;
+  uint32_t* mx = reinterpret_cast<uint32_t*>(d_scale);
+  LB_CUDA_OK(cudaMemsetAsync(mx, 0, (size_t)n_cand * 4, st));
+  const unsigned gx = (unsigned)((per + 256 * 8 - 1) / (256 * 8) < 1 ? 1 : ((per + 256 * 8 - 1) / (256 * 8) > 1024 ? 1024 : (per + 256 * 8 - 1) / (256 * 8)));
+  dim3 grid(gx, (unsigned)n_cand);
+  wq_max_kernel<<<grid, 256, 0, st>>>(d_W, per, mx);
+  wq_quant_kernel<<<grid, 256, 0, st>>>(d_W, per, mx, qmax, d_Wq);
+  wq_scale_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(mx, n_cand, qmax);
+  h->launches += 3;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;
 }

@@ -332,6 +332,45 @@ def test_score_tensor_core_equals_fp64_argmax(handle, K, n, F, c, amax):
     assert (pred[0] != c - 1).all() or c == 2          # ties resolved to the lower index
 
 
+@pytest.mark.parametrize("name,ntr,nte,K,bits", [("mnist", 1500, 700, 3, 8), ("gtsrb", 2600, 900, 2, 8), ("orl", 280, 120, 4, 6),
+                                                  ("tiny_mnist", 2000, 500, 3, 4)])
+def test_quantised_output_layer_matches_oracle(handle, name, ntr, nte, K, bits):
+    """SURVEY.md 8(f)-2 ("weights represented as 8 bits integers"; R16): lbcnn_quantize_output_layer
+    must reproduce the oracle's integers and scale BIT-EXACTLY, and lbcnn_elm_score_q (exact integer logits on the tensor
+    pipe) the oracle's labels ONE BY ONE with identical counts -- integer work, so no tolerance."""
+    w = _small(name, ntr, nte, K)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    W, _, _, info = _staged(handle, w, trx, try_, tex, tey, ker)
+    assert (info == 0).all()
+    W32 = W.astype(np.float32)
+    Hte = handle.expand(lb.arch_of(w, 1.0), _dev(tex), _dev(ker))
+    Wq, scale = handle.quantize_output_layer(_dev(W32), bits)
+    pred, corr = handle.elm_score_q(Hte, Wq, _dev(tey))
+    torch.cuda.synchronize()
+    Wq, scale, pred, corr = Wq.cpu().numpy(), scale.cpu().numpy(), pred.cpu().numpy(), corr.cpu().numpy()
+    oa = _orc_arch(w)
+    for k in range(K):
+        qo, so = orc.quantize_output_layer(W32[k], bits)
+        assert np.array_equal(Wq[k], qo), k
+        assert scale[k] == so
+        po, co, logits = orc.elm_score_q(orc.expand(oa, tex, ker[k]), qo, tey)
+        assert np.array_equal(pred[k], po), (k, np.nonzero(pred[k] != po)[0][:10])
+        assert corr[k] == co
+    # constructed ties and a row with a non-integer feature (evaluated in fp64 by the second kernel)
+    H2 = Hte[:1].clone()
+    H2[0, 1, 0] += 0.5
+    q2 = Wq[:1].copy()
+    q2[0, :, w.n_classes - 1] = q2[0, :, 0]
+    p2, _ = handle.elm_score_q(H2, _dev(q2))
+    p2 = p2.cpu().numpy()[0]
+    ref = (H2[0].cpu().numpy().astype(np.float64) @ q2[0].astype(np.float64))
+    assert (p2 != w.n_classes - 1).all()
+    rows = np.arange(len(p2)) != 1
+    assert np.array_equal(p2[rows], np.argmax(ref, axis=1)[rows])
+    assert p2[1] == int(np.argmax(ref[1]))
+
+
 def _search_both(handle, w, budget=None):
     trx, try_, tex, tey = synth.make_dataset(w)
     ker = synth.make_kernels(w)

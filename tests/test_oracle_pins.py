@@ -537,3 +537,45 @@ def test_search_failed_fit_is_excluded(monkeypatch):
     assert np.array_equal(r["acc"][[0, 2, 3]], others["acc"])
     assert r["best"] == [0, 2, 3][others["best"]] and r["worst"] == [0, 2, 3][others["worst"]]
     assert r["best"] != 1 and r["worst"] != 1
+
+
+# ------------------------------------------------------------------------------------------------
+# <= 8-bit output layer (R16)
+# ------------------------------------------------------------------------------------------------
+def test_quantize_worked_example_and_bounds():
+    W = np.array([[0.5, -1.0], [0.25, 0.126]], dtype=np.float32)
+    q, scale = orc.quantize_output_layer(W, 8)
+    # 0.5 * 127 = 63.5 -> 64 (half to even), -127, 31.75 -> 32, 16.002 -> 16
+    assert q.tolist() == [[64, -127], [32, 16]] and q.dtype == np.int8
+    assert scale == np.float32(1.0 / 127.0)
+    q2, s2 = orc.quantize_output_layer(W, 2)            # qmax = 1: sign of everything above half the maximum
+    assert q2.tolist() == [[0, -1], [0, 0]] and s2 == np.float32(1.0)      # 0.5 -> rint(0.5) = 0 (half to even)
+    rng = np.random.default_rng(3)
+    for bits in (3, 5, 8):
+        Wr = (rng.standard_normal((40, 7)) * rng.uniform(1e-3, 10)).astype(np.float32)
+        q, scale = orc.quantize_output_layer(Wr, bits)
+        qmax = 2 ** (bits - 1) - 1
+        assert np.abs(q).max() == qmax                                     # the largest weight maps to +-qmax
+        assert np.all(np.abs(Wr.astype(np.float64) - float(scale) * q) <= 0.5 * float(scale) * (1 + 1e-6))
+        qa, sa = orc.quantize_output_layer(Wr * np.float32(4.0), bits)     # a power-of-two rescaling changes only the scale
+        assert np.array_equal(qa, q) and sa == np.float32(4.0) * scale
+        qd, _ = orc.quantize_output_layer((float(scale) * q).astype(np.float32), bits)      # a grid point stays put
+        assert np.array_equal(qd, q)
+    qz, sz = orc.quantize_output_layer(np.zeros((3, 2), dtype=np.float32), 8)
+    assert not qz.any() and sz == 0.0
+    with pytest.raises(ValueError):
+        orc.quantize_output_layer(W, 9)
+
+
+def test_score_q_is_exact_integer_arithmetic():
+    rng = np.random.default_rng(9)
+    U = rng.integers(-900000, 900000, size=(30, 17))
+    q = rng.integers(-127, 128, size=(17, 5)).astype(np.int8)
+    q[:, 4] = q[:, 1]                                                      # exact ties: the lower index must win
+    y = rng.integers(0, 5, size=30).astype(np.int32)
+    pred, corr, logits = orc.elm_score_q(U, q, y)
+    for i in range(30):                                                    # python integers: no rounding anywhere
+        row = [sum(int(U[i, f]) * int(q[f, c]) for f in range(17)) for c in range(5)]
+        assert row == logits[i].tolist()
+        assert pred[i] == row.index(max(row))
+    assert (pred != 4).all() and corr == int((pred == y).sum())
