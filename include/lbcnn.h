@@ -232,6 +232,22 @@ int lbcnn_elm_score_q(lbcnn_handle_t h, const float* d_H /*[n_cand][n][F]*/, int
                       const int8_t* d_Wq /*[n_cand][F][n_classes]*/, int32_t n_classes, const int32_t* d_labels /*[n] or NULL*/,
                       int32_t n_cand, int32_t* d_pred /*[n_cand][n] or NULL*/, int32_t* d_correct /*[n_cand] or NULL*/, void* stream);
 
+/* A non-random candidate generator ("nature inspired optimization methods (such as genetic algorithms or swarm
+ * intelligence methods)"; the paper gives no algorithm -- reading DESIGN.md R17): ONE generation of an elitist
+ * genetic search.  From this generation's kernel sets and the accuracies lbcnn_search_candidates returned for them:
+ *   1. rank the candidates by accuracy, best first, equal accuracies by index (a failed fit has accuracy -1: last);
+ *   2. d_next[0 .. n_elite-1] = the n_elite best kernel sets, unchanged, in rank order;
+ *   3. every other child j draws two parents, each the better-ranked of two uniformly drawn candidates (binary tournament),
+ *      takes every tap from parent 1 or parent 2 with probability 1/2 (uniform crossover) and flips it with probability
+ *      mut_ppm / 10^6 (mutation).
+ * Random numbers: u64 draw(i) = mix(ckey + G (i + 1)), ckey = mix(key + 0xBF58476D1CE4E5B9 (j + 1)),
+ * key = mix(seed XOR G (generation + 1)), G = 0x9E3779B97F4A7C15, mix = the splitmix64 finaliser; draws 0,1 / 2,3 are the
+ * tournament candidates (mod n_cand), draw 4 + t decides tap t (bit 0: parent; (draw >> 20) mod 10^6 < mut_ppm: flip).
+ * Byte work, bit-exact against the oracle.  Needs 8 * n_cand bytes of workspace; n_cand <= 16384; d_next != d_kernels. */
+int lbcnn_evolve_candidates(lbcnn_handle_t h, const int8_t* d_kernels /*[n_cand][n_weights]*/, const float* d_acc /*[n_cand]*/,
+                            int32_t n_cand, int64_t n_weights, int32_t n_elite, uint32_t mut_ppm, uint64_t seed,
+                            uint32_t generation, int8_t* d_next /*[n_cand][n_weights]*/, void* stream);
+
 /* Workspace lbcnn_elm_score needs under LBCNN_SCORER_TENSOR (host-only arithmetic; 0 is never returned). */
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes);
 

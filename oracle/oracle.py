@@ -236,3 +236,59 @@ def elm_score_q(U: np.ndarray, q: np.ndarray, labels: Optional[np.ndarray] = Non
     pred = np.argmax(logits, axis=1).astype(np.int32)          # numpy returns the first maximum
     corr = None if labels is None else int((pred == np.asarray(labels)).sum())
     return pred, corr, logits
+
+
+# ---- non-random candidate generator: one generation of a genetic search --------------------------------
+# "nature inspired optimization methods (such as genetic algorithms or swarm intelligence methods)" are named as the way to
+# go beyond random kernels; the paper gives no algorithm, so this is reading DESIGN.md R17, followed
+# step by step.  The random numbers are a counter-based generator both sides implement: a splitmix64 finaliser keyed by
+# (seed, generation, child, draw index).
+_U64 = (1 << 64) - 1
+_G1, _G2, _G3 = 0x9E3779B97F4A7C15, 0xBF58476D1CE4E5B9, 0x94D049BB133111EB
+
+
+def ga_mix64(z: int) -> int:
+    z &= _U64
+    z = ((z ^ (z >> 30)) * _G2) & _U64
+    z = ((z ^ (z >> 27)) * _G3) & _U64
+    return z ^ (z >> 31)
+
+
+def ga_draw(seed: int, generation: int, child: int, i: int) -> int:
+    key = ga_mix64((seed & _U64) ^ ((_G1 * (generation + 1)) & _U64))
+    ckey = ga_mix64(key + _G2 * (child + 1))
+    return ga_mix64(ckey + _G1 * (i + 1))
+
+
+def evolve_candidates(kernels: np.ndarray, acc: np.ndarray, n_elite: int, mut_ppm: int, seed: int, generation: int):
+    """kernels int8 [K][n_weights] (+-1), acc [K] (the search's accuracies; a failed fit has -1).
+    R17: 1. rank the candidates by accuracy, best first, equal accuracies by index;
+         2. children 0 .. n_elite-1 are the n_elite best, unchanged, in rank order (elitism);
+         3. every other child j draws two parents, each the better-ranked of two uniformly drawn candidates (binary
+            tournament: draws 0,1 and 2,3, candidate = draw mod K), takes each tap from parent 1 or 2 by bit 0 of draw 4 + t
+            (uniform crossover), and flips it when (draw >> 20) mod 10^6 < mut_ppm (mutation).
+    Returns (next int8 [K][n_weights], parents int32 [K][2] with -1 for elites, order int32 [K])."""
+    kernels = np.ascontiguousarray(kernels, dtype=np.int8)
+    K, nw = kernels.shape
+    a = np.asarray(acc, dtype=np.float32)
+    order = sorted(range(K), key=lambda i: (-float(a[i]), i))
+    rank = [0] * K
+    for r, i in enumerate(order):
+        rank[i] = r
+    nxt = np.empty_like(kernels)
+    parents = np.full((K, 2), -1, dtype=np.int32)
+    for j in range(K):
+        if j < n_elite:
+            nxt[j] = kernels[order[j]]
+            continue
+        c = [ga_draw(seed, generation, j, i) % K for i in range(4)]
+        p1 = c[0] if rank[c[0]] <= rank[c[1]] else c[1]
+        p2 = c[2] if rank[c[2]] <= rank[c[3]] else c[3]
+        parents[j] = (p1, p2)
+        for t in range(nw):
+            d = ga_draw(seed, generation, j, 4 + t)
+            v = int(kernels[p1, t]) if (d & 1) == 0 else int(kernels[p2, t])
+            if ((d >> 20) % 1000000) < mut_ppm:
+                v = -v
+            nxt[j, t] = v
+    return nxt, parents, np.array(order, dtype=np.int32)

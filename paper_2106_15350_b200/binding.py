@@ -27,7 +27,7 @@ EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destro
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
            "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes",
-           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q")
+           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q", "lbcnn_evolve_candidates")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -284,6 +284,17 @@ class Handle:
                                      _ptr(W, torch.float32), C.c_int32(c), _ptr(labels, torch.int32, True), C.c_int32(K),
                                      _ptr(pred, None, True), _ptr(corr, None, True), _stream()), "lbcnn_elm_score")
         return pred, corr
+
+    def evolve_candidates(self, kernels, acc, n_elite: int, mut_ppm: int, seed: int, generation: int):
+        """one generation of the genetic candidate generator: kernels i8 [K][n_weights], acc f32 [K] -> next i8 [K][n_weights]."""
+        import torch
+        K, nw = kernels.shape
+        nxt = torch.empty_like(kernels)
+        self.ensure_workspace(256 + 8 * K)
+        _check(lib().lbcnn_evolve_candidates(self._h, _ptr(kernels, torch.int8), _ptr(acc, torch.float32), C.c_int32(K),
+                                             C.c_int64(nw), C.c_int32(n_elite), C.c_uint32(mut_ppm), C.c_uint64(seed),
+                                             C.c_uint32(generation), _ptr(nxt), _stream()), "lbcnn_evolve_candidates")
+        return nxt
 
     def quantize_output_layer(self, W, bits: int = 8):
         """W f32 [K][F][c] -> (Wq i8 [K][F][c], scale f32 [K]); W ~ scale * Wq (include/lbcnn.h)."""

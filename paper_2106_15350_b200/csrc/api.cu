@@ -352,6 +352,15 @@ int lbcnn_elm_score_q(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, 
   return lb_launch_score_q8(h, lb_ws_base(h), d_H, n, F, d_Wq, n_classes, d_labels, n_cand, d_pred, d_correct, (cudaStream_t)stream);
 }
 
+int lbcnn_evolve_candidates(lbcnn_handle_t h, const int8_t* d_kernels, const float* d_acc, int32_t n_cand, int64_t n_weights,
+                            int32_t n_elite, uint32_t mut_ppm, uint64_t seed, uint32_t generation, int8_t* d_next, void* stream) {
+  if (!h || !d_kernels || !d_acc || !d_next || n_cand < 1 || n_cand > 16384 || n_weights < 1) return LBCNN_ERR_INVALID_ARG;
+  if (n_elite < 0 || n_elite > n_cand || mut_ppm > 1000000u || d_next == d_kernels) return LBCNN_ERR_INVALID_ARG;
+  if (!h->ws || lb_ws_avail(h) < (size_t)n_cand * 8) return LBCNN_ERR_WORKSPACE;
+  return lb_launch_evolve(h, lb_ws_base(h), d_kernels, d_acc, n_cand, n_weights, n_elite, mut_ppm, seed, generation, d_next,
+                          (cudaStream_t)stream);
+}
+
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes) {
   if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   *bytes = lb_score_tc_ws_bytes(n, F, n_classes, n_cand) + LB_WS_HEAD;

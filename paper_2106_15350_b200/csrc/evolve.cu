@@ -1,0 +1,68 @@
+// evolve.cu -- a non-random candidate generator on top of the search driver: one generation of an
+// elitist genetic search over binary kernel sets.  The paper names "nature inspired optimization methods (such as
+// genetic algorithms or swarm intelligence methods)" as the step beyond random kernels without
+// giving an algorithm; this follows reading DESIGN.md R17 (include/lbcnn.h states it in full).  Everything is integer /
+// byte work and the random numbers are a counter-based splitmix64 finaliser keyed by (seed, generation, child, draw), so
+// the result is bit-exact against the oracle, which implements the same generator on its own.
+#include "internal.h"
+
+namespace {
+
+constexpr unsigned long long G1 = 0x9E3779B97F4A7C15ull, G2 = 0xBF58476D1CE4E5B9ull, G3 = 0x94D049BB133111EBull;
+
+__host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+  z = (z ^ (z >> 30)) * G2;
+  z = (z ^ (z >> 27)) * G3;
+  return z ^ (z >> 31);
+}
+
+// rank by accuracy, best first, equal accuracies by index: order[rank] = candidate, rank_of[candidate] = rank
+__global__ void __launch_bounds__(256) ga_rank_kernel(const float* __restrict__ acc, int K, int32_t* __restrict__ order,
+                                                      int32_t* __restrict__ rank_of) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= K) return;
+  const float ai = acc[i];
+  int r = 0;
+  for (int j = 0; j < K; ++j) {
+    const float aj = acc[j];
+    r += (aj > ai || (aj == ai && j < i)) ? 1 : 0;
+  }
+  order[r] = i;
+  rank_of[i] = r;
+}
+
+__global__ void __launch_bounds__(256) ga_child_kernel(const int8_t* __restrict__ ker, int K, long long nw, int n_elite,
+                                                       unsigned int mut_ppm, unsigned long long key,
+                                                       const int32_t* __restrict__ order, const int32_t* __restrict__ rank_of,
+                                                       int8_t* __restrict__ next) {
+  const int j = blockIdx.y;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nw) return;
+  int8_t* dst = next + (long long)j * nw;
+  if (j < n_elite) { dst[t] = ker[(long long)order[j] * nw + t]; return; }
+  const unsigned long long ckey = mix64(key + G2 * (unsigned long long)(j + 1));
+  int c[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) c[i] = (int)(mix64(ckey + G1 * (unsigned long long)(i + 1)) % (unsigned long long)K);
+  const int p1 = (rank_of[c[0]] <= rank_of[c[1]]) ? c[0] : c[1];
+  const int p2 = (rank_of[c[2]] <= rank_of[c[3]]) ? c[2] : c[3];
+  const unsigned long long d = mix64(ckey + G1 * (unsigned long long)(4 + t + 1));
+  int v = ((d & 1ull) == 0ull) ? ker[(long long)p1 * nw + t] : ker[(long long)p2 * nw + t];
+  if (((d >> 20) % 1000000ull) < (unsigned long long)mut_ppm) v = -v;
+  dst[t] = (int8_t)v;
+}
+
+}  // namespace
+
+int lb_launch_evolve(lbcnn_handle_s* h, void* ws, const int8_t* d_kernels, const float* d_acc, int n_cand, int64_t n_weights,
+                     int n_elite, uint32_t mut_ppm, uint64_t seed, uint32_t generation, int8_t* d_next, cudaStream_t st) {
+  int32_t* order = reinterpret_cast<int32_t*>(ws);
+  int32_t* rank_of = order + n_cand;
+  ga_rank_kernel<<<(n_cand + 255) / 256, 256, 0, st>>>(d_acc, n_cand, order, rank_of);
+  const unsigned long long key = mix64((unsigned long long)seed ^ (G1 * (unsigned long long)(generation + 1)));
+  dim3 grid((unsigned)((n_weights + 255) / 256), (unsigned)n_cand);
+  ga_child_kernel<<<grid, 256, 0, st>>>(d_kernels, n_cand, n_weights, n_elite, mut_ppm, key, order, rank_of, d_next);
+  h->launches += 2;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}

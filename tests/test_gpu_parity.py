@@ -371,6 +371,36 @@ def test_quantised_output_layer_matches_oracle(handle, name, ntr, nte, K, bits):
     assert p2[1] == int(np.argmax(ref[1]))
 
 
+def test_genetic_generator_bit_exact_and_improves(handle):
+    """lbcnn_evolve_candidates must reproduce the oracle's next
+    generation byte for byte (ties in the ranking, a failed candidate, elites, several mutation rates), and a search driven
+    by it keeps its best accuracy from generation to generation (elitism) on the tiny config."""
+    rng = np.random.default_rng(33)
+    for K, nw, elite, ppm, seed, gen in [(24, 300, 4, 20000, 7, 2), (7, 1890, 1, 0, 123456789012345, 0), (64, 37, 0, 1000000, 1, 9),
+                                         (130, 513, 130, 5000, 2, 1)]:
+        ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+        acc = rng.integers(50, 60, size=K).astype(np.float32) / 100.0          # many exact ties
+        acc[K // 2] = -1.0
+        nxt = handle.evolve_candidates(_dev(ker), _dev(acc), elite, ppm, seed, gen).cpu().numpy()
+        ref, _, _ = orc.evolve_candidates(ker, acc, elite, ppm, seed, gen)
+        assert np.array_equal(nxt, ref), (K, nw)
+    # a three-generation search on configs[0]: elitism keeps the running best, children are evaluated by the same driver
+    w = synth.WORKLOADS["tiny_mnist"]
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = _dev(synth.make_kernels(w))
+    arch = lb.arch_of(w)
+    data = (_dev(trx), _dev(try_), _dev(tex), _dev(tey))
+    best = []
+    for g in range(3):
+        handle.set_workspace(None)
+        handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+        out = handle.search_candidates(arch, *data, w.n_classes, w.C, ker)
+        acc = out["acc"].clone()
+        best.append(float(acc.max()))
+        ker = handle.evolve_candidates(ker, acc, 2, 30000, 99, g)
+    assert best[1] >= best[0] and best[2] >= best[1]
+
+
 def _search_both(handle, w, budget=None):
     trx, try_, tex, tey = synth.make_dataset(w)
     ker = synth.make_kernels(w)

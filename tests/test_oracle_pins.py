@@ -579,3 +579,50 @@ def test_score_q_is_exact_integer_arithmetic():
         assert row == logits[i].tolist()
         assert pred[i] == row.index(max(row))
     assert (pred != 4).all() and corr == int((pred == y).sum())
+
+
+# ------------------------------------------------------------------------------------------------
+# genetic candidate generator (R17)
+# ------------------------------------------------------------------------------------------------
+def test_ga_generator_known_answers():
+    # splitmix64 (Steele, Lea, Flood 2014) from state 0: the published first outputs are mix(1 * golden), mix(2 * golden)
+    assert orc.ga_mix64(0x9E3779B97F4A7C15) == 0xE220A8397B1DCDAF
+    assert orc.ga_mix64(2 * 0x9E3779B97F4A7C15) == 0x6E789E6AA1B965F4
+    assert orc.ga_draw(1, 0, 0, 0) != orc.ga_draw(1, 0, 0, 1) != orc.ga_draw(1, 1, 0, 0)
+
+
+def test_ga_generation_properties():
+    rng = np.random.default_rng(21)
+    K, nw = 24, 300
+    ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+    acc = rng.uniform(0.5, 0.9, size=K).astype(np.float32)
+    acc[5] = acc[11] = 0.95                   # a tie for the best: index 5 ranks first
+    acc[3] = -1.0                             # a failed fit ranks last
+    nxt, par, order = orc.evolve_candidates(ker, acc, n_elite=4, mut_ppm=0, seed=7, generation=2)
+    assert order[0] == 5 and order[1] == 11 and order[-1] == 3
+    assert list(order) == sorted(range(K), key=lambda i: (-acc[i], i))
+    for j in range(4):                        # elitism: the best four, unchanged, in rank order
+        assert np.array_equal(nxt[j], ker[order[j]]) and (par[j] == -1).all()
+    assert set(np.unique(nxt)) <= {-1, 1}
+    frac1 = []
+    for j in range(4, K):                     # without mutation every tap comes from one of the two parents
+        p1, p2 = par[j]
+        assert np.all((nxt[j] == ker[p1]) | (nxt[j] == ker[p2]))
+        differ = ker[p1] != ker[p2]
+        if differ.sum() > 50:
+            frac1.append((nxt[j][differ] == ker[p1][differ]).mean())
+    assert 0.4 < np.mean(frac1) < 0.6         # uniform crossover
+    # tournament: a parent is the better-ranked of its two draws, so parents rank better than uniform on average
+    rank = np.empty(K, dtype=int); rank[order] = np.arange(K)
+    assert rank[par[4:].ravel()].mean() < (K - 1) / 2.0
+    # mutation only: with rate 1 every tap of the crossover result is flipped; with rate 2 % about 2 % are
+    flipped, _, _ = orc.evolve_candidates(ker, acc, 4, 1000000, 7, 2)
+    assert np.array_equal(flipped[4:], -nxt[4:]) and np.array_equal(flipped[:4], nxt[:4])
+    some, _, _ = orc.evolve_candidates(ker, acc, 4, 20000, 7, 2)
+    rate = (some[4:] != nxt[4:]).mean()
+    assert 0.012 < rate < 0.028
+    # counter-based: same arguments -> same children; another generation or seed -> different ones
+    again, _, _ = orc.evolve_candidates(ker, acc, 4, 20000, 7, 2)
+    assert np.array_equal(again, some)
+    assert not np.array_equal(orc.evolve_candidates(ker, acc, 4, 20000, 7, 3)[0], some)
+    assert not np.array_equal(orc.evolve_candidates(ker, acc, 4, 20000, 8, 2)[0], some)
