@@ -383,6 +383,70 @@ def _summary(res, steps, world, replicas, peaks):
                 config=_config(w, res["K"], res["l2_note"]))
 
 
+def _extras(lb, synth, torch, np, name, peaks, local):
+    """the SURVEY.md 8(f) rows built so far, measured on the bench workload (CUDA events, 3 timed repeats after 2 warm-ups):
+    streamed search (8(f)-1), int8 output layer + exact integer scorer (8(f)-2), one genetic generation (8(f)-3)."""
+    w = synth.WORKLOADS[name]
+    K = w.n_cand
+    trx, try_, tex, tey = synth.make_dataset(w)
+    dev = torch.device("cuda", local)
+    d = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (trx, try_, tex, tey, synth.make_kernels(w, K))]
+    arch = lb.arch_of(w)
+    F, _ = lb.feature_dim(arch)
+    h = lb.Handle(local)
+
+    def timed(fn, reps=3, warm=2):
+        for _ in range(warm):
+            fn()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        torch.cuda.synchronize()
+        for a, b in ev:
+            a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev) / reps
+
+    out = {}
+    # 8(f)-1: streamed search, 4096 samples resident at once
+    rows = 4096
+    full = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, handle=h)[0]
+    h.set_option(lb.OPT_STREAM_ROWS, rows)
+    small = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, handle=h)[0]
+    h.ensure_workspace(small)
+    res = {}
+    ms = timed(lambda: res.update(h.search_candidates(arch, d[0], d[1], d[2], d[3], w.n_classes, w.C, d[4], out=res or None)))
+    out["streamed_search"] = dict(stream_rows=rows, value=K / (ms * 1e-3), unit=UNIT, ms_per_step=round(ms, 3),
+                                  workspace_gb=round(small / 1e9, 3), resident_workspace_gb=round(full / 1e9, 3),
+                                  note="bit-identical results to the resident search (tests/test_gpu_parity.py)")
+    h.set_option(lb.OPT_STREAM_ROWS, 0)
+    acc = res["acc"].clone()
+    h.set_workspace(None)
+    # 8(f)-2: int8 output layer on the first min(K, 16) candidates' test features
+    kq = min(K, 16)
+    a1 = lb.arch_of(w, 1.0)
+    Hte = h.expand(a1, d[2], d[4][:kq])
+    Htr = h.expand(a1, d[0], d[4][:kq])
+    h.ensure_workspace(lb.fit_workspace_bytes(w.n_train, F, w.n_classes, kq, lb.H_INTEGER))
+    s = float(np.float32(w.feature_scale))
+    W, _ = h.elm_fit(Htr, d[1], w.n_classes, w.C, h_scale=s, flags=lb.H_INTEGER)
+    del Htr
+    Wq, _ = h.quantize_output_layer(W, 8)
+    corr = {}
+    ms_q = timed(lambda: corr.update(c=h.elm_score_q(Hte, Wq, d[3], want_pred=False)[1]))
+    _, corr_f = h.elm_score(Hte, W, d[3], h_scale=s, want_pred=False)
+    gb = kq * (float(w.n_test) * F * 4.0 + F * w.n_classes) / 1e9
+    out["score_q8"] = dict(candidates=kq, ms=round(ms_q, 4), achieved=round(gb / (ms_q * 1e-3), 1), peak=round(peaks["hbm_gbs"], 1),
+                           unit="GB/s", frac=round(gb / (ms_q * 1e-3) / peaks["hbm_gbs"], 4), bound="hbm",
+                           accuracy_int8=round(float(corr["c"].float().mean().item()) / w.n_test, 4),
+                           accuracy_fp32=round(float(corr_f.float().mean().item()) / w.n_test, 4),
+                           note="exact integer logits (lbcnn_elm_score_q), test features read once as fp32")
+    # 8(f)-3: one genetic generation over the K kernel sets
+    ms_g = timed(lambda: h.evolve_candidates(d[4], acc, max(1, K // 8), 20000, 1, 0))
+    out["evolve"] = dict(candidates=K, ms=round(ms_g, 4), note="rank + tournament + uniform crossover + mutation (lbcnn_evolve_candidates)")
+    h.close()
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_cuda(args):
     import numpy as np
     import torch
@@ -430,6 +494,9 @@ def run_cuda(args):
             del sm["roofline"]
             per_config[name] = sm
 
+    extras = None
+    if not args.no_extras and not args.n_cand and world == 1:
+        extras = _extras(lb, synth, torch, np, args.workload, peaks, local)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -442,6 +509,8 @@ def run_cuda(args):
                 accuracy=main["accuracy"])
     if per_config:
         line["per_config"] = per_config
+    if extras:
+        line["extras"] = extras
     if not args.no_cpu_baseline:
         # bounded sample (about 10-30 s of host work): (candidates, N_train, N_test) of the same workload
         trx, try_, tex, tey = res["data"]
@@ -483,6 +552,7 @@ def main():
     ap.add_argument("--mid-panel", type=int, default=-1, help="LBCNN_OPT_MID_PANEL (measurement)")
     ap.add_argument("--stream-rows", type=int, default=0, help="LBCNN_OPT_STREAM_ROWS: streamed search, samples per chunk")
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the measurements of the SURVEY.md 8(f) rows")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
     ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")
     args = ap.parse_args()
