@@ -467,8 +467,6 @@ def run_cuda(args):
         OPTIONS.append((lb.OPT_SOLVER, {"auto": lb.SOLVER_AUTO, "fp64": lb.SOLVER_FP64, "mixed": lb.SOLVER_MIXED}[args.solver]))
     if args.panel:
         OPTIONS.append((lb.OPT_PANEL, args.panel))
-    if args.inner_tc >= 0:
-        OPTIONS.append((lb.OPT_INNER_TC, args.inner_tc))
     if args.mid_panel >= 0:
         OPTIONS.append((lb.OPT_MID_PANEL, args.mid_panel))
     if args.stream_rows > 0:
@@ -548,7 +546,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--solver", default="", choices=["", "auto", "fp64", "mixed"], help="LBCNN_OPT_SOLVER (measurement)")
     ap.add_argument("--panel", type=int, default=0, help="LBCNN_OPT_PANEL (measurement)")
-    ap.add_argument("--inner-tc", type=int, default=-1, help="LBCNN_OPT_INNER_TC (measurement)")
     ap.add_argument("--mid-panel", type=int, default=-1, help="LBCNN_OPT_MID_PANEL (measurement)")
     ap.add_argument("--stream-rows", type=int, default=0, help="LBCNN_OPT_STREAM_ROWS: streamed search, samples per chunk")
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")

@@ -110,16 +110,15 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                run in fp64; a finished block updates the rest of its panel on the tensor pipe
  *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 1024) of the blocked Cholesky when its trailing
  *                                updates run on the tensor pipe (measurement)
- *   LBCNN_OPT_INNER_TC           1: the 64-column steps inside a panel use the tensor-pipe update too (default 0: fp64 DMMA;
- *                                at K = 64 the update is bound by its read-modify-write traffic, measured slower)
- *   LBCNN_OPT_DEFLATE            0: the first block column's trailing update goes through the int8 slices too (default 1: it
- *                                stays fp64 -- it carries the common mode of the all-positive features)
+ *   LBCNN_OPT_DEFLATE            d = 0..64 (default 16): the first d columns of the factor -- they carry the common mode of the
+ *                                all-positive features -- update the matrix beyond the first block in fp64 instead of through
+ *                                the int8 slices; 0 = everything through the slices
  *   LBCNN_OPT_SCORER             LBCNN_SCORER_AUTO: the search driver scores its integer features on the tensor pipe (int8 digit
  *                                products, rows inside the error bound re-evaluated in fp64 -- the decision equals the fp64
  *                                argmax), lbcnn_elm_score uses the fp64 kernel; _FP64: fp64 everywhere; _TENSOR: lbcnn_elm_score
  *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
  *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
-enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_INNER_TC = 4, LBCNN_OPT_DEFLATE = 5,
+enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_DEFLATE = 5,
        LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7, LBCNN_OPT_STREAM_ROWS = 8 };
 enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };

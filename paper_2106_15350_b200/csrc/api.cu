@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->inner_tc = 0; p->deflate = 1; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->deflate = 16; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -96,8 +96,9 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
       if (value != LBCNN_SOLVER_AUTO && value != LBCNN_SOLVER_FP64 && value != LBCNN_SOLVER_MIXED) return LBCNN_ERR_INVALID_ARG;
       h->solver = value; return LBCNN_OK;
     case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
-    case LBCNN_OPT_INNER_TC: h->inner_tc = value ? 1 : 0; return LBCNN_OK;
-    case LBCNN_OPT_DEFLATE: h->deflate = value ? 1 : 0; return LBCNN_OK;
+    case LBCNN_OPT_DEFLATE:
+      if (value < 0 || value > 64) return LBCNN_ERR_INVALID_ARG;
+      h->deflate = value; return LBCNN_OK;
     case LBCNN_OPT_SCORER:
       if (value != LBCNN_SCORER_AUTO && value != LBCNN_SCORER_FP64 && value != LBCNN_SCORER_TENSOR) return LBCNN_ERR_INVALID_ARG;
       h->scorer = value; return LBCNN_OK;

@@ -353,6 +353,8 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   const bool tc_solve = pl.stc_kmax > 0 && (h->solver == LBCNN_SOLVER_MIXED || (h->solver == LBCNN_SOLVER_AUTO && dim >= LB_STC_AUTO_DIM));
   const int NBO = tc_solve ? h->panel : 256;
   const int NBM = (tc_solve && h->mid_panel >= NB && h->mid_panel < NBO) ? h->mid_panel : NBO;      // mid level (fp64 steps inside)
+  // columns of the common-mode deflation (fp64); never wider than one 64-column step or the system
+  const int dfl = (tc_solve && h->deflate > 0) ? (int)((h->deflate < NB ? h->deflate : NB) < dim ? (h->deflate < NB ? h->deflate : NB) : dim) : 0;
   CholTcCtx tcx;
   if (tc_solve) {
     rc = lb_chol_tc_begin(h, base + pl.stc_off, rows, dim, n_cand, pl.stc_kmax, A, a_stride, ld, lb_ws_counter(h, 1), &tcx);
@@ -377,23 +379,20 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
         g.M = (int)(rows - j1); g.N = nbj; g.K = nbj; g.alpha = 1.0; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
         rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
         if (rc) return rc;
-        // The very first block column carries the features' common mode (all features are positive: L's first column
-        // is 10-100x larger than the rest of its row).  Inside a row-scaled int8 slice it would cost the other columns
-        // that many bits, so its update of the WHOLE trailing matrix stays on the fp64 path and the tensor-core update of
-        // panel 0 starts at column 64.
-        const bool deflate = tc_solve && h->deflate && j0 == 0;
-        if (deflate && dim - j1 > 0) {
+        // The very first columns carry the features' common mode (all features are positive: L's first column is 10-100x
+        // larger than the rest of its row).  Inside a row-scaled int8 slice it would cost the other columns that many
+        // bits, so the update of everything beyond the first mid block by the first `dfl` columns stays on the fp64 path
+        // (a K = dfl product) and the tensor-core updates of block 0 / panel 0 start at column dfl.
+        if (dfl > 0 && j0 == 0 && dim - M1 > 0) {
           GemmP u{};
-          u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
-          u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
-          u.C = A + j1 * ld + j1; u.ldc = ld; u.bC = a_stride;
-          u.M = (int)(rows - j1); u.N = (int)(dim - j1); u.K = nbj; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
+          u.A = A + M1 * ld; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
+          u.B = A + M1 * ld; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
+          u.C = A + M1 * ld + M1; u.ldc = ld; u.bC = a_stride;
+          u.M = (int)(rows - M1); u.N = (int)(dim - M1); u.K = dfl; u.alpha = -1.0; u.accumulate = 1; u.lower = 1; u.diag = 0.0;
           rc = launch_gemm<double, double, double, true, true>(h, u, n_cand, st);
           if (rc) return rc;
-        } else if (J1 - j1 > 0 && tc_solve && h->inner_tc) {           // rest of the panel on the tensor pipe (K = 64; measurement)
-          rc = lb_chol_tc_update(h, tcx, (int)j1, (int)J1, (int)j0, nbj, st);
-          if (rc) return rc;
-        } else if (M1 - j1 > 0) {                                      // rest of the mid block: columns j1 .. M1-1 (fp64)
+        }
+        if (M1 - j1 > 0) {                                      // rest of the mid block: columns j1 .. M1-1 (fp64)
           GemmP u{};
           u.A = A + j1 * ld + j0; u.sAr = ld; u.sAk = 1; u.bA = a_stride;
           u.B = A + j1 * ld + j0; u.sBr = ld; u.sBk = 1; u.bB = a_stride;
@@ -404,15 +403,15 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
         }
         // a finished mid block updates the rest of its panel on the tensor pipe (K = NBM): the fp64 steps above then only
         // ever touch NBM-wide strips, and the wide trailing matrix is read and written once per NBO columns
-        if (j1 == M1 && J1 - M1 > 0 && NBM < NBO && !(h->inner_tc)) {
-          const long long K0 = (h->deflate && M0 == 0) ? ((NB < M1) ? NB : M1) : M0;
+        if (j1 == M1 && J1 - M1 > 0 && NBM < NBO) {
+          const long long K0 = (M0 == 0) ? dfl : M0;
           rc = lb_chol_tc_update(h, tcx, (int)M1, (int)J1, (int)K0, (int)(M1 - K0), st);
           if (rc) return rc;
         }
       }
     }
     if (dim - J1 > 0 && tc_solve) {                                    // trailing matrix on the tensor pipe
-      const long long K0 = (h->deflate && J0 == 0) ? ((NB < J1) ? NB : J1) : J0;      // block column 0 was applied in fp64
+      const long long K0 = (J0 == 0) ? dfl : J0;                       // columns 0 .. dfl-1 were applied in fp64
       rc = lb_chol_tc_update(h, tcx, (int)J1, (int)dim, (int)K0, (int)(J1 - K0), st);
       if (rc) return rc;
     } else if (dim - J1 > 0) {                                         // trailing matrix, K = the whole panel

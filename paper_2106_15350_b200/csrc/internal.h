@@ -19,7 +19,6 @@ struct lbcnn_handle_s {
   int force_simt_expand;            // testing (lbcnn_set_option): keep the expander on the SIMT kernel
   int solver;                       // LBCNN_SOLVER_* (lbcnn_set_option)
   int panel;                        // panel width of the blocked Cholesky when its trailing updates run on tcgen05
-  int inner_tc;                     // ... and whether the 64-column steps inside a panel use them too
   int deflate;                      // ... with the first block column's update kept in fp64 (common-mode deflation)
   int scorer;                       // LBCNN_SCORER_* (lbcnn_set_option)
   int mid_panel;                    // width of the fp64-stepped blocks inside a panel (three-level factorisation); 0 = two levels
