@@ -471,6 +471,8 @@ def run_cuda(args):
         OPTIONS.append((lb.OPT_MID_PANEL, args.mid_panel))
     if args.stream_rows > 0:
         OPTIONS.append((lb.OPT_STREAM_ROWS, args.stream_rows))
+    if args.dual_trick >= 0:
+        OPTIONS.append((lb.OPT_DUAL_TRICK, args.dual_trick))
     if args.scorer:
         OPTIONS.append((lb.OPT_SCORER, {"auto": lb.SCORER_AUTO, "fp64": lb.SCORER_FP64, "tensor": lb.SCORER_TENSOR}[args.scorer]))
 
@@ -547,6 +549,7 @@ def main():
     ap.add_argument("--solver", default="", choices=["", "auto", "fp64", "mixed"], help="LBCNN_OPT_SOLVER (measurement)")
     ap.add_argument("--panel", type=int, default=0, help="LBCNN_OPT_PANEL (measurement)")
     ap.add_argument("--mid-panel", type=int, default=-1, help="LBCNN_OPT_MID_PANEL (measurement)")
+    ap.add_argument("--dual-trick", type=int, default=-1, help="LBCNN_OPT_DUAL_TRICK (measurement)")
     ap.add_argument("--stream-rows", type=int, default=0, help="LBCNN_OPT_STREAM_ROWS: streamed search, samples per chunk")
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")
     ap.add_argument("--no-extras", action="store_true", help="skip the measurements of the SURVEY.md 8(f) rows")

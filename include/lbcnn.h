@@ -106,6 +106,10 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                of the chunks add up (bit-identical to the unstreamed result), the test set is scored chunk by
  *                                chunk, so the features of the whole set never exist and the workspace no longer grows with
  *                                N_train / N_test.  Takes effect on the primal branch with the exact tensor-core Gram; 0 = off
+ *   LBCNN_OPT_DUAL_TRICK         0: the search driver forms W = H^T Z for EVERY candidate of the dual branch and scores H_te W (default 1:
+ *                                when all candidates fit one chunk, train and test features are stacked, the exact Gram of the
+ *                                stack carries the cross-Gram K_te = H_te H^T, the logits K_te (H H^T + I/C)^-1 T come out of the
+ *                                factorisation's appended rows, and W is formed for the best candidate only)
  *   LBCNN_OPT_MID_PANEL          width (multiple of 64; default 256; 0 = none) of the blocks inside a panel whose 64-column steps
  *                                run in fp64; a finished block updates the rest of its panel on the tensor pipe
  *   LBCNN_OPT_PANEL              panel width (multiple of 64, 64..1024; default 1024) of the blocked Cholesky when its trailing
@@ -119,7 +123,7 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
  *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
 enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_DEFLATE = 5,
-       LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7, LBCNN_OPT_STREAM_ROWS = 8 };
+       LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7, LBCNN_OPT_STREAM_ROWS = 8, LBCNN_OPT_DUAL_TRICK = 9 };
 enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };
 int lbcnn_set_option(lbcnn_handle_t h, int option, int value);

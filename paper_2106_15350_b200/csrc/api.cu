@@ -83,7 +83,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->deflate = 16; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->deflate = 16; p->dual_trick = 1; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -108,6 +108,7 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
     case LBCNN_OPT_STREAM_ROWS:
       if (value < 0) return LBCNN_ERR_INVALID_ARG;
       h->stream_rows = value; return LBCNN_OK;
+    case LBCNN_OPT_DUAL_TRICK: h->dual_trick = value ? 1 : 0; return LBCNN_OK;
     case LBCNN_OPT_PANEL:
       if (value < 64 || value > LB_STC_KMAX || value % 64) return LBCNN_ERR_INVALID_ARG;
       h->panel = value; return LBCNN_OK;
@@ -199,11 +200,12 @@ struct SearchPlan {
   FitPlan fit;
   size_t xw_off, fit_off, htr_off, hte_off, w_off, sc_off, total;
   int stream; int64_t ntr_ws, nte_ws;      // streamed: rows of the train / test features resident at once
+  int dual_kt;                             // dual branch scored through the kernel trick: train and test features stacked in one buffer
 };
 // xw1 = expander scratch per candidate (lb_expand_ws_bytes(.., 1)); kc = candidates per chunk
 // sr: streamed search (LBCNN_OPT_STREAM_ROWS) -- at most sr samples of the train / test set are resident at once
 void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, int64_t sr,
-                 SearchPlan* p) {
+                 SearchPlan* p, bool dual_kt = true) {
   lb_fit_plan(n_train, F, c, kc, flags, &p->fit);
   p->stream = (sr > 0 && (sr < n_train || sr < n_test) && p->fit.primal && p->fit.use_tc && p->fit.fuse_rhs) ? 1 : 0;
   if (p->stream) {
@@ -211,11 +213,15 @@ void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, 
     if (sr < n_test) n_test = sr;
   }
   p->ntr_ws = n_train; p->nte_ws = n_test;
+  // dual branch with the exact tensor-core Gram and every candidate in ONE chunk: test rows are stacked behind the train rows,
+  // the Gram of the stack carries the cross-Gram and the scores come out of the factorisation (fit.cu, DualScore)
+  p->dual_kt = (dual_kt && !p->fit.primal && p->fit.use_tc && kc >= n_cand) ? 1 : 0;
+  if (p->dual_kt) lb_fit_plan(n_train, F, c, kc, flags, &p->fit, 0, n_test);
   size_t off = 0;
   p->xw_off = off;  off += (size_t)lb_align_up((int64_t)(xw1 * (size_t)kc), 256);
   p->fit_off = off; off += p->fit.total;
-  p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * n_train * F * 4, 256);
-  p->hte_off = off; off += (size_t)lb_align_up((int64_t)kc * n_test * F * 4, 256);
+  p->htr_off = off; off += (size_t)lb_align_up((int64_t)kc * (n_train + (p->dual_kt ? n_test : 0)) * F * 4, 256);
+  p->hte_off = off; off += p->dual_kt ? 0 : (size_t)lb_align_up((int64_t)kc * n_test * F * 4, 256);
   p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
   // scratch of the tensor-core scorer (integer features only; it may still be left unused at run time)
   p->sc_off = off;  if (flags & LBCNN_H_INTEGER) off += lb_score_tc_ws_bytes(n_test, F, c, kc);
@@ -228,9 +234,10 @@ uint32_t search_fit_flags(const ArchShape& s, bool has_bias) {
   return (!has_bias && s.max_abs <= LB_H_INTEGER_MAX) ? LBCNN_H_INTEGER : 0u;
 }
 // largest chunk size whose plan fits in `bytes` (0 if none)
-int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, int64_t sr, size_t bytes) {
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, int64_t sr, size_t bytes,
+              bool dual_kt = true) {
   SearchPlan p;
-  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, sr, &p);
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, sr, &p, dual_kt);
   if (p.total <= bytes) return n_cand;
   int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
   while (hi - lo > 1) {
@@ -267,8 +274,10 @@ int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_
     kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, sr, budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0);
     if (kc < 1) kc = 1;
   }
-  SearchPlan p;
+  SearchPlan p, pn;
   plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, &pn, false);   // LBCNN_OPT_DUAL_TRICK off: the larger one fits both
+  if (pn.total > p.total) p = pn;
   if (min_bytes) *min_bytes += LB_WS_HEAD;
   *bytes = p.total + LB_WS_HEAD;
   return LBCNN_OK;
@@ -389,11 +398,12 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   const uint32_t fflags = search_fit_flags(s, d_bias != nullptr);
   const size_t xw1 = lb_expand_ws_bytes(h, s, d_bias != nullptr, 1);
   const int64_t sr = h->stream_rows;
-  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, sr, ws_bytes);
+  const bool want_kt = h->dual_trick != 0 && h->scorer != LBCNN_SCORER_FP64;
+  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, sr, ws_bytes, want_kt);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
   if (kc > 65535) kc = 65535;                          // grid.y / grid.z of the batched kernels
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, sr, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, sr, &p, want_kt);
   char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
@@ -411,6 +421,23 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
                           lb_score_tc_usable(Hte, p.nte_ws, s.F, n_classes, kn) &&
                           (h->scorer == LBCNN_SCORER_TENSOR || lb_score_tc_worthwhile(n_test, s.F, n_classes, kn));
     FitPlan fp;
+    if (p.dual_kt) {
+      // dual branch through the kernel trick: one buffer [candidate][train rows | test rows][F]; the exact Gram of the stack
+      // holds the cross-Gram H_te U^T, the factorisation turns it into the logits (fit.cu); W only for the best, afterwards
+      const int64_t n_all = n_train + n_test;
+      lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, 0, n_test);
+      rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st, false, n_all);
+      if (rc) return rc;
+      rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Htr + n_train * s.F, base + p.xw_off, xw1 * (size_t)kn, st, true, n_all);
+      if (rc) return rc;
+      const DualScore dsc{d_test_labels, d_correct + k0};
+      rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn, Wk, d_info + k0, st, nullptr, &dsc);
+      if (rc) return rc;
+      rc = lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, nullptr, wel, nullptr, st);
+      if (rc) return rc;
+      if (d_W_best) return lb_launch_w_best_dual(h, base + p.fit_off, fp, d_best, Htr, n_train, s.F, hs, n_classes, d_W_best, st);
+      return LBCNN_OK;
+    }
     lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, p.ntr_ws);
     // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale.
     // Streamed ("limited GPU-RAM"): the train set passes through in chunks of

@@ -33,6 +33,7 @@ struct ExpandParams {
   int w_words, b_words;
   long long F;
   long long n;
+  long long out_rows;   // rows per candidate of the output buffer (>= n)
   float scale;
   const uint8_t* img;
   const int8_t* ker;
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(256) expand_kernel(const ExpandParams p) {
         sb[L.sb_off + t] = p.bias ? p.bias[(long long)kc * p.n_bias + L.b_off + t] : 0;
     }
     __syncthreads();
-    float* Hrow = p.H + ((long long)kc * p.n + img_idx) * p.F;
+    float* Hrow = p.H + ((long long)kc * p.out_rows + img_idx) * p.F;
     for (int l = 0; l < p.n_layers; ++l) {
       const LayerDev& L = p.L[l];
       const bool last = (l == p.n_layers - 1);
@@ -184,9 +185,9 @@ size_t lb_expand_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_
 
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, void* xw, size_t xw_bytes,
-                     cudaStream_t st, bool prepared) {
+                     cudaStream_t st, bool prepared, int64_t out_rows) {
   if (!h->force_simt_expand && lb_expand_tc_usable(h, s, d_bias != nullptr))
-    return lb_launch_expand_tc(h, s, feature_scale, d_images, n, d_kernels, n_cand, d_H, xw, xw_bytes, st, prepared);
+    return lb_launch_expand_tc(h, s, feature_scale, d_images, n, d_kernels, n_cand, d_H, xw, xw_bytes, st, prepared, out_rows);
   LbPhase ph(h, LBCNN_PHASE_EXPAND, st);
   ExpandParams p{};
   p.n_layers = s.n_layers;
@@ -218,7 +219,7 @@ int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale,
   p.n_cand = n_cand;
   p.cand_per_block = n_cand < 8 ? n_cand : 8;
   p.n_weights = (int)s.n_weights; p.n_bias = (int)s.n_bias;
-  p.F = s.F; p.n = n; p.scale = feature_scale;
+  p.F = s.F; p.n = n; p.out_rows = out_rows > 0 ? out_rows : n; p.scale = feature_scale;
   p.img = d_images; p.ker = d_kernels; p.bias = d_bias; p.H = d_H;
   int threads = (max_items + 31) / 32 * 32;
   if (threads < 64) threads = 64;

@@ -39,6 +39,7 @@ constexpr int XT_THREADS = XT_WARPS * 32;
 
 struct XtcParams {
   const uint8_t* img; long long n_img; int H, W, C;
+  long long out_rows;            // rows per candidate of the output buffer (>= n_img: train and test features stacked)
   const uint8_t* wblob; int blob_bytes, w1_bytes, w2_bytes;   // per candidate: [B1 image | B2 image]
   int n_cand, cand_per_cta;
   float* Hout; long long F; float scale;
@@ -209,8 +210,8 @@ __device__ __forceinline__ void e1_single(const XtcParams& p, const uint8_t* sme
   const int32_t* tab1 = reinterpret_cast<const int32_t*>(smem + p.off_tab1) + quad * 32 + lane;
   const uint32_t taddr0 = tmem + lane_base + p.tm_r1;
   const uint32_t bar_full0 = bar_addr(bars, R1_FULL), bar_empty0 = bar_addr(bars, R1_EMPTY);
-  const long long cand_stride = p.n_img * p.F;
-  float* Hb = p.Hout + ((long long)c_begin * p.n_img + img0) * p.F;
+  const long long cand_stride = p.out_rows * p.F;
+  float* Hb = p.Hout + ((long long)c_begin * p.out_rows + img0) * p.F;
   for (int ci = 0; ci < n_cta_cand; ++ci, Hb += cand_stride) {
     for (int t1 = 0; t1 < T1; ++t1) {
       const int n1 = ci * T1 + t1;
@@ -286,8 +287,8 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
   const uint32_t hw = (uint32_t)(p.Ho2 * p.Wo2);
   const float scale = p.scale;
   const uint32_t taddr = tmem + lane_base + p.tm_r2 + set * (nph2 * N2);
-  const long long cand_stride = p.n_img * p.F;
-  float* Hb = p.Hout + ((long long)c_begin * p.n_img + img0) * p.F;
+  const long long cand_stride = p.out_rows * p.F;
+  float* Hb = p.Hout + ((long long)c_begin * p.out_rows + img0) * p.F;
   for (int ci = 0; ci < n_cta_cand; ++ci, Hb += cand_stride) {
     for (int t2 = 0; t2 < T2; ++t2) {
       const int n2 = ci * T2 + t2;
@@ -734,7 +735,7 @@ size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool h
 
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                         const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st,
-                        bool prepared) {
+                        bool prepared, int64_t out_rows) {
   XtcParams p; size_t smem = 0;
   if (!plan_xtc(h, s, false, &p, &smem)) return LBCNN_ERR_INVALID_ARCH;
   if (n_cand > 65535) return LBCNN_ERR_INVALID_ARG;
@@ -755,7 +756,7 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
     LB_CUDA_OK(cudaGetLastError());
   }
   p.img = d_images; p.n_img = n; p.wblob = reinterpret_cast<const uint8_t*>(xw); p.n_cand = n_cand;
-  p.Hout = d_H; p.F = s.F; p.scale = feature_scale;
+  p.Hout = d_H; p.F = s.F; p.scale = feature_scale; p.out_rows = out_rows > 0 ? out_rows : n;
   const long long batches = (n + p.B - 1) / p.B;
   // candidates per CTA: as many as possible (they share the staged images and A1) while the grid still
   // covers the SMs about four times over

@@ -234,17 +234,72 @@ __global__ void w_from_xt_kernel(const double* __restrict__ A, long long a_strid
   W[z * dim * c + t] = (float)(A[z * a_stride + (dim + cls) * dim + f] * inv_s);
 }
 
+// dual branch, kernel trick: class = first maximum of a row of logits [n_te][c] (fp64); one warp per 32 rows
+__global__ void __launch_bounds__(256) dual_argmax_kernel(const double* __restrict__ logits, long long n_te, int c,
+                                                          const int32_t* __restrict__ y, int32_t* __restrict__ correct) {
+  const long long z = blockIdx.y;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int ok = 0;
+  if (i < n_te) {
+    const double* l = logits + (z * n_te + i) * c;
+    double best = l[0]; int bi = 0;
+    for (int j = 1; j < c; ++j) { const double v = l[j]; if (v > best) { best = v; bi = j; } }
+    ok = (y[i] == bi) ? 1 : 0;
+  }
+  ok = __reduce_add_sync(0xffffffffu, ok);
+  if ((threadIdx.x & 31) == 0 && ok) atomicAdd(&correct[z], ok);
+}
+
+// W of the best candidate only (its index is read on the device): W[f][cls] = (1/s) sum_n U[n][f] Z^T[cls][n]
+__global__ void __launch_bounds__(128) w_best_dual_kernel(const int32_t* __restrict__ best, const float* __restrict__ Hall,
+                                                          long long n, long long n_rows, long long F, const double* __restrict__ A,
+                                                          long long a_stride, long long ld, long long dim, int c, double inv_s,
+                                                          float* __restrict__ W) {
+  const long long z = best[0];
+  const long long f = (long long)blockIdx.x * 128 + threadIdx.x;
+  const int c0 = blockIdx.y * 8;
+  if (f >= F) return;
+  const float* U = Hall + z * n_rows * F + f;
+  const double* Zt = A + z * a_stride + (dim + c0) * ld;
+  double acc[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+  const int nc = (c - c0 < 8) ? c - c0 : 8;
+  for (long long i = 0; i < n; ++i) {
+    const double u = (double)U[i * F];
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      if (q < nc) acc[q] = fma(u, Zt[q * ld + i], acc[q]);
+  }
+#pragma unroll
+  for (int q = 0; q < 8; ++q)
+    if (q < nc) W[f * c + c0 + q] = (float)(acc[q] * inv_s);
+}
+
 }  // namespace
 
+int lb_launch_w_best_dual(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const int32_t* d_best, const float* d_Hall, int64_t n,
+                          int64_t F, float h_scale, int n_classes, float* d_W_best, cudaStream_t st) {
+  double* A = reinterpret_cast<double*>(reinterpret_cast<char*>(ws) + pl.a_off);
+  dim3 grid((unsigned)((F + 127) / 128), (unsigned)((n_classes + 7) / 8));
+  w_best_dual_kernel<<<grid, 128, 0, st>>>(d_best, d_Hall, n, n + pl.n_extra, F, A, pl.rows * pl.dim, pl.dim, pl.dim, n_classes,
+                                           1.0 / (double)h_scale, d_W_best);
+  h->launches += 1;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
-void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws) {
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws, int64_t n_extra) {
   if (n_ws <= 0 || n_ws > n) n_ws = n;
   int primal = (F < n) ? 1 : 0;                       // PAPER.md:68 `if n_inputs<Ntr` ('LLL'), else 'MMM'
   if (flags & LBCNN_FORCE_PRIMAL) primal = 1;
   if (flags & LBCNN_FORCE_DUAL) primal = 0;
   p->primal = primal;
   p->dim = primal ? F : n;
-  p->rows = p->dim + n_classes;
+  p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
+  p->n_extra = (!primal && p->use_tc && n_extra > 0) ? n_extra : 0;
+  p->rows = p->dim + n_classes + p->n_extra;
   p->a_bytes = (size_t)p->rows * (size_t)p->dim * sizeof(double);
   size_t off = 0;
   p->perm_off = off; off += (size_t)lb_align_up(n * 4, 256);
@@ -252,7 +307,8 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
   p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
   p->tc_off = off;   p->fuse_rhs = (p->use_tc && primal && lb_gram_tc_fuse_rhs(F, n_classes)) ? 1 : 0;
-  if (p->use_tc) off += lb_gram_tc_ws_bytes(n_ws, F, n_cand, p->fuse_rhs ? n_classes : 0);
+  if (p->use_tc) off += lb_gram_tc_ws_bytes(n_ws + p->n_extra, F, n_cand, p->fuse_rhs ? n_classes : 0);
+  p->lg_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * p->n_extra * n_classes * 8, 256);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   // digit planes + row scales of the tensor-core trailing updates (chol_tc.cu), for systems large enough to have them
   p->stc_kmax = (p->dim >= LB_STC_MIN_DIM) ? LB_STC_KMAX : 0;
@@ -263,7 +319,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
 
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d_H, int64_t n, int64_t F, float h_scale,
                   const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
-                  cudaStream_t st, const FitStream* fs) {
+                  cudaStream_t st, const FitStream* fs, const DualScore* ds) {
   char* base = reinterpret_cast<char*>(ws);
   int32_t* perm = reinterpret_cast<int32_t*>(base + pl.perm_off);
   int32_t* off = reinterpret_cast<int32_t*>(base + pl.off_off);
@@ -320,7 +376,8 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     {
     LbPhase ph(h, LBCNN_PHASE_GRAM, st);
     if (pl.use_tc) {
-      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, nullptr, 0, d_info, st);
+      rc = lb_launch_gram_tc(h, base + pl.tc_off, d_H, n, F, n_cand, lam, A, a_stride, ld, false, nullptr, 0, d_info, st, false, true,
+                             n + pl.n_extra, c);
       if (rc) return rc;
     } else {
     GemmP g{};
@@ -425,6 +482,27 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
       if (rc) return rc;
     }
   }
+  if (ds && pl.n_extra > 0) {
+    // kernel trick (dual branch): the appended rows now hold Y_T = (L^-1 T)^T (c rows) and Y_te = (L^-1 K_te^T)^T (n_extra
+    // rows, K_te = H_te U^T the exact cross-Gram), so  logits = K_te A^-1 T = Y_te Y_T^T  -- no W, no pass over H_te
+    ph3.stop();
+    {
+      LbPhase phs(h, LBCNN_PHASE_SCORE, st);
+      double* lg = reinterpret_cast<double*>(base + pl.lg_off);
+      GemmP g{};
+      g.A = A + (dim + c) * ld; g.sAr = ld; g.sAk = 1; g.bA = a_stride;
+      g.B = A + dim * ld; g.sBr = ld; g.sBk = 1; g.bB = a_stride;
+      g.C = lg; g.ldc = c; g.bC = pl.n_extra * c;
+      g.M = (int)pl.n_extra; g.N = c; g.K = (int)dim; g.alpha = 1.0; g.accumulate = 0; g.lower = 0; g.diag = 0.0;
+      rc = launch_gemm<double, double, double, true, true>(h, g, n_cand, st);
+      if (rc) return rc;
+      LB_CUDA_OK(cudaMemsetAsync(ds->correct, 0, (size_t)n_cand * 4, st));
+      dim3 ga((unsigned)((pl.n_extra + 255) / 256), (unsigned)n_cand);
+      dual_argmax_kernel<<<ga, 256, 0, st>>>(lg, pl.n_extra, c, ds->te_labels, ds->correct);
+      h->launches += 1;
+    }
+  }
+  LbPhase ph4(h, LBCNN_PHASE_SOLVE, st, ds && pl.n_extra > 0);      // a second bracket only when the scoring above split the phase
   // backward sweep on the appended rows: X^T L = Y^T, block columns from the last to the first;
   // the diagonal step is X_j = Y_j L_jj^-1 (a product with the stored inverse)
   for (long long jb = nblk - 1; jb >= 0; --jb) {
@@ -455,7 +533,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
     dim3 gw((unsigned)((dim * c + 255) / 256), 1, (unsigned)n_cand);
     w_from_xt_kernel<<<gw, 256, 0, st>>>(A, a_stride, dim, c, 1.0 / s, d_W);
     h->launches += 1;
-  } else {
+  } else if (!(ds && pl.n_extra > 0)) {
     // W[f][cls] = (1/s) sum_n U[n][f] Z^T[cls][n]
     GemmP g{};
     g.A = d_H; g.sAr = 1; g.sAk = F; g.bA = n * F;

@@ -45,6 +45,7 @@ struct GramTcParams {
   double lam;
   unsigned long long* ops;   // int8 multiply-adds issued (measurement)
   int accumulate;            // A += G (a further chunk of samples of a streamed Gram) instead of A = G
+  int rshift;                // output rows >= Fcols are stored rshift rows further down (dual: cross-Gram rows behind the right-hand sides)
   int add_lam;               // ... + lam I (the last chunk: (G1 + G2 + ..) + lam rounds like the unstreamed G + lam)
 };
 
@@ -349,7 +350,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) gram_tc_kernel(const __grid_const
     tc::mbar_wait(tc::smem_u32(&bar_tmem), 0);
     tc::tc_fence_after();
     const int i = i0 + q * 32 + lane;
-    double* Arow = p.A + (long long)z * p.a_stride + (long long)i * p.ld;
+    double* Arow = p.A + (long long)z * p.a_stride + (long long)(i + (i >= p.Fcols ? p.rshift : 0)) * p.ld;
     const int nacc = Li + Lj - 1;
     for (int c0 = 0; c0 < TN; c0 += 16) {
       uint32_t r[5][16];
@@ -425,13 +426,16 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {
 // (U^T T)^T, T the one-hot coding of the labels (the appended right-hand-side rows of the Cholesky layout).
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
                       long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
-                      cudaStream_t st, bool accumulate, bool add_lam) {
+                      cudaStream_t st, bool accumulate, bool add_lam, int64_t n_rows, int rshift) {
+  // dual branch with n_rows > n: the planes hold n_rows samples per candidate (train rows, then test rows); the output has
+  // n_rows rows x n columns -- the n x n system matrix and, in rows n.., the cross-Gram of the test with the train samples
+  if (n_rows <= 0 || primal) n_rows = n;
   EncodeTiledFn enc = get_encode();
   if (!enc) return LBCNN_ERR_CUDA;
   const int c_aug = (primal && d_labels && lb_gram_tc_fuse_rhs(F, n_classes)) ? n_classes : 0;
   const int64_t Fp = lb_gram_tc_fp(F, c_aug);
   int8_t* planes = reinterpret_cast<int8_t*>(ws);
-  int32_t* nlimb = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + lb_align_up((int64_t)n_cand * 3 * n * Fp, 256));
+  int32_t* nlimb = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + lb_align_up((int64_t)n_cand * 3 * n_rows * Fp, 256));
   const int G32 = (int)((Fp + 31) / 32);
   int32_t* nl32 = nlimb + n_cand;                  // [n_cand][G32] right behind the per-candidate counts
   const int n_counts = n_cand * (1 + G32);
@@ -440,15 +444,15 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   fill_i32_kernel<<<(nfill + 255) / 256, 256, 0, st>>>(nlimb, n_counts, 1, accumulate ? nullptr : d_info, n_cand);
   h->launches += 1;
   {
-    const long long work = n * (Fp / 8);
+    const long long work = n_rows * (Fp / 8);
     dim3 grid((unsigned)((work + 255) / 256), (unsigned)n_cand);
-    split_kernel<<<grid, 256, 0, st>>>(d_U, n, (int)F, (int)Fp, planes, nlimb, nl32, G32, d_info, d_labels, c_aug);
+    split_kernel<<<grid, 256, 0, st>>>(d_U, n_rows, (int)F, (int)Fp, planes, nlimb, nl32, G32, d_info, d_labels, c_aug);
     h->launches += 1;
   }
   LB_CUDA_OK(cudaGetLastError());
   CUtensorMap tmap, tmapB;
-  const cuuint64_t gdim[3] = {(cuuint64_t)(F + c_aug), (cuuint64_t)n, (cuuint64_t)n_cand * 3};
-  const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)n * Fp};
+  const cuuint64_t gdim[3] = {(cuuint64_t)(F + c_aug), (cuuint64_t)n_rows, (cuuint64_t)n_cand * 3};
+  const cuuint64_t gstr[2] = {(cuuint64_t)Fp, (cuuint64_t)n_rows * Fp};
   const cuuint32_t box[3] = {BOXW, KS, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
   if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, planes, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -465,7 +469,8 @@ int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, 
   }
   GramTcParams p{};
   p.nlimb = nlimb; p.nl32 = nl32; p.G32 = G32; p.A = A; p.a_stride = a_stride; p.ld = ld; p.dual = primal ? 0 : 1;
-  const int64_t odim = primal ? F + c_aug : n, ocols = primal ? F : n;
+  const int64_t odim = primal ? F + c_aug : n_rows, ocols = primal ? F : n;
+  p.rshift = rshift;
   p.Fcols = (int)ocols; p.ops = lb_ws_counter(h, 0); p.accumulate = accumulate ? 1 : 0; p.add_lam = add_lam ? 1 : 0;
   p.F = (int)odim; p.n = (int)n; p.n_iters = primal ? (int)((n + KS - 1) / KS) : (int)((F + 127) / 128); p.lam = lam;
   const size_t smem = (size_t)RING_BYTES + 1024;

@@ -23,6 +23,7 @@ struct lbcnn_handle_s {
   int scorer;                       // LBCNN_SCORER_* (lbcnn_set_option)
   int mid_panel;                    // width of the fp64-stepped blocks inside a panel (three-level factorisation); 0 = two levels
   int64_t stream_rows;              // search driver: samples expanded / accumulated per chunk (0 = all at once)
+  int dual_trick;                   // search driver, dual branch: score through the cross-Gram (kernel trick), W for the best only
   int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
@@ -31,10 +32,11 @@ struct lbcnn_handle_s {
 // RAII phase marker: records start/stop events on the stream when profiling is on
 struct LbPhase {
   lbcnn_handle_s* h; cudaStream_t st; LbPhaseRec r; bool on;
-  LbPhase(lbcnn_handle_s* h_, int phase, cudaStream_t st_) : h(h_), st(st_), on(h_->profiling != 0) {
+  LbPhase(lbcnn_handle_s* h_, int phase, cudaStream_t st_, bool enable = true) : h(h_), st(st_), on(h_->profiling != 0 && enable) {
     if (on) { r.phase = phase; cudaEventCreate(&r.start); cudaEventCreate(&r.stop); cudaEventRecord(r.start, st); }
   }
-  ~LbPhase() { if (on) { cudaEventRecord(r.stop, st); h->recs.push_back(r); } }
+  void stop() { if (on) { cudaEventRecord(r.stop, st); h->recs.push_back(r); on = false; } }
+  ~LbPhase() { stop(); }
 };
 
 #define LB_CUDA_OK(expr)                                  \
@@ -79,14 +81,14 @@ size_t lb_expand_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_
 // set with the same kernel sets): the re-layout kernel is not launched again
 int lb_launch_expand(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                      const int8_t* d_kernels, const int32_t* d_bias, int n_cand, float* d_H, void* xw, size_t xw_bytes,
-                     cudaStream_t st, bool prepared = false);
+                     cudaStream_t st, bool prepared = false, int64_t out_rows = 0);   // out_rows: rows per candidate of d_H (0 = n)
 
 // tensor-core expander (expand_tc.cu): FULL convolutions, non-overlapping pooling, 1-2 layers, no bias
 bool lb_expand_tc_usable(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias);
 size_t lb_expand_tc_ws_bytes(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias, int n_cand);
 int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_scale, const uint8_t* d_images, int64_t n,
                         const int8_t* d_kernels, int n_cand, float* d_H, void* xw, size_t xw_bytes, cudaStream_t st,
-                        bool prepared = false);
+                        bool prepared = false, int64_t out_rows = 0);
 
 // ---- fit (fit.cu) --------------------------------------------------------------------------
 struct FitPlan {
@@ -95,17 +97,24 @@ struct FitPlan {
   int64_t rows;          // dim + n_classes (right-hand sides appended as rows)
   size_t a_bytes;        // per candidate: rows * dim doubles
   size_t perm_off, off_off, a_off, tc_off, linv_off, stc_off, total; // offsets inside the fit workspace
+  int64_t n_extra;       // dual branch, search driver: test samples stacked behind the train samples (cross-Gram rows in A)
+  size_t lg_off;         // ... and their logits [n_cand][n_extra][n_classes] fp64
   int stc_kmax;          // widest panel the tensor-core trailing update is planned for (0: no scratch reserved)
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
   int fuse_rhs;          // ... which then also produces the right-hand side (one-hot label columns)
 };
 // n_ws: rows of H resident at once (streamed Gram: the digit planes are sized for one chunk of samples); 0 = n
-void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws = 0);
+void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags, FitPlan* p, int64_t n_ws = 0, int64_t n_extra = 0);
 // streamed fit: stage 1 = add one chunk of samples to the Gram (+ fused right-hand side), stage 2 = solve
 struct FitStream { int stage; int first_chunk; int last_chunk; };
+// dual branch scored through the kernel trick (plan.n_extra test rows stacked behind the train rows of d_H): logits =
+// (H_te U^T) Z come out of the factorisation's appended rows; W is not formed for every candidate
+struct DualScore { const int32_t* te_labels; int32_t* correct; };
+int lb_launch_w_best_dual(lbcnn_handle_s* h, void* ws, const FitPlan& p, const int32_t* d_best, const float* d_Hall, int64_t n,
+                          int64_t F, float h_scale, int n_classes, float* d_W_best, cudaStream_t st);
 int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_H, int64_t n, int64_t F, float h_scale,
                   const int32_t* d_labels, int n_classes, float C, int n_cand, float* d_W, int32_t* d_info,
-                  cudaStream_t st, const FitStream* fs = nullptr);
+                  cudaStream_t st, const FitStream* fs = nullptr, const DualScore* ds = nullptr);
 
 // ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
 bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
@@ -113,7 +122,8 @@ size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug);
 bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-hot columns of the Gram's digit plane 0
 int lb_launch_gram_tc(lbcnn_handle_s* h, void* ws, const float* d_U, int64_t n, int64_t F, int n_cand, double lam, double* A,
                       long long a_stride, long long ld, bool primal, const int32_t* d_labels, int n_classes, int32_t* d_info,
-                      cudaStream_t st, bool accumulate = false, bool add_lam = true);   // streamed: A += this chunk's Gram; ridge with the last chunk
+                      cudaStream_t st, bool accumulate = false, bool add_lam = true,    // streamed: A += this chunk's Gram; ridge with the last chunk
+                      int64_t n_rows = 0, int rshift = 0);   // dual: n_rows >= n samples in H (test rows behind the train rows)
 
 constexpr int LB_STC_KMAX = 1024;      // widest panel (digit-plane pitch)
 constexpr int LB_STC_MIN_DIM = 512;    // systems below this never reserve the scratch

@@ -565,6 +565,31 @@ def test_streamed_search_equals_resident(handle, name, ntr, nte, K, rows):
     handle.set_workspace(None)
 
 
+@pytest.mark.parametrize("name,ntr,nte,K", [("orl", 280, 120, 16), ("vggface", 700, 300, 3), ("paper_anchor", 300, 200, 2)])
+def test_dual_branch_kernel_trick_equals_explicit_w(handle, name, ntr, nte, K):
+    """dual branch (F >= N): by default the driver scores through the cross-Gram -- logits =
+    (H_te H^T)(H H^T + I/C)^-1 T out of the factorisation's appended rows, W only for the best candidate; with
+    LBCNN_OPT_DUAL_TRICK = 0 it forms W = H^T Z for every candidate and scores H_te W.  Same mathematics: identical
+    counts, best / worst, and W_best equal up to the rounding order of its fp64 sums."""
+    w = _small(name, ntr, nte, K)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    handle.set_workspace(None)
+    handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+    args = (arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    a = {k: v.clone() for k, v in handle.search_candidates(*args).items()}
+    try:
+        handle.set_option(lb.OPT_DUAL_TRICK, 0)
+        b = handle.search_candidates(*args)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_option(lb.OPT_DUAL_TRICK, 1)
+    for k in ("acc", "correct", "info", "best"):
+        assert torch.equal(a[k], b[k]), k
+    assert _fro(a["W_best"].cpu().numpy().astype(np.float64), b["W_best"].cpu().numpy().astype(np.float64)) <= 1e-6
+
+
 def test_search_chunked_equals_unchunked(handle):
     w = _small("mnist", 400, 150, 7)
     arch = lb.arch_of(w)
