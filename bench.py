@@ -45,7 +45,7 @@ if ROOT not in sys.path:
 
 # cpu_baseline sample per workload: (candidates, N_train, N_test), sized for about 10-30 s of host work
 CPU_SAMPLE = {"tiny_mnist": (8, 2000, 500), "mnist": (10, 20000, 10000), "orl": (32, 280, 120),
-              "gtsrb": (1, 3000, 1263), "vggface": (1, 1000, 250)}
+              "gtsrb": (1, 3000, 1263), "vggface": (1, 1000, 250), "paper_table1": (1, 1000, 500)}
 
 METRIC = "ELM candidate kernel-sets evaluated/sec (expand+fit+score); % HBM & tensor roofline"
 UNIT = "candidates/s"
@@ -219,8 +219,9 @@ def run_reference(args):
 
 
 def _config(w, n_cand, l2_note):
-    return dict(workload="BASELINE.json configs[%d] (%s): %dx%dx%d u8, N_train=%d N_test=%d classes=%d, layers=%s, C=%g"
-                % (w.config - 1, w.name, w.in_h, w.in_w, w.in_c, w.n_train, w.n_test, w.n_classes,
+    origin = ("BASELINE.json configs[%d]" % (w.config - 1)) if w.config <= 5 else "paper Table I shape (PAPER.md:104-113), not a BASELINE config"
+    return dict(workload="%s (%s): %dx%dx%d u8, N_train=%d N_test=%d classes=%d, layers=%s, C=%g"
+                % (origin, w.name, w.in_h, w.in_w, w.in_c, w.n_train, w.n_test, w.n_classes,
                    "+".join("%d@%dx%d/pool%d" % (L.n_kernels, L.ksize, L.ksize, L.pool_k) for L in w.layers), w.C),
                 candidates_per_step=n_cand, parallelism="replicas only (candidates independent; no collective)",
                 l2=l2_note)
@@ -540,7 +541,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="mnist", choices=["tiny_mnist", "mnist", "gtsrb", "orl", "vggface"])
+    ap.add_argument("--workload", default="mnist", choices=["tiny_mnist", "mnist", "gtsrb", "orl", "vggface", "paper_table1"])
     ap.add_argument("--n-cand", type=int, default=0, help="override the workload's candidate count (not a bench line)")
     ap.add_argument("--ws-gb", type=float, default=100.0, help="workspace budget; candidates are chunked to fit")
     ap.add_argument("--ref-cands", type=int, default=1, help="--impl reference: candidates per step")

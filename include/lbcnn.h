@@ -94,11 +94,14 @@ int lbcnn_destroy(lbcnn_handle_t h);
 
 /* Options (testing and measurement; the defaults are the product path).
  *   LBCNN_OPT_FORCE_SIMT_EXPAND  1: lbcnn_expand always takes the exact int32 SIMT kernel
- *   LBCNN_OPT_SOLVER             LBCNN_SOLVER_AUTO: F3 picks per system size; _FP64: blocked fp64 Cholesky only;
- *                                _MIXED: the trailing updates of the blocked factorisation run on tcgen05 as int8 digit
- *                                products of the row-scaled panel (four balanced radix-256 digits, ten of the sixteen digit
- *                                products: ~2^-27 relative, against 2^-24 of an fp32 factorisation) whenever the system has
- *                                a trailing update; the matrix, the diagonal blocks and the panel solves stay fp64
+ *   LBCNN_OPT_SOLVER             LBCNN_SOLVER_AUTO: lbcnn_search_candidates runs the trailing updates of the blocked factorisation on
+ *                                tcgen05 (int8 digit products of the row-scaled panel: four balanced radix-256 digits, ten of the
+ *                                sixteen digit products, ~2^-27 relative against 2^-24 of an fp32 factorisation) for systems of
+ *                                dimension >= 1024 whose architecture cannot produce identical or negated feature maps (last layer
+ *                                FULL with >= 32 taps per kernel); everything else, and lbcnn_elm_fit on data it knows nothing
+ *                                about, takes the all-fp64 factorisation.  _FP64: all-fp64 everywhere.  _MIXED: tensor-core
+ *                                updates whenever the system has a trailing update -- the caller vouches that the system is not
+ *                                singular up to the ridge (cond * 2^-27 << 1)
  *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
  *                                captured CUDA graph (default 1)
  *   LBCNN_OPT_STREAM_ROWS        r > 0: streamed search ("limited GPU-RAM ... reduced fraction of the training
@@ -142,8 +145,9 @@ int lbcnn_kernel_set_size(const lbcnn_arch_t* arch, int64_t* n_weights, int64_t*
  * stays owned by the caller and must outlive every call enqueued with it. */
 int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_train, int64_t n_test,
                           int32_t n_classes, int32_t n_cand, size_t budget_bytes, size_t* bytes, size_t* min_bytes);
-/* d_ws: 256-byte aligned, at least 256 bytes (its first 256 bytes are zeroed on the default stream: the
- * measurement counters of lbcnn_get_op_stats), or NULL with bytes = 0 to detach. */
+/* d_ws: 256-byte aligned, at least 256 bytes (its first 256 bytes are zeroed with a blocking cudaMemset: the
+ * measurement counters of lbcnn_get_op_stats), or NULL with bytes = 0 to detach.  A configuration call, not stream-ordered:
+ * do not call it while work enqueued with the previous workspace is still running. */
 int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes);
 /* Workspace a stand-alone lbcnn_elm_fit(n, F, n_classes, n_cand, flags) needs (host-only arithmetic). */
 int lbcnn_fit_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, uint32_t flags, size_t* bytes);

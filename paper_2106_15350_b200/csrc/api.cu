@@ -177,7 +177,7 @@ int lbcnn_set_workspace(lbcnn_handle_t h, void* d_ws, size_t bytes) {
   if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0) return LBCNN_ERR_INVALID_ARG;
   if (d_ws && bytes < LB_WS_HEAD) return LBCNN_ERR_INVALID_ARG;
   h->ws = d_ws; h->ws_bytes = bytes;
-  if (d_ws) LB_CUDA_OK(cudaMemsetAsync(d_ws, 0, LB_WS_HEAD, 0));     // the measurement counters at the head of the workspace
+  if (d_ws) LB_CUDA_OK(cudaMemset(d_ws, 0, LB_WS_HEAD));     // the measurement counters at the head of the workspace (a configuration call: blocking)
   return LBCNN_OK;
 }
 
@@ -230,6 +230,16 @@ void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, 
 // The driver's features are exact integers; inside the digit envelope of the exact tensor-core Gram (three balanced
 // radix-256 digits hold |u| <= 8355711) the fit may use it.  A bias is an arbitrary int32 and is not part of the bound,
 // so a search with bias keeps the general fp64 Gram.
+// The tensor-core Cholesky updates carry ~2^-27 relative error: fine for the conditioning of distinct random features
+// (cond ~1e6), fatal for a system that is singular up to the ridge -- two identical or negated feature maps.  That happens
+// when two +-1 kernels of the LAST layer coincide: with t = Cin k^2 taps the chance per pair is 2^(1-t).  A depthwise last
+// layer (t = k^2 = 9: about every second candidate of the paper's (16,20) architecture) or a tiny full one must keep the
+// all-fp64 solver; from 32 taps on (configs[2], [4]: 144) the chance is below 1e-9 per pair.
+bool arch_allows_tc_solver(const ArchShape& s) {
+  const LayerShape& L = s.L[s.n_layers - 1];
+  return L.conv_type == LBCNN_CONV_FULL && (int64_t)L.cin * L.k * L.k >= 32;
+}
+
 uint32_t search_fit_flags(const ArchShape& s, bool has_bias) {
   return (!has_bias && s.max_abs <= LB_H_INTEGER_MAX) ? LBCNN_H_INTEGER : 0u;
 }
@@ -426,6 +436,7 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
       // holds the cross-Gram H_te U^T, the factorisation turns it into the logits (fit.cu); W only for the best, afterwards
       const int64_t n_all = n_train + n_test;
       lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, 0, n_test);
+      fp.allow_tc = arch_allows_tc_solver(s) ? 1 : 0;
       rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, ker, bias, kn, Htr, base + p.xw_off, xw1 * (size_t)kn, st, false, n_all);
       if (rc) return rc;
       rc = lb_launch_expand(h, s, 1.0f, d_test, n_test, ker, bias, kn, Htr + n_train * s.F, base + p.xw_off, xw1 * (size_t)kn, st, true, n_all);
@@ -439,6 +450,7 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
       return LBCNN_OK;
     }
     lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, p.ntr_ws);
+    fp.allow_tc = arch_allows_tc_solver(s) ? 1 : 0;
     // E1-E4 with scale 1: H holds the exact integers; the scale enters the fit and the score as h_scale.
     // Streamed ("limited GPU-RAM"): the train set passes through in chunks of
     // ntr_ws samples whose exact integer Grams (and fused right-hand sides) add up in A -- H of the whole set never exists.

@@ -311,6 +311,7 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->lg_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * p->n_extra * n_classes * 8, 256);
   p->linv_off = off; off += (size_t)lb_align_up((int64_t)n_cand * ((p->dim + NB - 1) / NB) * NB * NB * 8, 256);
   // digit planes + row scales of the tensor-core trailing updates (chol_tc.cu), for systems large enough to have them
+  p->allow_tc = 0;
   p->stc_kmax = (p->dim >= LB_STC_MIN_DIM) ? LB_STC_KMAX : 0;
   p->stc_off = off;
   if (p->stc_kmax) off += lb_chol_tc_ws_bytes(p->rows, n_cand, p->stc_kmax);
@@ -407,7 +408,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& pl, const float* d
   // which cuts its read-modify-write traffic by NBO / NB.
   // With the tensor-core trailing update (chol_tc.cu) the wide update costs ~1/10 of its fp64 time, so the panel is made
   // wider (its read-modify-write traffic on the trailing matrix falls with 1/NBO).
-  const bool tc_solve = pl.stc_kmax > 0 && (h->solver == LBCNN_SOLVER_MIXED || (h->solver == LBCNN_SOLVER_AUTO && dim >= LB_STC_AUTO_DIM));
+  const bool tc_solve = pl.stc_kmax > 0 && (h->solver == LBCNN_SOLVER_MIXED || (h->solver == LBCNN_SOLVER_AUTO && pl.allow_tc && dim >= LB_STC_AUTO_DIM));
   const int NBO = tc_solve ? h->panel : 256;
   const int NBM = (tc_solve && h->mid_panel >= NB && h->mid_panel < NBO) ? h->mid_panel : NBO;      // mid level (fp64 steps inside)
   // columns of the common-mode deflation (fp64); never wider than one 64-column step or the system

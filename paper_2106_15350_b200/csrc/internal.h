@@ -99,6 +99,8 @@ struct FitPlan {
   size_t perm_off, off_off, a_off, tc_off, linv_off, stc_off, total; // offsets inside the fit workspace
   int64_t n_extra;       // dual branch, search driver: test samples stacked behind the train samples (cross-Gram rows in A)
   size_t lg_off;         // ... and their logits [n_cand][n_extra][n_classes] fp64
+  int allow_tc;          // LBCNN_SOLVER_AUTO may take the tensor-core updates (set by the search driver when the architecture
+                         // cannot produce (anti)collinear features; lbcnn_elm_fit leaves it 0: unknown data -> all-fp64)
   int stc_kmax;          // widest panel the tensor-core trailing update is planned for (0: no scratch reserved)
   int use_tc;            // Gram on the tensor pipe (exact int8-digit path, gram_tc.cu)
   int fuse_rhs;          // ... which then also produces the right-hand side (one-hot label columns)

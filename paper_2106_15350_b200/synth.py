@@ -129,6 +129,9 @@ WORKLOADS: Dict[str, Workload] = {
     "vggface": Workload("vggface", 5, 64, 64, 3, (_full(16, 3, 2, 2), _full(32, 3, 2, 2)), 20000, 5000, 100, 32, 1e4, "lowrank"),
     # P6: the paper's own architecture family: depthwise (16,20), pool (4,2,1,cover_all)
     "paper_anchor": Workload("paper_anchor", 6, 28, 28, 1, (_dw(16, 3, 4, 2, 1, 1), _dw(20, 3, 4, 2, 1, 1)), 1000, 500, 10, 2, 1e4, "blobs"),
+    # the same architecture at the size of the paper's Table I run ("first 20k" MNIST training samples,
+    # F = 15680, primal 15680 x 15680 system): a measured context line (bench.py --workload paper_table1), not a BASELINE config
+    "paper_table1": Workload("paper_table1", 6, 28, 28, 1, (_dw(16, 3, 4, 2, 1, 1), _dw(20, 3, 4, 2, 1, 1)), 20000, 10000, 10, 4, 1e4, "blobs"),
 }
 
 
