@@ -41,6 +41,7 @@ struct XtcParams {
   const uint8_t* img; long long n_img; int H, W, C;
   long long out_rows;            // rows per candidate of the output buffer (>= n_img: train and test features stacked)
   const uint8_t* wblob; int blob_bytes, w1_bytes, w2_bytes;   // per candidate: [B1 image | B2 image]
+  int shift_mode, nw2;           // layer 2 issued per plane SHIFT (2x2 pooling, 3x3 kernels); number of B2 slots (2 or 3)
   int n_cand, cand_per_cta;
   float* Hout; long long F; float scale;
   int n_layers;
@@ -70,6 +71,7 @@ struct PrepParams {
   const int8_t* ker; int n_weights; uint8_t* blob; int blob_bytes, w1_bytes, n_layers;
   int k1, P1, nph1, Cout1, N1, K1, K1p, Pk1, Cin1, w1_off;
   int k2, Cout2, N2, w2_off;
+  int shift_mode;
 };
 __global__ void __launch_bounds__(256) xtc_prep_kernel(const PrepParams p) {
   const int cand = blockIdx.y;
@@ -88,6 +90,25 @@ __global__ void __launch_bounds__(256) xtc_prep_kernel(const PrepParams p) {
         const int py = ph / p.P1, px = ph - py * p.P1;
         const int dy = yy - py, dx = xx - px;
         if (dy >= 0 && dy < p.k1 && dx >= 0 && dx < p.k1) v = kw[p.w1_off + ((o * p.Cin1 + c) * p.k1 + dy) * p.k1 + dx];
+      }
+    } else if (p.n_layers == 2 && p.shift_mode) {
+      // per-shift B2 (2x2 pooling, 3x3 kernels): [chunk lo | hi][28 blocks][N2 columns][16 B = input channel].  Blocks 4 s .. 4 s + 3
+      // (s = 2 ry + rx, the four plane shifts ry, rx in {0,1} that every pool phase reads): the taps of phases 00, 01, 10, 11,
+      // (ry+1, rx+1), (ry+1, rx), (ry, rx+1), (ry, rx).  Blocks 16 + 3 e .. + 2 (e = 2 ry + side; shifts rx = -1 / rx = 2, read by
+      // the phases px = 0 / px = 1 only): tap (ry+1, tx), a zero block, tap (ry, tx) with tx = 0 / 2.
+      const int u = t - p.w1_bytes;
+      const int c = u & 15, o = (u >> 4) % p.N2, blk = ((u >> 4) / p.N2) % 28, half = (u >> 4) / (p.N2 * 28);
+      int dy = -1, dx = -1;
+      if (blk < 16) {
+        const int sft = blk >> 2, q = blk & 3, ry = sft >> 1, rx = sft & 1;
+        dy = ry + 1 - (q >> 1); dx = rx + 1 - (q & 1);
+      } else {
+        const int e = (blk - 16) / 3, q = (blk - 16) % 3, ry = e >> 1, side = e & 1;
+        if (q != 1) { dy = ry + (q == 0 ? 1 : 0); dx = side ? 2 : 0; }
+      }
+      if (dy >= 0 && o < p.Cout2 && c < p.Cout1) {
+        v = kw[p.w2_off + (o * p.Cout1 + c) * 9 + dy * 3 + dx];
+        if (half) v *= 64;
       }
     } else if (p.n_layers == 2) {
       const int u = t - p.w1_bytes, kk2 = p.k2 * p.k2;
@@ -387,6 +408,44 @@ __device__ __forceinline__ void l2_issue_tile(const XtcParams& p, int half, uint
   }
 }
 
+// ---- layer-2 MMA issue per plane SHIFT (2x2 pooling, 3x3 kernels) ------------------------------------------------------------
+// A conv output of pool phase (py, px) and tap (dy, dx) reads the phase planes shifted by (ry, rx) = (py + dy - 1, px + dx - 1);
+// the 36 (phase, tap) pairs share only 16 shifts.  One MMA per shift feeds every phase that reads it -- the accumulators
+// of the four phases are adjacent in TMEM (00 | 01 | 10 | 11) and B2 holds the matching taps side by side:
+//   4 centre shifts  : all four phases, N = 4 N2                      (64 clk at N2 = 32: tensor-bound)
+//   4 top / bottom   : phases 00,01 / 10,11, N = 2 N2, the tap blocks are the second / first half of a centre block
+//   4 left / right   : phases 00,10 / 01,11 -- not adjacent: N = 3 N2 with a zero block between them
+//   4 corners        : one phase, N = N2, a block of the left / right images
+// 16 MMAs and 832 clk per 128 positions instead of 24 and 1056 (operand fetch, profiles/r2_ubench.md); one issuer warp.
+__device__ __forceinline__ void l2_issue_shift(const XtcParams& p, uint32_t d0, uint64_t da0, uint64_t db0, uint32_t idesc2) {
+  const int plane16 = p.plane_bytes >> 4, n2 = p.N2;
+  const uint32_t nf = ((uint32_t)n2 >> 3) << 17;                       // one more N2 in the descriptor's N field
+  bool first = true;
+#pragma unroll
+  for (int pass = 0; pass < 2; ++pass) {             // the centre shifts first: the very first MMA initialises all four accumulators
+#pragma unroll
+    for (int ry = -1; ry <= 2; ++ry) {
+#pragma unroll
+      for (int rx = -1; rx <= 2; ++rx) {
+        const bool ymid = (ry == 0 || ry == 1), xmid = (rx == 0 || rx == 1);
+        if ((ymid && xmid) != (pass == 0)) continue;
+        const int qy = floordiv(ry, 2), sy = ry - qy * 2, qx = floordiv(rx, 2), sx = rx - qx * 2;
+        const uint64_t da = da0 + (uint64_t)(long long)((sy * 2 + sx) * plane16 + qy * p.Wq + qx);
+        const int cy = ry < 0 ? 0 : (ry > 1 ? 1 : ry);                    // row of the nearest centre shift
+        int blk, dphase, nmul;
+        if (ymid && xmid)      { blk = 4 * (2 * ry + rx); dphase = 0; nmul = 4; }
+        else if (xmid)         { blk = 4 * (2 * cy + rx) + (ry < 0 ? 2 : 0); dphase = ry < 0 ? 0 : 2; nmul = 2; }      // top / bottom
+        else if (ymid)         { blk = 16 + 3 * (2 * ry + (rx < 0 ? 0 : 1)); dphase = rx < 0 ? 0 : 1; nmul = 3; }      // left / right
+        else                   { blk = 16 + 3 * (2 * cy + (rx < 0 ? 0 : 1)) + (ry < 0 ? 2 : 0); dphase = (ry < 0 ? 0 : 2) + (rx < 0 ? 0 : 1); nmul = 1; }
+        const uint64_t db = db0 + (uint64_t)(blk * n2);
+        const uint32_t idesc = idesc2 + (uint32_t)(nmul - 1) * nf;
+        if (tc::elect_one()) tc::mma_i8(d0 + dphase * n2, da, db, idesc, first ? 0u : 1u);
+        first = false;
+      }
+    }
+  }
+}
+
 // ---- the kernel ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParams p) {
   extern __shared__ __align__(128) uint8_t smem[];
@@ -401,7 +460,7 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
   const uint32_t s_base = tc::smem_u32(smem);
   const int nslot1 = 1 << p.lg_nslot1;
   const int n_e1_warps = 4 << p.lg_nset1;
-  const int n_l2_issuers = (p.n_layers == 2 && p.P2 > 1) ? 2 : 1;     // warps 1 and 18 split a tile's pool phases
+  const int n_l2_issuers = (p.n_layers == 2 && p.P2 > 1 && !p.shift_mode) ? 2 : 1;     // warps 1 and 18 split a tile's pool phases
 
   if (tid == 0) {
     for (int i = 0; i < N_BARS; ++i) {
@@ -539,7 +598,8 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
     const int half = (warp == 1) ? 0 : 1;
     if (p.n_layers == 2 && half < n_l2_issuers) {
       const uint32_t idesc2 = tc::idesc_i8(128, p.N2, 1, 1, 0, 0);
-      const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)(p.k2 * p.k2 * p.N2) * 16;   // digit-chunk strides
+      const uint32_t lbo_a = (uint32_t)p.NPOS2 * 16, lbo_b = (uint32_t)((p.shift_mode ? 28 : p.k2 * p.k2) * p.N2) * 16;   // digit-chunk strides
+      const int nw2 = p.nw2;
       const int acc_cols = p.nph2 * p.N2;
       int n2 = 0;
       for (int ci = 0; ci < n_cta_cand; ++ci) {
@@ -548,7 +608,7 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
           tc::bulk_load(s_base + p.off_w2, p.wblob + (long long)c_begin * p.blob_bytes + p.w1_bytes, p.w2_bytes, bar_addr(bars, W2_FULL));
         }
         if (half == 0 && ci + 1 < n_cta_cand) {
-          const int slot = (ci + 1) % 3, use = (ci + 1) / 3;
+          const int slot = (ci + 1) % nw2, use = (ci + 1) / nw2;
           tc::mbar_wait(bar_addr(bars, W2_EMPTY + slot), (use & 1) ^ 1);
           if (tc::elect_one()) {
             tc::mbar_arrive_expect_tx(bar_addr(bars, W2_FULL + slot), p.w2_bytes);
@@ -556,8 +616,8 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
                           p.w2_bytes, bar_addr(bars, W2_FULL + slot));
           }
         }
-        const int wslot = ci % 3;
-        tc::mbar_wait(bar_addr(bars, W2_FULL + wslot), (ci / 3) & 1);
+        const int wslot = ci % nw2;
+        tc::mbar_wait(bar_addr(bars, W2_FULL + wslot), (ci / nw2) & 1);
         const int buf = (p.NPB == 2) ? (ci & 1) : 0;
         const int use = (p.NPB == 2) ? (ci >> 1) : ci;
         tc::mbar_wait(bar_addr(bars, PL_FULL + buf), use & 1);
@@ -571,7 +631,8 @@ __global__ void __launch_bounds__(XT_THREADS, 1) expand_tc_kernel(const XtcParam
           const uint32_t row0 = (uint32_t)(p.base0 + t2 * 128) * 16;
           const uint64_t da0 = tc::smem_desc(pl_base + row0, lbo_a, 128, tc::LAYOUT_NONE);
           const uint64_t db0 = tc::smem_desc(b_base, lbo_b, 128, tc::LAYOUT_NONE);
-          if (p.P2 == 2 && p.k2 == 3) l2_issue_tile<2, 3>(p, half, d0, da0, db0, idesc2);
+          if (p.shift_mode) l2_issue_shift(p, d0, da0, db0, idesc2);
+          else if (p.P2 == 2 && p.k2 == 3) l2_issue_tile<2, 3>(p, half, d0, da0, db0, idesc2);
           else if (p.P2 == 1 && p.k2 == 3) l2_issue_tile<1, 3>(p, half, d0, da0, db0, idesc2);
           else l2_issue_tile<0, 0>(p, half, d0, da0, db0, idesc2);
           if (tc::elect_one()) tc::mma_commit(bar_addr(bars, R2_FULL + slot));
@@ -660,7 +721,9 @@ static bool plan_xtc(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias,
     p.lg_nset1 = 1; p.lg_nslot1 = (4 * p.N1 + 2 * p.nph2 * p.N2 <= 512) ? 2 : 1;
     p.tm_r1 = 0; p.tm_r2 = (1 << p.lg_nslot1) * p.N1;
     if (p.tm_r2 + 2 * p.nph2 * p.N2 > 512) return false;
-    p.w2_bytes = p.k2 * p.k2 * p.N2 * 32;
+    // 2x2 pooling with 3x3 kernels: one MMA per plane shift (l2_issue_shift) -- B2 then holds 28 tap blocks instead of 9
+    p.shift_mode = (p.P2 == 2 && p.k2 == 3 && 4 * p.N2 <= 256) ? 1 : 0;
+    p.w2_bytes = (p.shift_mode ? 28 : p.k2 * p.k2) * p.N2 * 32;
     const int hq = (p.pd2 + p.P2 - 1) / p.P2, qmax = (p.P2 - 1 + p.pd2) / p.P2;
     halo = hq > qmax ? hq : qmax;
     // Row pitch and first row of the halo-sharing grid.  A shifted operand whose start is not a multiple of 8 rows
@@ -700,7 +763,8 @@ static bool plan_xtc(const lbcnn_handle_s* h, const ArchShape& s, bool has_bias,
         u.plane_bytes = 2 * u.NPOS2 * 16;
         u.plbuf_bytes = p.nph2 * u.plane_bytes;
         u.NPB = npb;
-        u.off_w2 = take2(3 * p.w2_bytes);
+        u.nw2 = p.shift_mode ? 2 : 3;                                // the per-shift image is 3x larger: two slots
+        u.off_w2 = take2(u.nw2 * p.w2_bytes);
         u.off_tab2 = take2(u.T2 * 128 * 4);
         u.off_pl = take2(npb * u.plbuf_bytes);
         score = 0.3 * t.NP1 / t.NP1p + 0.7 * u.NM2 / (u.T2 * 128.0);
@@ -749,7 +813,7 @@ int lb_launch_expand_tc(lbcnn_handle_s* h, const ArchShape& s, float feature_sca
     w.blob_bytes = p.blob_bytes; w.w1_bytes = p.w1_bytes; w.n_layers = p.n_layers;
     w.k1 = p.k1; w.P1 = p.P1; w.nph1 = p.nph1; w.Cout1 = p.Cout1; w.N1 = p.N1; w.K1 = p.K1; w.K1p = p.K1p; w.Pk1 = p.Pk1;
     w.Cin1 = p.C; w.w1_off = (int)s.L[0].w_off;
-    if (p.n_layers == 2) { w.k2 = p.k2; w.Cout2 = p.Cout2; w.N2 = p.N2; w.w2_off = (int)s.L[1].w_off; }
+    if (p.n_layers == 2) { w.k2 = p.k2; w.Cout2 = p.Cout2; w.N2 = p.N2; w.w2_off = (int)s.L[1].w_off; w.shift_mode = p.shift_mode; }
     dim3 grid((unsigned)((p.blob_bytes + 1023) / 1024 < 1 ? 1 : (p.blob_bytes + 1023) / 1024), (unsigned)n_cand);
     xtc_prep_kernel<<<grid, 256, 0, st>>>(w);
     h->launches += 1;
