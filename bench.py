@@ -134,8 +134,12 @@ def _phase_rooflines(w, F, n_cand, phase_ms, steps, peaks, sustained: bool, stat
     tens = bf16 / 2.0 / 3.0
     int8 = 2.0 * bf16
     stats = stats or {}
-    gram_flop = n_cand * (float(N) * F * (F + 1) if primal else float(F) * N * (N + 1))
-    solve_flop = n_cand * (dim ** 3 / 3.0 + 2.0 * dim * dim * c + (0 if primal else 2.0 * N * F * c))
+    # dual branch (F >= N), scored through the kernel trick (the driver's default): the Gram of the stacked
+    # [train; test] rows also yields the cross-Gram (2 F N_te N flop), the factorisation carries c + N_te appended rows, the
+    # scores are one N_te x N x c product of appended rows (fp64) -- no F x c back-projection, no pass over the test features
+    kt = (not primal) and not any(o == 9 and v == 0 for o, v in OPTIONS)
+    gram_flop = n_cand * (float(N) * F * (F + 1) if primal else float(F) * N * (N + 1) + (2.0 * F * Nte * N if kt else 0.0))
+    solve_flop = n_cand * (dim ** 3 / 3.0 + 2.0 * dim * dim * c + (0 if primal else (float(dim) * dim * Nte if kt else 2.0 * N * F * c)))
     work = {
         # H written once (4 F bytes per image per candidate) + every image read once per launch
         "expand": ("hbm", "GB/s", hbm, (n_cand * (N + Nte) * F * 4.0 + (N + Nte) * px) / 1e9, "HBM copy GB/s"),
@@ -150,6 +154,9 @@ def _phase_rooflines(w, F, n_cand, phase_ms, steps, peaks, sustained: bool, stat
         # test features read once + W
         "score": ("hbm", "GB/s", hbm, n_cand * (float(Nte) * F * 4.0 + F * c * 4.0) / 1e9, "HBM copy GB/s"),
     }
+    if kt:
+        work["score"] = ("fp64", "TFLOP/s", FP64_TFLOPS, n_cand * 2.0 * Nte * N * c / 1e12,
+                         "fp64 DMMA pipe (kernel-trick logits: a product of the factorisation's appended rows)")
     out = {}
     for ph, (bound, unit, peak, amount, src) in work.items():
         ms = phase_ms.get(ph, (0.0, 0))[0] / max(steps, 1)
