@@ -318,6 +318,28 @@ __device__ __forceinline__ void e2_run(const XtcParams& p, const uint8_t* smem, 
       tc::tc_fence_after();
       const int32_t off = tab2[t2 * 128 + quad * 32 + lane];
       for (int c0 = 0; c0 < cout2; c0 += 16) {
+        if (cout2 - c0 <= 4 && nph2 == 4) {
+          // tail of up to four channels (configs[1]: 20 = 16 + 4): four-column loads, a quarter of the max / store work
+          uint32_t q0[4], q1[4], q2[4], q3[4];
+          tc::tmem_ld4(taddr + c0, q0);
+          tc::tmem_ld4(taddr + N2 + c0, q1);
+          tc::tmem_ld4(taddr + 2 * N2 + c0, q2);
+          tc::tmem_ld4(taddr + 3 * N2 + c0, q3);
+          tc::tmem_ld_wait();
+          if (off >= 0) {
+            uint32_t idx = (uint32_t)off + (uint32_t)c0 * hw;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              if (c0 + e < cout2) {
+                int v = max(max((int)q0[e], (int)q1[e]), max((int)q2[e], (int)q3[e]));
+                if (RELU) v = max(v, 0);
+                Hb[idx] = UNIT ? (float)v : scale * (float)v;
+                idx += hw;
+              }
+            }
+          }
+          continue;
+        }
         int mx[16];
         {
           uint32_t r0[16], r1[16];
