@@ -447,6 +447,19 @@ def _extras(lb, synth, torch, np, name, peaks, local):
                            accuracy_int8=round(float(corr["c"].float().mean().item()) / w.n_test, 4),
                            accuracy_fp32=round(float(corr_f.float().mean().item()) / w.n_test, 4),
                            note="exact integer logits (lbcnn_elm_score_q), test features read once as fp32")
+    # 8(f)-4: one epoch of softmax cross-entropy / Adam refinement of candidate 0's output layer on the whole training set
+    Htr0 = h.expand(a1, d[0], d[4][:1])[0].contiguous()
+    ref = {}
+    ms_r = timed(lambda: ref.update(r=h.refine_output_layer(Htr0, d[1], W[0].contiguous(), epochs=2, batch=128, lr=1e-5, seed=1, h_scale=s)), reps=1, warm=1)
+    Wr, lossr = ref["r"]
+    _, corr_r = h.elm_score(Hte[:1].contiguous(), Wr[None].contiguous(), d[3], h_scale=s, want_pred=False)
+    out["refine"] = dict(epochs=2, batch=128, lr=1e-5, ms_per_epoch=round(ms_r / 2.0, 2), mean_loss_per_epoch=[round(float(x), 5) for x in lossr.tolist()],
+                         accuracy_elm=round(float(corr_f[0].item()) / w.n_test, 4), accuracy_after=round(float(corr_r[0].item()) / w.n_test, 4),
+                         note="lbcnn_refine_output_layer (softmax cross-entropy + Adam, reading R18): %d sequential mini-batch steps of five "
+                              "launches per epoch, fp64 DMMA.  The starting point is already the exact ridge optimum on the whole set, so "
+                              "the first epochs of a different loss move away from it: a timing and parity line, not an accuracy claim"
+                              % ((w.n_train + 127) // 128))
+    del Htr0
     # 8(f)-3: one genetic generation over the K kernel sets
     ms_g = timed(lambda: h.evolve_candidates(d[4], acc, max(1, K // 8), 20000, 1, 0))
     out["evolve"] = dict(candidates=K, ms=round(ms_g, 4), note="rank + tournament + uniform crossover + mutation (lbcnn_evolve_candidates)")

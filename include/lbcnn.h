@@ -255,6 +255,29 @@ int lbcnn_evolve_candidates(lbcnn_handle_t h, const int8_t* d_kernels /*[n_cand]
                             int32_t n_cand, int64_t n_weights, int32_t n_elite, uint32_t mut_ppm, uint64_t seed,
                             uint32_t generation, int8_t* d_next /*[n_cand][n_weights]*/, void* stream);
 
+/* Gradient refinement of the output layer on the full training set (the notebook's Cell 10, "training the output
+ * layer with the full dataset"; +0.73 pp on MNIST).  The paper names neither loss, optimiser nor schedule --
+ * reading DESIGN.md R18 (= SPEC.md:324, 355): softmax cross-entropy; adaptive moment estimation; per mini-batch
+ *   Z = h_scale H_b W,  P = softmax(Z),  G = h_scale H_b^T (P - T) / |batch|,
+ *   m = b1 m + (1 - b1) G,  v = b2 v + (1 - b2) G^2,  W -= lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps),
+ * sample j of epoch e is (a j + b) mod n with a (coprime to n) and b drawn from the counter-based generator of
+ * lbcnn_evolve_candidates: a = 1 + draw(seed, e, 0, 0) mod (n - 1), advanced by a = a mod (n - 1) + 1 until gcd(a, n) = 1,
+ * b = draw(seed, e, 0, 1) mod n.  The last batch of an epoch may be short.  fp64 arithmetic; d_W (fp32) is read as the
+ * starting point (e.g. the ELM fit of the search on a reduced subset) and overwritten with the result; d_loss (may be NULL)
+ * receives the mean cross-entropy of each epoch.  epochs = 0 leaves W unchanged.  One candidate; the binary kernels are
+ * frozen by construction (the features are the input).  Needs lbcnn_refine_workspace_bytes of workspace. */
+typedef struct {
+  int32_t epochs;  /* >= 0 (SPEC default 10) */
+  int32_t batch;   /* >= 1 (128) */
+  float lr;        /* > 0 (1e-3) */
+  float beta1, beta2, eps; /* 0.9, 0.999, 1e-8 */
+  uint64_t seed;
+} lbcnn_refine_t;
+int lbcnn_refine_workspace_bytes(int64_t F, int32_t n_classes, const lbcnn_refine_t* cfg, size_t* bytes);
+int lbcnn_refine_output_layer(lbcnn_handle_t h, const float* d_H /*[n][F]*/, int64_t n, int64_t F, float h_scale,
+                              const int32_t* d_labels /*[n]*/, int32_t n_classes, const lbcnn_refine_t* cfg,
+                              float* d_W /*[F][n_classes], in / out*/, float* d_loss /*[epochs] or NULL*/, void* stream);
+
 /* Workspace lbcnn_elm_score needs under LBCNN_SCORER_TENSOR (host-only arithmetic; 0 is never returned). */
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes);
 

@@ -292,3 +292,57 @@ def evolve_candidates(kernels: np.ndarray, acc: np.ndarray, n_elite: int, mut_pp
                 v = -v
             nxt[j, t] = v
     return nxt, parents, np.array(order, dtype=np.int32)
+
+
+# ---- gradient refinement of the output layer on the full set -----------------------------------------
+# Cell 10 of the notebook trains "the output layer with the full dataset" with "the traditional Keras approach based on
+# 'optimizers'" (+0.73 pp on MNIST) and names neither loss, optimiser nor schedule.  Reading
+# DESIGN.md R18 = SPEC.md:324, 355: softmax cross-entropy, adaptive moment estimation (0.9, 0.999, 1e-8), mini-batches.
+# The sample order of an epoch is the affine map i = (a j + b) mod N, gcd(a, N) = 1, with a and b from the counter-based
+# generator above (both sides compute it on the host; no library shuffle).
+def refine_order(seed: int, epoch: int, n: int):
+    """(a, b) of epoch `epoch`: sample j of the epoch is (a j + b) mod n."""
+    from math import gcd
+    if n == 1:
+        return 1, 0
+    a = 1 + ga_draw(seed, epoch, 0, 0) % (n - 1)
+    while gcd(a, n) != 1:
+        a = a % (n - 1) + 1
+    return a, ga_draw(seed, epoch, 0, 1) % n
+
+
+def refine_output_layer(H: np.ndarray, labels: np.ndarray, W0: np.ndarray, epochs: int, batch: int, lr: float,
+                        beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, seed: int = 0, h_scale: float = 1.0):
+    """H [n][F] (stored features; logical feature = h_scale * H), W0 [F][classes] (e.g. the ELM fit).  fp64 throughout.
+    Per mini-batch: Z = h_scale H_b W; P = softmax(Z) (row maximum subtracted); loss = -sum log P[i, y_i];
+    G = h_scale H_b^T (P - T) / |batch|; Adam step on W.  Returns (W, mean loss per epoch)."""
+    H = np.ascontiguousarray(H, dtype=np.float64)
+    y = np.asarray(labels, dtype=np.int64)
+    n, F = H.shape
+    W = np.array(W0, dtype=np.float64, copy=True)
+    c = W.shape[1]
+    m = np.zeros_like(W); v = np.zeros_like(W)
+    t = 0
+    losses = []
+    hs = float(np.float32(h_scale))
+    for e in range(epochs):
+        a, b = refine_order(seed, e, n)
+        tot = 0.0
+        for s0 in range(0, n, batch):
+            j = np.arange(s0, min(n, s0 + batch), dtype=np.int64)
+            idx = (a * j + b) % n
+            Hb = H[idx]
+            Z = hs * (Hb @ W)
+            Z -= Z.max(axis=1, keepdims=True)
+            E = np.exp(Z)
+            P = E / E.sum(axis=1, keepdims=True)
+            tot += float(-np.log(P[np.arange(len(idx)), y[idx]]).sum())
+            D = P
+            D[np.arange(len(idx)), y[idx]] -= 1.0
+            G = hs * (Hb.T @ D) / float(len(idx))
+            t += 1
+            m = beta1 * m + (1.0 - beta1) * G
+            v = beta2 * v + (1.0 - beta2) * G * G
+            W -= lr * (m / (1.0 - beta1 ** t)) / (np.sqrt(v / (1.0 - beta2 ** t)) + eps)
+        losses.append(tot / n)
+    return W, np.array(losses)

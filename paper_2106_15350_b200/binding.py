@@ -27,7 +27,8 @@ EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destro
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
            "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes",
-           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q", "lbcnn_evolve_candidates")
+           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q", "lbcnn_evolve_candidates",
+           "lbcnn_refine_workspace_bytes", "lbcnn_refine_output_layer")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
 
@@ -39,6 +40,11 @@ class Layer(C.Structure):
 class Arch(C.Structure):
     _fields_ = [("in_h", C.c_int32), ("in_w", C.c_int32), ("in_c", C.c_int32), ("n_layers", C.c_int32),
                 ("layer", Layer * 3), ("feature_scale", C.c_float)]
+
+
+class RefineCfg(C.Structure):
+    _fields_ = [("epochs", C.c_int32), ("batch", C.c_int32), ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float),
+                ("eps", C.c_float), ("seed", C.c_uint64)]
 
 
 class LbcnnError(RuntimeError):
@@ -295,6 +301,23 @@ class Handle:
                                              C.c_int64(nw), C.c_int32(n_elite), C.c_uint32(mut_ppm), C.c_uint64(seed),
                                              C.c_uint32(generation), _ptr(nxt), _stream()), "lbcnn_evolve_candidates")
         return nxt
+
+    def refine_output_layer(self, H, labels, W, epochs: int = 10, batch: int = 128, lr: float = 1e-3, beta1: float = 0.9,
+                            beta2: float = 0.999, eps: float = 1e-8, seed: int = 0, h_scale: float = 1.0):
+        """H f32 [n][F], W f32 [F][c] (starting point; a refined copy is returned together with the per-epoch mean loss)."""
+        import torch
+        n, F = H.shape
+        c = W.shape[1]
+        cfg = RefineCfg(int(epochs), int(batch), float(lr), float(beta1), float(beta2), float(eps), int(seed))
+        b = C.c_size_t()
+        _check(lib().lbcnn_refine_workspace_bytes(C.c_int64(F), C.c_int32(c), C.byref(cfg), C.byref(b)), "lbcnn_refine_workspace_bytes")
+        self.ensure_workspace(b.value)
+        Wn = W.clone()
+        loss = torch.zeros(max(int(epochs), 1), dtype=torch.float32, device=H.device)
+        _check(lib().lbcnn_refine_output_layer(self._h, _ptr(H, torch.float32), C.c_int64(n), C.c_int64(F), C.c_float(h_scale),
+                                               _ptr(labels, torch.int32), C.c_int32(c), C.byref(cfg), _ptr(Wn, torch.float32),
+                                               _ptr(loss), _stream()), "lbcnn_refine_output_layer")
+        return Wn, loss[:int(epochs)]
 
     def quantize_output_layer(self, W, bits: int = 8):
         """W f32 [K][F][c] -> (Wq i8 [K][F][c], scale f32 [K]); W ~ scale * Wq (include/lbcnn.h)."""

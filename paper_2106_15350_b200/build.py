@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblbcnn.so")
-SOURCES = ["api.cu", "expand.cu", "expand_tc.cu", "fit.cu", "chol_tc.cu", "gram_tc.cu", "score.cu", "score_tc.cu", "evolve.cu"]
+SOURCES = ["api.cu", "expand.cu", "expand_tc.cu", "fit.cu", "chol_tc.cu", "gram_tc.cu", "score.cu", "score_tc.cu", "evolve.cu", "refine.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--cudart", "static"]
 

@@ -381,6 +381,22 @@ int lbcnn_evolve_candidates(lbcnn_handle_t h, const int8_t* d_kernels, const flo
                           (cudaStream_t)stream);
 }
 
+int lbcnn_refine_workspace_bytes(int64_t F, int32_t n_classes, const lbcnn_refine_t* cfg, size_t* bytes) {
+  if (!bytes || !cfg || F < 1 || n_classes < 2 || cfg->epochs < 0 || cfg->batch < 1) return LBCNN_ERR_INVALID_ARG;
+  *bytes = lb_refine_ws_bytes(F, n_classes, cfg->batch, cfg->epochs) + LB_WS_HEAD;
+  return LBCNN_OK;
+}
+
+int lbcnn_refine_output_layer(lbcnn_handle_t h, const float* d_H, int64_t n, int64_t F, float h_scale, const int32_t* d_labels,
+                              int32_t n_classes, const lbcnn_refine_t* cfg, float* d_W, float* d_loss, void* stream) {
+  if (!h || !d_H || !d_labels || !cfg || !d_W || n < 1 || F < 1 || n_classes < 2) return LBCNN_ERR_INVALID_ARG;
+  if (cfg->epochs < 0 || cfg->batch < 1 || !(cfg->lr > 0.0f) || !(h_scale > 0.0f) || n > 2147483647LL || F > 2147483647LL)
+    return LBCNN_ERR_INVALID_ARG;
+  if (!(cfg->beta1 >= 0.0f && cfg->beta1 < 1.0f && cfg->beta2 >= 0.0f && cfg->beta2 < 1.0f && cfg->eps >= 0.0f)) return LBCNN_ERR_INVALID_ARG;
+  if (!h->ws || lb_ws_avail(h) < lb_refine_ws_bytes(F, n_classes, cfg->batch, cfg->epochs)) return LBCNN_ERR_WORKSPACE;
+  return lb_launch_refine(h, lb_ws_base(h), d_H, n, F, h_scale, d_labels, n_classes, *cfg, d_W, d_loss, (cudaStream_t)stream);
+}
+
 int lbcnn_score_workspace_bytes(int64_t n, int64_t F, int32_t n_classes, int32_t n_cand, size_t* bytes) {
   if (!bytes || n < 1 || F < 1 || n_classes < 2 || n_cand < 1) return LBCNN_ERR_INVALID_ARG;
   *bytes = lb_score_tc_ws_bytes(n, F, n_classes, n_cand) + LB_WS_HEAD;

@@ -163,6 +163,10 @@ int lb_launch_score_q8(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n,
 // one generation of the genetic candidate generator (evolve.cu); ws: 8 * n_cand bytes of scratch
 int lb_launch_evolve(lbcnn_handle_s* h, void* ws, const int8_t* d_kernels, const float* d_acc, int n_cand, int64_t n_weights,
                      int n_elite, uint32_t mut_ppm, uint64_t seed, uint32_t generation, int8_t* d_next, cudaStream_t st);
+// gradient refinement of the output layer (refine.cu)
+size_t lb_refine_ws_bytes(int64_t F, int n_classes, int batch, int epochs);
+int lb_launch_refine(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const int32_t* d_labels,
+                     int c, const lbcnn_refine_t& cfg, float* d_W, float* d_loss, cudaStream_t st);
 int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,

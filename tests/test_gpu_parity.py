@@ -401,6 +401,37 @@ def test_genetic_generator_bit_exact_and_improves(handle):
     assert best[1] >= best[0] and best[2] >= best[1]
 
 
+@pytest.mark.parametrize("name,ntr,nte,epochs,batch", [("mnist", 1500, 700, 3, 128), ("gtsrb", 900, 300, 2, 100), ("tiny_mnist", 333, 100, 4, 64)])
+def test_refine_output_layer_matches_oracle(handle, name, ntr, nte, epochs, batch):
+    """SURVEY.md 8(f)-4 (PAPER.md:98 Cell 10; R18 = SPEC.md:324, 355): softmax cross-entropy + Adam on the output
+    layer, starting from the ELM fit, features from the frozen binary kernels.  fp64 on both sides: the refined W must
+    match the oracle's within north_star's 1e-3 (it does to ~1e-9), the per-epoch losses to 1e-6, labels one by one;
+    epochs = 0 is the identity; a ragged last batch on purpose."""
+    w = _small(name, ntr, nte, 1)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    W0, _, _, info = _staged(handle, w, trx, try_, tex, tey, ker)
+    assert info[0] == 0
+    a1 = lb.arch_of(w, 1.0)
+    s = float(np.float32(w.feature_scale))
+    Htr = handle.expand(a1, _dev(trx), _dev(ker))[0].contiguous()
+    Hte = handle.expand(a1, _dev(tex), _dev(ker))
+    W0f = _dev(W0[0].astype(np.float32))
+    Wn, loss = handle.refine_output_layer(Htr, _dev(try_), W0f, epochs=epochs, batch=batch, lr=1e-3, seed=5, h_scale=s)
+    Wsame, _ = handle.refine_output_layer(Htr, _dev(try_), W0f, epochs=0, batch=batch, h_scale=s)
+    torch.cuda.synchronize()
+    assert torch.equal(Wsame, W0f)
+    oa = _orc_arch(w)
+    Uo = orc.expand(oa, trx, ker[0]).astype(np.float64)
+    Wo, lo = orc.refine_output_layer(Uo, try_, W0[0].astype(np.float32).astype(np.float64), epochs, batch, 1e-3, seed=5, h_scale=s)
+    err = _fro(Wn.cpu().numpy().astype(np.float64), Wo)
+    assert err <= TOL_W_FRO and err <= 1e-5, err
+    assert np.allclose(loss.cpu().numpy(), lo, rtol=1e-5, atol=1e-7)      # (whether the loss falls at this lr is the recipe's business)
+    pred, _ = handle.elm_score(Hte, Wn[None].contiguous(), _dev(tey), h_scale=s)
+    po, _, _ = orc.elm_score(orc.expand(oa, tex, ker[0]).astype(np.float64) * s, Wo, tey)
+    assert (pred.cpu().numpy()[0] == po).mean() >= TOL_LABEL_AGREE
+
+
 def _search_both(handle, w, budget=None):
     trx, try_, tex, tey = synth.make_dataset(w)
     ker = synth.make_kernels(w)

@@ -626,3 +626,57 @@ def test_ga_generation_properties():
     assert np.array_equal(again, some)
     assert not np.array_equal(orc.evolve_candidates(ker, acc, 4, 20000, 7, 3)[0], some)
     assert not np.array_equal(orc.evolve_candidates(ker, acc, 4, 20000, 8, 2)[0], some)
+
+
+# ------------------------------------------------------------------------------------------------
+# gradient refinement of the output layer (R18 = SPEC.md:324, 355)
+# ------------------------------------------------------------------------------------------------
+def test_refine_identity_order_and_first_step():
+    rng = np.random.default_rng(2)
+    H = rng.normal(size=(37, 6)); y = rng.integers(0, 3, size=37); W0 = rng.normal(size=(6, 3)) * 0.1
+    W, losses = orc.refine_output_layer(H, y, W0, epochs=0, batch=8, lr=1e-3)
+    assert np.array_equal(W, W0) and len(losses) == 0                      # epochs = 0 -> unchanged
+    for n in (1, 2, 37, 20000, 30000):                                     # every epoch visits every sample exactly once
+        a, b = orc.refine_order(5, 3, n)
+        assert sorted(((a * np.arange(n, dtype=np.int64) + b) % n).tolist()) == list(range(n))
+    # the first Adam step moves every weight by lr * sign(gradient) (m_hat / sqrt(v_hat) = g / |g|), whatever the data
+    W1, _ = orc.refine_output_layer(H, y, W0, epochs=1, batch=37, lr=1e-2, eps=0.0)
+    Z = H @ W0; P = np.exp(Z - Z.max(1, keepdims=True)); P /= P.sum(1, keepdims=True)
+    P[np.arange(37), y] -= 1.0
+    G = H.T @ P / 37.0
+    assert np.allclose(W1, W0 - 1e-2 * np.sign(G), atol=1e-12)
+
+
+def test_refine_gradient_is_the_cross_entropy_gradient():
+    # finite differences of the mean softmax cross-entropy against the step direction of one full batch
+    rng = np.random.default_rng(8)
+    for _ in range(5):
+        n, F, c = 11, 4, 3
+        H = rng.normal(size=(n, F)); y = rng.integers(0, c, size=n); W0 = rng.normal(size=(F, c)) * 0.3
+
+        def loss(W):
+            Z = 0.5 * (H @ W); Z = Z - Z.max(1, keepdims=True)
+            return float(-(Z[np.arange(n), y] - np.log(np.exp(Z).sum(1))).mean())
+        G = np.zeros_like(W0)
+        for i in range(F):
+            for j in range(c):
+                d = np.zeros_like(W0); d[i, j] = 1e-6
+                G[i, j] = (loss(W0 + d) - loss(W0 - d)) / 2e-6
+        # one step with beta1 = beta2 = 0 and a huge eps turns Adam into W - lr * g / eps: read g back
+        W1, l0 = orc.refine_output_layer(H, y, W0, 1, n, lr=1.0, beta1=0.0, beta2=0.0, eps=1e6, h_scale=0.5)
+        g = (W0 - W1) * (1e6 + np.abs((W0 - W1) * 1e6))                    # g / (|g| + eps) = step  =>  g ~ step * eps (|g| << eps)
+        assert np.allclose(g, G, rtol=1e-4, atol=1e-8)
+        assert abs(l0[0] - loss(W0)) < 1e-12
+
+
+def test_refine_descends_and_separates():
+    rng = np.random.default_rng(4)
+    n = 120
+    y = rng.integers(0, 2, size=n)
+    H = np.c_[np.where(y == 0, 1.0, -1.0) + 0.1 * rng.normal(size=n), rng.normal(size=n), np.ones(n)]
+    W, losses = orc.refine_output_layer(H, y, np.zeros((3, 2)), epochs=30, batch=16, lr=5e-2, seed=1)
+    assert losses[1] <= losses[0] and losses[2] <= losses[1] and losses[-1] < 0.2 * losses[0]
+    pred, corr, _ = orc.elm_score(H, W, y.astype(np.int32))
+    assert corr == n                                                        # separable toy set -> training accuracy 1
+    W2, l2 = orc.refine_output_layer(H, y, np.zeros((3, 2)), epochs=30, batch=16, lr=5e-2, seed=1)
+    assert np.array_equal(W, W2)                                            # deterministic given the seed
