@@ -14,7 +14,8 @@
 // on the configs about one row in a thousand takes the second kernel.
 //
 // One CTA per (128 test rows, candidate); 10 warps:
-//   warp 0      TMA producer: fp32 feature tile [128 rows][64 features] + the four W digit tiles [N][64 B] per stage
+//   warp 0      TMA producer: fp32 feature tiles [128 rows][64 features] into a 3-5 stage ring of their own (freed by the
+//               converters), the four W digit tiles [N][64 B] into the two-stage digit ring (freed by the MMAs)
 //   warp 1      MMA issuer (M = 128, N = 16..128, K = 32; K-major, 64-byte swizzle)
 //   warps 2..9  converters: fp32 tile -> three int8 digit tiles in the MMA's swizzled layout (+ digit sums, validity);
 //               afterwards warps 2..5 are the epilogue: TMEM -> logits -> argmax / margin test / correct count
@@ -36,7 +37,7 @@ constexpr int UD_BYTES = TM * KC;        // 8 KB per U digit tile
 
 struct ScoreTcParams {
   int n, F, c, N;                        // rows, features, classes, padded classes (multiple of 16)
-  int n_iters, nstage, stage_bytes;
+  int n_iters, na, nb, stage_b;           // K steps; fp32 ring stages; digit ring stages and bytes per digit stage
   double hs;
   const double* cscale;                  // [n_cand][N]: 2^(e_c - 30)
   const int32_t* y;
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(256) score_q8_prep_kernel(const int8_t* __rest
 }
 
 // ---- the scoring kernel -----------------------------------------------------------------------------------------------
-constexpr int MAXSTAGE = 4;
+constexpr int MAXA = 6, MAXB = 2;        // fp32 feature ring (32 KB per stage) / digit ring (U digits + W digits)
 
 // NW digit planes of W, diagonals SMIN .. NDU + NW - 2 issued: <4, 2> = fp32 W as four column-scaled digits (nine of the
 // twelve products, error-bounded); <1, 0> = an int8 output layer (lbcnn_elm_score_q): all three products, EXACT integer logits
@@ -166,22 +167,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
   const int i0 = blockIdx.x * TM;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  __shared__ __align__(8) uint64_t bar_full[MAXSTAGE], bar_conv[MAXSTAGE], bar_empty[MAXSTAGE], bar_tmem;
+  __shared__ __align__(8) uint64_t bar_fullA[MAXA], bar_emptyA[MAXA], bar_fullW[MAXB], bar_conv[MAXB], bar_emptyB[MAXB], bar_tmem;
   __shared__ uint32_t tmem_base_s;
   __shared__ int32_t row_s[TM][4];               // digit sums S0, S1, S2 and the invalid-feature flag of every row
   const int warp = tc::uniform_warp_id(), lane = threadIdx.x & 31;
   const uint32_t smem0 = tc::smem_u32(smem);
-  const int N = p.N, nstage = p.nstage, stage_bytes = p.stage_bytes;
+  const int N = p.N, na = p.na, nb = p.nb, stage_b = p.stage_b;
   const int w_tile = N * KC;                     // bytes of one W digit tile
-  const int off_ud = UF32_BYTES, off_w = UF32_BYTES + NDU * UD_BYTES;
+  const int off_b = na * UF32_BYTES;             // the digit ring starts behind the fp32 ring
+  const int off_w = NDU * UD_BYTES;              // W digit tiles inside a digit stage (behind the three U digit tiles)
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tensormap(&tmapU);
     tc::prefetch_tensormap(&tmapW);
-    for (int s = 0; s < MAXSTAGE; ++s) {
-      tc::mbar_init(tc::smem_u32(&bar_full[s]), 1);
+    for (int s = 0; s < MAXA; ++s) {
+      tc::mbar_init(tc::smem_u32(&bar_fullA[s]), 1);
+      tc::mbar_init(tc::smem_u32(&bar_emptyA[s]), NCONV / 32);
+    }
+    for (int s = 0; s < MAXB; ++s) {
+      tc::mbar_init(tc::smem_u32(&bar_fullW[s]), 1);
       tc::mbar_init(tc::smem_u32(&bar_conv[s]), NCONV / 32);
-      tc::mbar_init(tc::smem_u32(&bar_empty[s]), 1);
+      tc::mbar_init(tc::smem_u32(&bar_emptyB[s]), 1);
     }
     tc::mbar_init(tc::smem_u32(&bar_tmem), 1);
     tc::fence_barrier_init();
@@ -193,21 +199,33 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
   const uint32_t tmem = tmem_base_s;
 
   if (warp == 0) {
-    // ===== TMA producer =====
-    int s = 0, ph = 0;
-    const uint32_t tx = (uint32_t)(UF32_BYTES + NW * w_tile);
-    for (int it = 0; it < p.n_iters; ++it) {
-      tc::mbar_wait(tc::smem_u32(&bar_empty[s]), ph ^ 1);
-      if (tc::elect_one()) {
-        const uint32_t full = tc::smem_u32(&bar_full[s]);
-        tc::mbar_arrive_expect_tx(full, tx);
-        const uint32_t base = smem0 + s * stage_bytes;
-        tc::tma_load_3d(base, &tmapU, full, it * KC, i0, z);
-#pragma unroll
-        for (int b = 0; b < NW; ++b) tc::tma_load_3d(base + off_w + b * w_tile, &tmapW, full, it * KC, 0, z * NW + b);
+    // ===== TMA producer: two independent streams -- fp32 feature tiles into ring A (freed by the converters), W digit tiles
+    // into ring B (freed by the MMAs).  Whichever slot is free is filled, so up to `na` feature tiles are in flight. =====
+    int ia = 0, sa = 0, pa = 0, ib = 0, sb = 0, pb = 0;
+    const int n = p.n_iters;
+    while (ia < n || ib < n) {
+      if (ia < n && tc::mbar_try_wait(tc::smem_u32(&bar_emptyA[sa]), pa ^ 1)) {
+        if (tc::elect_one()) {
+          const uint32_t full = tc::smem_u32(&bar_fullA[sa]);
+          tc::mbar_arrive_expect_tx(full, UF32_BYTES);
+          tc::tma_load_3d(smem0 + sa * UF32_BYTES, &tmapU, full, ia * KC, i0, z);
+        }
+        __syncwarp();
+        ++ia;
+        if (++sa == na) { sa = 0; pa ^= 1; }
       }
-      __syncwarp();
-      if (++s == nstage) { s = 0; ph ^= 1; }
+      if (ib < n && tc::mbar_try_wait(tc::smem_u32(&bar_emptyB[sb]), pb ^ 1)) {
+        if (tc::elect_one()) {
+          const uint32_t full = tc::smem_u32(&bar_fullW[sb]);
+          tc::mbar_arrive_expect_tx(full, (uint32_t)(NW * w_tile));
+          const uint32_t base = smem0 + off_b + sb * stage_b + off_w;
+#pragma unroll
+          for (int b = 0; b < NW; ++b) tc::tma_load_3d(base + b * w_tile, &tmapW, full, ib * KC, 0, z * NW + b);
+        }
+        __syncwarp();
+        ++ib;
+        if (++sb == nb) { sb = 0; pb ^= 1; }
+      }
     }
   } else if (warp == 1) {
     // ===== MMA issuer: diagonals s = a + b = SMIN .. into accumulators 0 .. NACC-1 =====
@@ -215,10 +233,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
     const uint64_t d0 = tc::smem_desc(smem0, 16, 8 * KC, LAYOUT_SW64);
     int s = 0, ph = 0;
     for (int it = 0; it < p.n_iters; ++it) {
-      tc::mbar_wait(tc::smem_u32(&bar_full[s]), ph);      // W digit tiles have landed
+      tc::mbar_wait(tc::smem_u32(&bar_fullW[s]), ph);     // W digit tiles have landed
       tc::mbar_wait(tc::smem_u32(&bar_conv[s]), ph);      // U digit tiles are written
       tc::tc_fence_after();
-      const uint64_t ds = d0 + (uint64_t)((s * stage_bytes) >> 4);
+      const uint64_t ds = d0 + (uint64_t)((off_b + s * stage_b) >> 4);
 #pragma unroll
       for (int kk = 0; kk < KC / 32; ++kk) {
 #pragma unroll
@@ -227,7 +245,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
           for (int a = 0; a < NDU; ++a) {
             const int b = sd - a;
             if (b >= 0 && b < NW) {
-              const uint64_t da = ds + (uint64_t)((off_ud + a * UD_BYTES + kk * 32) >> 4);
+              const uint64_t da = ds + (uint64_t)((a * UD_BYTES + kk * 32) >> 4);
               const uint64_t db = ds + (uint64_t)((off_w + b * w_tile + kk * 32) >> 4);
               const int a_first = (sd - (NW - 1)) > 0 ? sd - (NW - 1) : 0;             // smallest a of this diagonal
               const bool first = (kk == 0) && (a == a_first);
@@ -236,9 +254,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
           }
         }
       }
-      if (tc::elect_one()) tc::mma_commit(tc::smem_u32(&bar_empty[s]));
+      if (tc::elect_one()) tc::mma_commit(tc::smem_u32(&bar_emptyB[s]));
       __syncwarp();
-      if (++s == nstage) { s = 0; ph ^= 1; }
+      if (++s == nb) { s = 0; ph ^= 1; }
     }
     if (tc::elect_one()) tc::mma_commit(tc::smem_u32(&bar_tmem));
     __syncwarp();
@@ -250,10 +268,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
     uint32_t bad = 0;
 #pragma unroll
     for (int m = 0; m < 8; ++m) { S0[m] = 0; S1[m] = 0; S2[m] = 0; }
-    int s = 0, ph = 0;
+    int sa = 0, pa = 0, sb = 0, pb = 0;
     for (int it = 0; it < p.n_iters; ++it) {
-      tc::mbar_wait(tc::smem_u32(&bar_full[s]), ph);
-      uint8_t* st = smem + s * stage_bytes;
+      tc::mbar_wait(tc::smem_u32(&bar_fullA[sa]), pa);          // the fp32 tile has landed
+      tc::mbar_wait(tc::smem_u32(&bar_emptyB[sb]), pb ^ 1);     // the digit stage is free (its MMAs of two steps ago are done)
+      const uint8_t* st = smem + sa * UF32_BYTES;
+      uint8_t* sd = smem + off_b + sb * stage_b;
 #pragma unroll
       for (int m = 0; m < 8; ++m) {
         const int r = r_base + 16 * m;
@@ -271,15 +291,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) score_tc_kernel(const __grid_cons
         S0[m] += (int)__vsads4(w0, 0u); S1[m] += (int)__vsads4(w1, 0u); S2[m] += (int)__vsads4(w2, 0u);
         // 64-byte swizzle: 16-byte chunk index (cc / 4) XOR bits 1..2 of the row; word cc % 4 inside the chunk
         const uint32_t off = (uint32_t)r * KC + ((((uint32_t)cc >> 2) ^ (((uint32_t)r >> 1) & 3u)) << 4) + (((uint32_t)cc & 3u) << 2);
-        uint8_t* ud = st + off_ud + off;
+        uint8_t* ud = sd + off;
         *reinterpret_cast<uint32_t*>(ud) = w0;
         *reinterpret_cast<uint32_t*>(ud + UD_BYTES) = w1;
         *reinterpret_cast<uint32_t*>(ud + 2 * UD_BYTES) = w2;
       }
       tc::fence_proxy_async();                 // generic-proxy writes of the digit tiles -> visible to the MMA's async proxy
       __syncwarp();
-      if (lane == 0) tc::mbar_arrive(tc::smem_u32(&bar_conv[s]));
-      if (++s == nstage) { s = 0; ph ^= 1; }
+      if (lane == 0) {
+        tc::mbar_arrive(tc::smem_u32(&bar_conv[sb]));           // digits ready for the MMAs
+        tc::mbar_arrive(tc::smem_u32(&bar_emptyA[sa]));         // fp32 slot free for the next TMA
+      }
+      if (++sa == na) { sa = 0; pa ^= 1; }
+      if (++sb == nb) { sb = 0; pb ^= 1; }
     }
     // digit sums of every row: reduce over the 16 threads (a half warp) that share the row
 #pragma unroll
@@ -508,12 +532,14 @@ int launch_score_common(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n
   }
   ScoreTcParams p{};
   p.n = (int)n; p.F = (int)F; p.c = c; p.N = N; p.n_iters = Fp / KC; p.hs = (double)h_scale;
-  p.stage_bytes = UF32_BYTES + NDU * UD_BYTES + NW * N * KC;
-  p.nstage = (int)((size_t)(h->max_smem_optin - 2048) / (size_t)p.stage_bytes);
-  if (p.nstage > MAXSTAGE) p.nstage = MAXSTAGE;
-  if (p.nstage < 2) return LBCNN_ERR_INVALID_ARG;
+  // shared memory: two digit stages (U digits + W digits) and as many 32 KB fp32 feature stages as fit beside them
+  p.stage_b = NDU * UD_BYTES + NW * N * KC;
+  p.nb = MAXB;
+  p.na = (int)(((size_t)h->max_smem_optin - 4096 - (size_t)p.nb * p.stage_b) / (size_t)UF32_BYTES);
+  if (p.na > MAXA) p.na = MAXA;
+  if (p.na < 2) return LBCNN_ERR_INVALID_ARG;
   p.cscale = cscale; p.y = d_labels; p.pred = d_pred; p.correct = d_correct; p.flag_count = flag_count; p.flag_list = flag_list;
-  const size_t smem = (size_t)p.nstage * p.stage_bytes + 1024;
+  const size_t smem = (size_t)p.na * UF32_BYTES + (size_t)p.nb * p.stage_b + 1024;
   dim3 grid((unsigned)((n + TM - 1) / TM), (unsigned)n_cand);
   if (d_Wq) {
     LB_CUDA_OK(cudaFuncSetAttribute(score_tc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
