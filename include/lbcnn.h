@@ -11,7 +11,8 @@
  *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch allocations); pointers
  *     named h_* and all struct / out-parameter pointers are HOST pointers.  The library never
  *     allocates, frees or retains device memory; ALL scratch comes from the caller-provided workspace
- *     (lbcnn_set_workspace), and a call whose scratch does not fit returns LBCNN_ERR_WORKSPACE.
+ *     (lbcnn_set_workspace), and a call whose scratch does not fit returns LBCNN_ERR_WORKSPACE.  (The one exception is
+ *     lbcnn_evolve_candidates_static, whose scratch is a fixed array inside the library: see there.)
  *     `stream` is a cudaStream_t passed as void* (NULL = default stream).  The handle's device must be the
  *     calling thread's current device for every call that takes a stream (lbcnn_create does not change it).
  *   - Every call returns an int status (LBCNN_OK = 0 ...) and only ENQUEUES work on `stream`; it
@@ -48,7 +49,9 @@ enum {
   LBCNN_ERR_SHAPE = 3,        /* F / channel mismatch */
   LBCNN_ERR_WORKSPACE = 4,    /* workspace absent or too small (never a hidden allocation) */
   LBCNN_ERR_CUDA = 5,         /* no device / launch or driver error */
-  LBCNN_ERR_NOMEM = 6         /* host allocation failed (lbcnn_create) */
+  LBCNN_ERR_NOMEM = 6,        /* host allocation failed (lbcnn_create) */
+  LBCNN_ERR_STATIC_LIMIT = 7  /* lbcnn_evolve_candidates_static only: the problem needs more scratch than the library's built-in
+                                 array holds (n_cand > LBCNN_EVOLVE_STATIC_MAX_CAND); use lbcnn_evolve_candidates with a workspace */
 };
 
 enum { LBCNN_CONV_FULL = 0, LBCNN_CONV_DEPTHWISE = 1 };
@@ -254,6 +257,39 @@ int lbcnn_elm_score_q(lbcnn_handle_t h, const float* d_H /*[n_cand][n][F]*/, int
 int lbcnn_evolve_candidates(lbcnn_handle_t h, const int8_t* d_kernels /*[n_cand][n_weights]*/, const float* d_acc /*[n_cand]*/,
                             int32_t n_cand, int64_t n_weights, int32_t n_elite, uint32_t mut_ppm, uint64_t seed,
                             uint32_t generation, int8_t* d_next /*[n_cand][n_weights]*/, void* stream);
+
+/* lbcnn_evolve_candidates for callers that cannot hand the library a workspace.
+ *
+ * Every other compute call here takes its scratch from the buffer given to lbcnn_set_workspace, so somebody has to
+ * allocate device memory first.  Some programs cannot: a plug-in that its host application hands input and output buffers
+ * and nothing else; a process whose HBM was given whole to a memory pool at start-up, where a later cudaMalloc fails or
+ * comes out of somebody else's budget; a control loop that must not stall, for which cudaMalloc / cudaFree are off limits
+ * because they synchronise the whole device.  For them this entry point runs the same generation step (same arguments,
+ * same kernels, byte-for-byte the same d_next) with NO workspace: the ranking scratch (8 bytes per candidate) lives in an
+ * array compiled into the library, LBCNN_EVOLVE_STATIC_MAX_CAND * 8 bytes = 128 KB.  The handle needs no workspace; the
+ * call makes no cudaMalloc / cudaFree and calls no library routine that allocates.  The caller passes inputs and outputs only.
+ *
+ * What that costs, and the rules that come with it:
+ *   - Limit: n_cand <= LBCNN_EVOLVE_STATIC_MAX_CAND.  A larger population is refused with LBCNN_ERR_STATIC_LIMIT (nothing
+ *     is enqueued); it needs lbcnn_evolve_candidates and a workspace.  All other argument rules are lbcnn_evolve_candidates'.
+ *   - Footprint: the 128 KB belong to the library image, so every GPU on which this process uses liblbcnn holds them from the
+ *     moment the library's code is loaded there until the process exits, whether or not this entry point is ever called.
+ *   - First call on a device: the library looks the array's device address up once per device (cudaGetSymbolAddress, with
+ *     that device current) and remembers it.  The look-up may make the CUDA runtime load the library's code onto the GPU,
+ *     so make the first call on each device during start-up, outside any stream capture and outside the part of the program
+ *     that must not stall.  Later calls on that device only enqueue work.
+ *   - The handle's device must be the calling thread's current device (checked here: LBCNN_ERR_INVALID_ARG otherwise),
+ *     because the address belongs to the current device.
+ *   - One array per GPU, shared by every handle, stream and host thread of the process.  Each call clears the part it uses
+ *     (stream-ordered, before its kernels) and then overwrites it, so nothing carries over from the previous call; but two
+ *     calls whose GPU work can overlap -- different streams, or different handles on the same GPU -- write the same bytes
+ *     and race.  Keep all calls of one GPU on one stream, or order them with events.  The array's contents after a call
+ *     are unspecified.
+ * Like the other compute calls it only enqueues on `stream` and does not synchronise. */
+#define LBCNN_EVOLVE_STATIC_MAX_CAND 16384
+int lbcnn_evolve_candidates_static(lbcnn_handle_t h, const int8_t* d_kernels /*[n_cand][n_weights]*/, const float* d_acc /*[n_cand]*/,
+                                   int32_t n_cand, int64_t n_weights, int32_t n_elite, uint32_t mut_ppm, uint64_t seed,
+                                   uint32_t generation, int8_t* d_next /*[n_cand][n_weights]*/, void* stream);
 
 /* Gradient refinement of the output layer on the full training set (the notebook's Cell 10, "training the output
  * layer with the full dataset"; +0.73 pp on MNIST).  The paper names neither loss, optimiser nor schedule --

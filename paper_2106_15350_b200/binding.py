@@ -13,7 +13,8 @@ from typing import Optional, Sequence, Tuple
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liblbcnn.so")
 
-OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA, ERR_NOMEM = range(7)
+OK, ERR_INVALID_ARG, ERR_INVALID_ARCH, ERR_SHAPE, ERR_WORKSPACE, ERR_CUDA, ERR_NOMEM, ERR_STATIC_LIMIT = range(8)
+EVOLVE_STATIC_MAX_CAND = 16384
 CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
@@ -27,7 +28,7 @@ EXPORTS = ("lbcnn_version", "lbcnn_status_string", "lbcnn_create", "lbcnn_destro
            "lbcnn_elm_score", "lbcnn_search_candidates", "lbcnn_host_staging_bytes", "lbcnn_search_candidates_host",
            "lbcnn_launch_count", "lbcnn_set_profiling", "lbcnn_expand_path", "lbcnn_fit_workspace_bytes",
            "lbcnn_get_phase_times", "lbcnn_set_option", "lbcnn_expand_workspace_bytes", "lbcnn_get_op_stats", "lbcnn_score_workspace_bytes",
-           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q", "lbcnn_evolve_candidates",
+           "lbcnn_quantize_output_layer", "lbcnn_elm_score_q", "lbcnn_evolve_candidates", "lbcnn_evolve_candidates_static",
            "lbcnn_refine_workspace_bytes", "lbcnn_refine_output_layer")
 PHASES = ("expand", "gram", "rhs", "solve", "score", "finish")
 
@@ -300,6 +301,25 @@ class Handle:
         _check(lib().lbcnn_evolve_candidates(self._h, _ptr(kernels, torch.int8), _ptr(acc, torch.float32), C.c_int32(K),
                                              C.c_int64(nw), C.c_int32(n_elite), C.c_uint32(mut_ppm), C.c_uint64(seed),
                                              C.c_uint32(generation), _ptr(nxt), _stream()), "lbcnn_evolve_candidates")
+        return nxt
+
+    def evolve_candidates_static(self, kernels, acc, n_elite: int, mut_ppm: int, seed: int, generation: int):
+        """evolve_candidates for a caller that cannot allocate a workspace (a plug-in given only its input and output
+        buffers, a process whose device memory is all spoken for, a loop that must not hit cudaMalloc's device-wide
+        synchronisation): same arguments and byte-for-byte the same result, but the 8 bytes of ranking scratch per
+        candidate come from a 128 KB array built into liblbcnn.so, so no workspace is set or needed and the C call
+        allocates nothing.  (This Python wrapper still creates the output tensor, as evolve_candidates does; a caller that
+        must not allocate goes through the C ABI with its own d_next.)  At most EVOLVE_STATIC_MAX_CAND candidates, else
+        LbcnnError(ERR_STATIC_LIMIT).  The first call on a device resolves the array's address and may load the library's
+        code there: make it at start-up, before any stream capture.  All handles and streams of a GPU share the one
+        array, so calls that can overlap on the GPU race; keep them on one stream."""
+        import torch
+        K, nw = kernels.shape
+        nxt = torch.empty_like(kernels)
+        _check(lib().lbcnn_evolve_candidates_static(self._h, _ptr(kernels, torch.int8), _ptr(acc, torch.float32), C.c_int32(K),
+                                                    C.c_int64(nw), C.c_int32(n_elite), C.c_uint32(mut_ppm), C.c_uint64(seed),
+                                                    C.c_uint32(generation), _ptr(nxt), _stream()),
+               "lbcnn_evolve_candidates_static")
         return nxt
 
     def refine_output_layer(self, H, labels, W, epochs: int = 10, batch: int = 128, lr: float = 1e-3, beta1: float = 0.9,

@@ -66,6 +66,7 @@ const char* lbcnn_status_string(int status) {
     case LBCNN_ERR_WORKSPACE: return "workspace absent or too small";
     case LBCNN_ERR_CUDA: return "CUDA error (no device, launch or driver failure)";
     case LBCNN_ERR_NOMEM: return "host allocation failed";
+    case LBCNN_ERR_STATIC_LIMIT: return "size beyond the capacity of the library's built-in scratch array (use the workspace variant)";
     default: return "unknown status";
   }
 }

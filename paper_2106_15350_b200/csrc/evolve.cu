@@ -5,6 +5,7 @@
 // byte work and the random numbers are a counter-based splitmix64 finaliser keyed by (seed, generation, child, draw), so
 // the result is bit-exact against the oracle, which implements the same generator on its own.
 #include "internal.h"
+#include <mutex>
 
 namespace {
 
@@ -65,4 +66,57 @@ int lb_launch_evolve(lbcnn_handle_s* h, void* ws, const int8_t* d_kernels, const
   h->launches += 2;
   LB_CUDA_OK(cudaGetLastError());
   return LBCNN_OK;
+}
+
+// ---- lbcnn_evolve_candidates_static: the same generation step without a caller workspace ---------------------------------
+// For callers that have no device allocator to draw a workspace from (include/lbcnn.h says who they are).  The ranking
+// scratch -- order[n_cand] then rank_of[n_cand], int32 each -- sits in an array that is part of the library image instead.
+// 2 * 16384 * 4 B = 128 KB on every GPU that loads liblbcnn, from module load to process exit.
+static __device__ __align__(256) int32_t g_evolve_scratch[2 * LBCNN_EVOLVE_STATIC_MAX_CAND];
+
+namespace {
+
+// On the host, `g_evolve_scratch` names a shadow object the runtime uses as a look-up key; it is NOT the device address, and a
+// kernel handed &g_evolve_scratch[0] from host code would fault (or scribble on host memory where the GPU can reach it).
+// The real address differs per device and comes from cudaGetSymbolAddress with that device current; it is looked up on
+// the first call per device and kept here.
+constexpr int LB_MAX_DEVICES = 64;
+std::mutex g_scratch_mu;
+int32_t* g_scratch_addr[LB_MAX_DEVICES];   // zero-initialised: not looked up yet
+
+// scratch address on the calling thread's current device, which must be `device`
+int evolve_static_scratch(int device, int32_t** out) {
+  if (device < 0 || device >= LB_MAX_DEVICES) return LBCNN_ERR_INVALID_ARG;
+  int cur = -1;
+  LB_CUDA_OK(cudaGetDevice(&cur));
+  if (cur != device) return LBCNN_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lock(g_scratch_mu);
+  if (!g_scratch_addr[device]) {
+    void* p = nullptr;
+    LB_CUDA_OK(cudaGetSymbolAddress(&p, g_evolve_scratch));   // may load the module on this device: first call = set-up
+    if (!p) return LBCNN_ERR_CUDA;
+    g_scratch_addr[device] = static_cast<int32_t*>(p);
+  }
+  *out = g_scratch_addr[device];
+  return LBCNN_OK;
+}
+
+}  // namespace
+
+extern "C" int lbcnn_evolve_candidates_static(lbcnn_handle_t h, const int8_t* d_kernels, const float* d_acc, int32_t n_cand,
+                                              int64_t n_weights, int32_t n_elite, uint32_t mut_ppm, uint64_t seed,
+                                              uint32_t generation, int8_t* d_next, void* stream) {
+  if (!h || !d_kernels || !d_acc || !d_next || n_cand < 1 || n_weights < 1) return LBCNN_ERR_INVALID_ARG;
+  if (n_cand > LBCNN_EVOLVE_STATIC_MAX_CAND) return LBCNN_ERR_STATIC_LIMIT;   // the array is a fixed size: refuse, never spill
+  if (n_elite < 0 || n_elite > n_cand || mut_ppm > 1000000u || d_next == d_kernels) return LBCNN_ERR_INVALID_ARG;
+  int32_t* scratch = nullptr;
+  const int rc = evolve_static_scratch(h->device, &scratch);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  // The array still holds whatever the previous call (any handle, any stream) left in it.  The rank kernel overwrites
+  // order[] and rank_of[] completely when the accuracies are ordered numbers; clearing first makes the result independent of
+  // the array's history in every case (an accuracy that compares with nothing leaves order[] entries unwritten: they then
+  // read candidate 0, never a stale index from a larger, earlier population).
+  LB_CUDA_OK(cudaMemsetAsync(scratch, 0, (size_t)n_cand * 8, st));
+  return lb_launch_evolve(h, scratch, d_kernels, d_acc, n_cand, n_weights, n_elite, mut_ppm, seed, generation, d_next, st);
 }
