@@ -262,7 +262,7 @@ def ga_draw(seed: int, generation: int, child: int, i: int) -> int:
 
 def evolve_candidates(kernels: np.ndarray, acc: np.ndarray, n_elite: int, mut_ppm: int, seed: int, generation: int):
     """kernels int8 [K][n_weights] (+-1), acc [K] (the search's accuracies; a failed fit has -1).
-    R17: 1. rank the candidates by accuracy, best first, equal accuracies by index;
+    R17: 1. rank the candidates by accuracy, best first, equal accuracies by index (NaN counts as minus infinity);
          2. children 0 .. n_elite-1 are the n_elite best, unchanged, in rank order (elitism);
          3. every other child j draws two parents, each the better-ranked of two uniformly drawn candidates (binary
             tournament: draws 0,1 and 2,3, candidate = draw mod K), takes each tap from parent 1 or 2 by bit 0 of draw 4 + t
@@ -271,6 +271,7 @@ def evolve_candidates(kernels: np.ndarray, acc: np.ndarray, n_elite: int, mut_pp
     kernels = np.ascontiguousarray(kernels, dtype=np.int8)
     K, nw = kernels.shape
     a = np.asarray(acc, dtype=np.float32)
+    a = np.where(np.isnan(a), np.float32(-np.inf), a)          # R17: not-a-number ranks as minus infinity (after failed fits)
     order = sorted(range(K), key=lambda i: (-float(a[i]), i))
     rank = [0] * K
     for r, i in enumerate(order):

@@ -628,6 +628,21 @@ def test_ga_generation_properties():
     assert not np.array_equal(orc.evolve_candidates(ker, acc, 4, 20000, 8, 2)[0], some)
 
 
+def test_ga_nan_accuracy_ranks_last():
+    """DESIGN.md R17: an accuracy that is not a number (0 / 0 when a caller scores on an empty test set, or garbage passed in)
+    is ranked as minus infinity -- after the -1 of a failed fit, ties by index -- so order[] stays a permutation and the
+    elites are real candidates."""
+    rng = np.random.default_rng(5)
+    K, nw = 12, 40
+    ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+    acc = np.linspace(0.9, 0.5, K).astype(np.float32)
+    acc[2] = np.nan; acc[7] = np.nan; acc[4] = -1.0
+    nxt, par, order = orc.evolve_candidates(ker, acc, n_elite=K, mut_ppm=0, seed=1, generation=0)
+    assert sorted(order.tolist()) == list(range(K))
+    assert order.tolist() == [0, 1, 3, 5, 6, 8, 9, 10, 11, 4, 2, 7]
+    assert np.array_equal(nxt, ker[order])
+
+
 # ------------------------------------------------------------------------------------------------
 # gradient refinement of the output layer (SURVEY.md 8(f)-4; PAPER.md:98; DESIGN.md R18 = SPEC.md:324, 355)
 # ------------------------------------------------------------------------------------------------
@@ -645,6 +660,34 @@ def test_refine_identity_order_and_first_step():
     P[np.arange(37), y] -= 1.0
     G = H.T @ P / 37.0
     assert np.allclose(W1, W0 - 1e-2 * np.sign(G), atol=1e-12)
+
+
+def test_refine_adam_second_step_worked_example():
+    """The recursion past its first step (m, v, BOTH bias corrections with t = 2, the running step counter), against the
+    hand-worked values of tests/golden/worked_examples.txt [adam_two_steps] (R18 = SPEC.md:324, 355).  The same
+    two steps are reached three ways: two epochs of one batch (the counter must run on across epochs), one epoch of two
+    batches over the data written twice (it must run on inside an epoch; with n = 4 and an odd multiplier every batch of two
+    consecutive draws holds one sample of each kind, whatever the seed), and a single step for the intermediate w1."""
+    g = {k: v.ravel() for k, v in WORKED["adam_two_steps"].items()}
+    sym = lambda x: np.array([[x, -x], [-x, x]])
+    H = np.eye(2); y = np.array([0, 1]); W0 = np.zeros((2, 2))
+    kw = dict(lr=0.1, beta1=0.9, beta2=0.999, eps=1e-8)
+    W1, l1 = orc.refine_output_layer(H, y, W0, epochs=1, batch=2, **kw)
+    assert np.allclose(W1, sym(g["w1"][0]), rtol=0, atol=1e-15) and abs(l1[0] - g["loss"][0]) < 1e-15
+    for seed in (0, 1, 2, 3):
+        W2, l2 = orc.refine_output_layer(H, y, W0, epochs=2, batch=2, seed=seed, **kw)
+        assert np.allclose(W2, sym(g["w2"][0]), rtol=0, atol=2e-15), W2
+        assert np.allclose(l2, g["loss"], rtol=0, atol=2e-15)
+        H4 = np.vstack([H, H]); y4 = np.r_[y, y]
+        W2b, l2b = orc.refine_output_layer(H4, y4, W0, epochs=1, batch=2, seed=seed, **kw)
+        assert np.allclose(W2b, sym(g["w2"][0]), rtol=0, atol=2e-15), W2b
+        assert abs(l2b[0] - g["loss"].mean()) < 2e-15
+    # the golden block is consistent with itself (guards against a typo in the file, not against the oracle)
+    assert abs(g["m2"][0] - (0.9 * g["m1"][0] + 0.1 * g["q"][0])) < 1e-17
+    assert abs(g["mhat2"][0] - g["m2"][0] / g["c1"][0]) < 1e-16 and abs(g["vhat2"][0] - g["v2"][0] / g["c2"][0]) < 1e-16
+    assert abs(g["w2"][0] - g["w1"][0] - 0.1 * g["mhat2"][0] / (math.sqrt(g["vhat2"][0]) + 1e-8)) < 1e-16
+    # the two plausible mistakes named in the golden file land far away
+    assert abs(g["w2"][0] - 0.2338324893844486) > 0.03
 
 
 def test_refine_gradient_is_the_cross_entropy_gradient():
