@@ -105,13 +105,16 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                about, takes the all-fp64 factorisation.  _FP64: all-fp64 everywhere.  _MIXED: tensor-core
  *                                updates whenever the system has a trailing update -- the caller vouches that the system is not
  *                                singular up to the ridge (cond * 2^-27 << 1)
- *   LBCNN_OPT_CUDA_GRAPH         0: enqueue the solve's launch-bound block loop kernel by kernel instead of as a
- *                                captured CUDA graph (default 1)
  *   LBCNN_OPT_STREAM_ROWS        r > 0: streamed search ("limited GPU-RAM ... reduced fraction of the training
  *                                set"): the driver expands at most r samples at a time; the exact integer Gram and right-hand side
  *                                of the chunks add up (bit-identical to the unstreamed result), the test set is scored chunk by
  *                                chunk, so the features of the whole set never exist and the workspace no longer grows with
- *                                N_train / N_test.  Takes effect on the primal branch with the exact tensor-core Gram; 0 = off
+ *                                N_train / N_test.  It takes effect when the fit is the primal branch (F < N_train) with the exact
+ *                                tensor-core Gram and the fused right-hand side: no bias, integer features inside the three-digit
+ *                                envelope (LBCNN_H_INTEGER's bound), n_classes <= 128; otherwise the search runs resident and
+ *                                lbcnn_workspace_bytes says so through its size.  The exact Gram contracts at most 43690 samples per
+ *                                launch (int32 accumulators), so r > 43690 is served with chunks of 43690; N_train itself may be
+ *                                larger (the paper's full 60000): only the chunk is bounded.  0 = off
  *   LBCNN_OPT_DUAL_TRICK         0: the search driver forms W = H^T Z for EVERY candidate of the dual branch and scores H_te W (default 1:
  *                                when all candidates fit one chunk, train and test features are stacked, the exact Gram of the
  *                                stack carries the cross-Gram K_te = H_te H^T, the logits K_te (H H^T + I/C)^-1 T come out of the
@@ -128,7 +131,7 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                argmax), lbcnn_elm_score uses the fp64 kernel; _FP64: fp64 everywhere; _TENSOR: lbcnn_elm_score
  *                                takes the tensor-pipe kernel too (needs lbcnn_score_workspace_bytes of workspace; rows holding
  *                                non-integer or out-of-range features are re-evaluated in fp64, so any H stays correct) */
-enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, LBCNN_OPT_CUDA_GRAPH = 2, LBCNN_OPT_PANEL = 3, LBCNN_OPT_DEFLATE = 5,
+enum { LBCNN_OPT_FORCE_SIMT_EXPAND = 0, LBCNN_OPT_SOLVER = 1, /* 2: retired (never had an effect) */ LBCNN_OPT_PANEL = 3, LBCNN_OPT_DEFLATE = 5,
        LBCNN_OPT_SCORER = 6, LBCNN_OPT_MID_PANEL = 7, LBCNN_OPT_STREAM_ROWS = 8, LBCNN_OPT_DUAL_TRICK = 9 };
 enum { LBCNN_SCORER_AUTO = 0, LBCNN_SCORER_FP64 = 1, LBCNN_SCORER_TENSOR = 2 };
 enum { LBCNN_SOLVER_AUTO = 0, LBCNN_SOLVER_FP64 = 1, LBCNN_SOLVER_MIXED = 2 };

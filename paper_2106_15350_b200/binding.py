@@ -19,7 +19,7 @@ CONV_FULL, CONV_DEPTHWISE = 0, 1
 ACT_NONE, ACT_RELU = 0, 1
 H_INTEGER, FORCE_PRIMAL, FORCE_DUAL = 1, 2, 4
 EXPAND_SIMT, EXPAND_TENSOR = 0, 1
-OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_CUDA_GRAPH, OPT_PANEL, OPT_DEFLATE, OPT_SCORER, OPT_MID_PANEL, OPT_STREAM_ROWS, OPT_DUAL_TRICK = 0, 1, 2, 3, 5, 6, 7, 8, 9
+OPT_FORCE_SIMT_EXPAND, OPT_SOLVER, OPT_PANEL, OPT_DEFLATE, OPT_SCORER, OPT_MID_PANEL, OPT_STREAM_ROWS, OPT_DUAL_TRICK = 0, 1, 3, 5, 6, 7, 8, 9
 SCORER_AUTO, SCORER_FP64, SCORER_TENSOR = 0, 1, 2
 SOLVER_AUTO, SOLVER_FP64, SOLVER_MIXED = 0, 1, 2
 

@@ -84,7 +84,7 @@ int lbcnn_create(lbcnn_handle_t* h, int device) {
   if (!p) return LBCNN_ERR_NOMEM;
   p->device = device; p->n_sm = n_sm; p->max_smem_optin = smem_optin;
   p->ws = nullptr; p->ws_bytes = 0; p->launches = 0; p->profiling = 0;
-  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->use_graph = 1; p->panel = 1024; p->deflate = 16; p->dual_trick = 1; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
+  p->force_simt_expand = 0; p->solver = LBCNN_SOLVER_AUTO; p->panel = 1024; p->deflate = 16; p->dual_trick = 1; p->stream_rows = 0; p->mid_panel = 256; p->scorer = LBCNN_SCORER_AUTO;
   *h = p;
   return LBCNN_OK;
 }
@@ -96,7 +96,6 @@ int lbcnn_set_option(lbcnn_handle_t h, int option, int value) {
     case LBCNN_OPT_SOLVER:
       if (value != LBCNN_SOLVER_AUTO && value != LBCNN_SOLVER_FP64 && value != LBCNN_SOLVER_MIXED) return LBCNN_ERR_INVALID_ARG;
       h->solver = value; return LBCNN_OK;
-    case LBCNN_OPT_CUDA_GRAPH: h->use_graph = value ? 1 : 0; return LBCNN_OK;
     case LBCNN_OPT_DEFLATE:
       if (value < 0 || value > 64) return LBCNN_ERR_INVALID_ARG;
       h->deflate = value; return LBCNN_OK;
@@ -199,24 +198,33 @@ int lbcnn_get_op_stats(lbcnn_handle_t h, uint64_t* h_counts) {
 namespace {
 struct SearchPlan {
   FitPlan fit;
-  size_t xw_off, fit_off, htr_off, hte_off, w_off, sc_off, total;
+  size_t xw_off, fit_off, htr_off, hte_off, w_off, sc_off, gs_off, total;
   int stream; int64_t ntr_ws, nte_ws;      // streamed: rows of the train / test features resident at once
   int dual_kt;                             // dual branch scored through the kernel trick: train and test features stacked in one buffer
 };
 // xw1 = expander scratch per candidate (lb_expand_ws_bytes(.., 1)); kc = candidates per chunk
 // sr: streamed search (LBCNN_OPT_STREAM_ROWS) -- at most sr samples of the train / test set are resident at once
+// gs: bytes of one candidate's kernel set + bias (the slot a chunked kernel-trick search gathers its best candidate into)
 void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, int kc, uint32_t flags, size_t xw1, int64_t sr,
-                 SearchPlan* p, bool dual_kt = true) {
-  lb_fit_plan(n_train, F, c, kc, flags, &p->fit);
-  p->stream = (sr > 0 && (sr < n_train || sr < n_test) && p->fit.primal && p->fit.use_tc && p->fit.fuse_rhs) ? 1 : 0;
+                 size_t gs, SearchPlan* p, bool dual_kt = true) {
+  // The streamed plan is judged on the chunk it would contract per launch, not on the whole set: N_train = 60000 is beyond
+  // the exact Gram's int32 bound as one launch and inside it as chunks.  A request for longer chunks than that bound is
+  // served with chunks of the bound ("at most r samples at a time" still holds).
+  const int64_t sr_tr = (sr > LB_GRAM_TC_MAX_K) ? LB_GRAM_TC_MAX_K : sr;
+  const bool chunk_train = sr_tr > 0 && sr_tr < n_train;
+  lb_fit_plan(n_train, F, c, kc, flags, &p->fit, chunk_train ? sr_tr : 0);
+  p->stream = (sr > 0 && (chunk_train || sr < n_test) && p->fit.primal && p->fit.use_tc && p->fit.fuse_rhs) ? 1 : 0;
   if (p->stream) {
-    if (sr < n_train) { lb_fit_plan(n_train, F, c, kc, flags, &p->fit, sr); n_train = sr; }
+    if (chunk_train) n_train = sr_tr;
     if (sr < n_test) n_test = sr;
+  } else if (chunk_train) {
+    lb_fit_plan(n_train, F, c, kc, flags, &p->fit);      // not streamable (dual branch, bias, > 128 classes, ...): the resident plan
   }
   p->ntr_ws = n_train; p->nte_ws = n_test;
-  // dual branch with the exact tensor-core Gram and every candidate in ONE chunk: test rows are stacked behind the train rows,
-  // the Gram of the stack carries the cross-Gram and the scores come out of the factorisation (fit.cu, DualScore)
-  p->dual_kt = (dual_kt && !p->fit.primal && p->fit.use_tc && kc >= n_cand) ? 1 : 0;
+  // dual branch with the exact tensor-core Gram: test rows are stacked behind the train rows, the Gram of the stack carries
+  // the cross-Gram and the scores come out of the factorisation (fit.cu, DualScore).  Taken whatever the chunk size, so that
+  // the decisions (correct[], acc, best) do not depend on how much workspace the caller gave.
+  p->dual_kt = (dual_kt && !p->fit.primal && p->fit.use_tc) ? 1 : 0;
   if (p->dual_kt) lb_fit_plan(n_train, F, c, kc, flags, &p->fit, 0, n_test);
   size_t off = 0;
   p->xw_off = off;  off += (size_t)lb_align_up((int64_t)(xw1 * (size_t)kc), 256);
@@ -226,6 +234,8 @@ void plan_search(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, 
   p->w_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * F * c * 4, 256);
   // scratch of the tensor-core scorer (integer features only; it may still be left unused at run time)
   p->sc_off = off;  if (flags & LBCNN_H_INTEGER) off += lb_score_tc_ws_bytes(n_test, F, c, kc);
+  // kernel-trick search in several chunks: slot for the best candidate's kernel set, bias and the info word of its re-fit
+  p->gs_off = off;  if (p->dual_kt && kc < n_cand) off += (size_t)lb_align_up((int64_t)gs, 256) + 256;
   p->total = off;
 }
 // The driver's features are exact integers; inside the digit envelope of the exact tensor-core Gram (three balanced
@@ -245,20 +255,21 @@ uint32_t search_fit_flags(const ArchShape& s, bool has_bias) {
   return (!has_bias && s.max_abs <= LB_H_INTEGER_MAX) ? LBCNN_H_INTEGER : 0u;
 }
 // largest chunk size whose plan fits in `bytes` (0 if none)
-int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, int64_t sr, size_t bytes,
-              bool dual_kt = true) {
+int fit_chunk(int64_t F, int64_t n_train, int64_t n_test, int c, int n_cand, uint32_t flags, size_t xw1, int64_t sr, size_t gs,
+              size_t bytes, bool dual_kt = true) {
   SearchPlan p;
-  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, sr, &p, dual_kt);
+  plan_search(F, n_train, n_test, c, n_cand, n_cand, flags, xw1, sr, gs, &p, dual_kt);
   if (p.total <= bytes) return n_cand;
   int lo = 0, hi = n_cand;   // plan(lo) fits (lo = 0 means none), plan(hi) does not
   while (hi - lo > 1) {
     const int mid = lo + (hi - lo) / 2;
-    plan_search(F, n_train, n_test, c, n_cand, mid, flags, xw1, sr, &p);
+    plan_search(F, n_train, n_test, c, n_cand, mid, flags, xw1, sr, gs, &p, dual_kt);
     if (p.total <= bytes) lo = mid; else hi = mid;
   }
   return lo;
 }
 // expander scratch per candidate; a NULL handle (pure host arithmetic) assumes the B200's 227 KB of shared memory
+size_t gather_slot_bytes(const ArchShape& s) { return (size_t)lb_align_up(s.n_weights, 256) + (size_t)s.n_bias * 4; }
 size_t expand_ws_per_cand(lbcnn_handle_t h, const ArchShape& s, bool has_bias) {
   lbcnn_handle_s tmp{};
   tmp.max_smem_optin = 232448;
@@ -277,17 +288,23 @@ int lbcnn_workspace_bytes(lbcnn_handle_t h, const lbcnn_arch_t* arch, int64_t n_
   const uint32_t flags = search_fit_flags(s, false);     // the bias-free plan is the larger one (digit planes)
   const size_t xw1 = expand_ws_per_cand(h, s, false);
   const int64_t sr = h ? h->stream_rows : 0;
-  SearchPlan p1;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, sr, &p1);
+  const size_t gs = gather_slot_bytes(s);
+  SearchPlan p1, p1n;
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, sr, gs, &p1);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, 1, flags, xw1, sr, gs, &p1n, false);
+  if (p1n.total > p1.total) p1 = p1n;
   if (min_bytes) *min_bytes = p1.total;
   int kc = n_cand;
   if (budget_bytes) {
-    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, sr, budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0);
+    const size_t room = budget_bytes > LB_WS_HEAD ? budget_bytes - LB_WS_HEAD : 0;
+    kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, sr, gs, room);
+    const int kn = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, flags, xw1, sr, gs, room, false);
+    if (kn < kc) kc = kn;                                  // a size both settings of LBCNN_OPT_DUAL_TRICK can run in
     if (kc < 1) kc = 1;
   }
   SearchPlan p, pn;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, &p);
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, &pn, false);   // LBCNN_OPT_DUAL_TRICK off: the larger one fits both
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, gs, &p);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, flags, xw1, sr, gs, &pn, false);   // LBCNN_OPT_DUAL_TRICK off: the larger one fits both
   if (pn.total > p.total) p = pn;
   if (min_bytes) *min_bytes += LB_WS_HEAD;
   *bytes = p.total + LB_WS_HEAD;
@@ -426,11 +443,12 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
   const size_t xw1 = lb_expand_ws_bytes(h, s, d_bias != nullptr, 1);
   const int64_t sr = h->stream_rows;
   const bool want_kt = h->dual_trick != 0 && h->scorer != LBCNN_SCORER_FP64;
-  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, sr, ws_bytes, want_kt);
+  const size_t gs = gather_slot_bytes(s);
+  int kc = fit_chunk(s.F, n_train, n_test, n_classes, n_cand, fflags, xw1, sr, gs, ws_bytes, want_kt);
   if (kc < 1) return LBCNN_ERR_WORKSPACE;
   if (kc > 65535) kc = 65535;                          // grid.y / grid.z of the batched kernels
   SearchPlan p;
-  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, sr, &p, want_kt);
+  plan_search(s.F, n_train, n_test, n_classes, n_cand, kc, fflags, xw1, sr, gs, &p, want_kt);
   char* base = reinterpret_cast<char*>(ws);
   float* Htr = reinterpret_cast<float*>(base + p.htr_off);
   float* Hte = reinterpret_cast<float*>(base + p.hte_off);
@@ -461,10 +479,26 @@ static int search_impl(lbcnn_handle_t h, void* ws, size_t ws_bytes, const lbcnn_
       const DualScore dsc{d_test_labels, d_correct + k0};
       rc = lb_launch_fit(h, base + p.fit_off, fp, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, kn, Wk, d_info + k0, st, nullptr, &dsc);
       if (rc) return rc;
+      if (k0 + kn < n_cand) continue;                  // more chunks to come
       rc = lb_launch_finish(h, d_correct, d_info, n_test, n_cand, d_acc, d_best, nullptr, wel, nullptr, st);
       if (rc) return rc;
-      if (d_W_best) return lb_launch_w_best_dual(h, base + p.fit_off, fp, d_best, Htr, n_train, s.F, hs, n_classes, d_W_best, st);
-      return LBCNN_OK;
+      if (!d_W_best) return LBCNN_OK;
+      if (kc >= n_cand)                                // one chunk: the best candidate's features and solution are still here
+        return lb_launch_w_best_dual(h, base + p.fit_off, fp, d_best, Htr, n_train, s.F, hs, n_classes, d_W_best, st);
+      // several chunks: the best candidate's chunk may be gone and its index exists on the device only.  Its kernel set is
+      // gathered into a slot of its own and the candidate is fitted once more, alone, with the explicit W = H^T Z.
+      int8_t* gker = reinterpret_cast<int8_t*>(base + p.gs_off);
+      int32_t* gbias = reinterpret_cast<int32_t*>(base + p.gs_off + lb_align_up(s.n_weights, 256));
+      int32_t* ginfo = reinterpret_cast<int32_t*>(base + p.gs_off + lb_align_up((int64_t)gs, 256));
+      rc = lb_launch_gather_best(h, d_best, d_kernels, s.n_weights, d_bias, s.n_bias, gker, gbias, st);
+      if (rc) return rc;
+      FitPlan f1;
+      lb_fit_plan(n_train, s.F, n_classes, 1, fflags, &f1);
+      f1.allow_tc = fp.allow_tc;
+      if (f1.total > p.fit.total) return LBCNN_ERR_WORKSPACE;
+      rc = lb_launch_expand(h, s, 1.0f, d_train, n_train, gker, d_bias ? gbias : nullptr, 1, Htr, base + p.xw_off, xw1, st, false);
+      if (rc) return rc;
+      return lb_launch_fit(h, base + p.fit_off, f1, Htr, n_train, s.F, hs, d_train_labels, n_classes, C, 1, d_W_best, ginfo, st);
     }
     lb_fit_plan(n_train, s.F, n_classes, kn, fflags, &fp, p.ntr_ws);
     fp.allow_tc = arch_allows_tc_solver(s) ? 1 : 0;

@@ -17,15 +17,18 @@ __host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long 
   return z ^ (z >> 31);
 }
 
+// a NaN accuracy compares with nothing: ranked as minus infinity (R17) so that the ranks stay a permutation
+__device__ __forceinline__ float ga_key(float a) { return (a != a) ? __int_as_float(0xff800000) : a; }
+
 // rank by accuracy, best first, equal accuracies by index: order[rank] = candidate, rank_of[candidate] = rank
 __global__ void __launch_bounds__(256) ga_rank_kernel(const float* __restrict__ acc, int K, int32_t* __restrict__ order,
                                                       int32_t* __restrict__ rank_of) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= K) return;
-  const float ai = acc[i];
+  const float ai = ga_key(acc[i]);
   int r = 0;
   for (int j = 0; j < K; ++j) {
-    const float aj = acc[j];
+    const float aj = ga_key(acc[j]);
     r += (aj > ai || (aj == ai && j < i)) ? 1 : 0;
   }
   order[r] = i;
@@ -114,9 +117,8 @@ extern "C" int lbcnn_evolve_candidates_static(lbcnn_handle_t h, const int8_t* d_
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   // The array still holds whatever the previous call (any handle, any stream) left in it.  The rank kernel overwrites
-  // order[] and rank_of[] completely when the accuracies are ordered numbers; clearing first makes the result independent of
-  // the array's history in every case (an accuracy that compares with nothing leaves order[] entries unwritten: they then
-  // read candidate 0, never a stale index from a larger, earlier population).
+  // order[0 .. n_cand) and rank_of[0 .. n_cand) completely (the ranks are a permutation); the clear is there so that this
+  // call's result can never depend on the array's history, whatever a later change to the kernels does.
   LB_CUDA_OK(cudaMemsetAsync(scratch, 0, (size_t)n_cand * 8, st));
   return lb_launch_evolve(h, scratch, d_kernels, d_acc, n_cand, n_weights, n_elite, mut_ppm, seed, generation, d_next, st);
 }

@@ -247,7 +247,9 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   if (flags & LBCNN_FORCE_DUAL) primal = 0;
   p->primal = primal;
   p->dim = primal ? F : n;
-  p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
+  // the int32 bound of the exact Gram is on the samples contracted per LAUNCH: a streamed plan (n_ws < n) adds the exact
+  // fp64 Grams of chunks of n_ws rows, so its bound is on n_ws, not on n (N = 60000 streams in chunks of <= 43690)
+  p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(primal ? n_ws : n, F, primal != 0)) ? 1 : 0;
   p->n_extra = (!primal && p->use_tc && n_extra > 0) ? n_extra : 0;
   p->rows = p->dim + n_classes + p->n_extra;
   p->a_bytes = (size_t)p->rows * (size_t)p->dim * sizeof(double);
@@ -255,7 +257,6 @@ void lb_fit_plan(int64_t n, int64_t F, int n_classes, int n_cand, uint32_t flags
   p->perm_off = off; off += (size_t)lb_align_up(n * 4, 256);
   p->off_off = off;  off += (size_t)lb_align_up(((int64_t)n_classes + 1) * 4, 256);
   p->a_off = off;    off += (size_t)lb_align_up((int64_t)p->a_bytes * n_cand, 256);
-  p->use_tc = ((flags & LBCNN_H_INTEGER) && lb_gram_tc_usable(n, F, primal != 0)) ? 1 : 0;
   p->tc_off = off;   p->fuse_rhs = (p->use_tc && primal && lb_gram_tc_fuse_rhs(F, n_classes)) ? 1 : 0;
   if (p->use_tc) off += lb_gram_tc_ws_bytes(n_ws + p->n_extra, F, n_cand, p->fuse_rhs ? n_classes : 0);
   p->lg_off = off;   off += (size_t)lb_align_up((int64_t)n_cand * p->n_extra * n_classes * 8, 256);

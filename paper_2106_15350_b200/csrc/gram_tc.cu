@@ -413,7 +413,7 @@ bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes) { (void)F; return n_classes <
 // (primal) or over the features (dual)
 bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal) {
   const int64_t k = primal ? n : F;
-  return n >= 1 && F >= 1 && k <= 43690 && n < (1 << 30) && F < (1 << 30);
+  return n >= 1 && F >= 1 && k <= LB_GRAM_TC_MAX_K && n < (1 << 30) && F < (1 << 30);
 }
 
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug) {

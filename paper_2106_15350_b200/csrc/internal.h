@@ -24,7 +24,6 @@ struct lbcnn_handle_s {
   int mid_panel;                    // width of the fp64-stepped blocks inside a panel (three-level factorisation); 0 = two levels
   int64_t stream_rows;              // search driver: samples expanded / accumulated per chunk (0 = all at once)
   int dual_trick;                   // search driver, dual branch: score through the cross-Gram (kernel trick), W for the best only
-  int use_graph;                    // capture the launch-bound solve loops in CUDA graphs
   int profiling;                    // record CUDA events around each phase of the path
   std::vector<LbPhaseRec> recs;
 };
@@ -119,6 +118,7 @@ int lb_launch_fit(lbcnn_handle_s* h, void* ws, const FitPlan& p, const float* d_
                   cudaStream_t st, const FitStream* fs = nullptr, const DualScore* ds = nullptr);
 
 // ---- exact integer Gram on tcgen05 (gram_tc.cu) ---------------------------------------------------
+constexpr int64_t LB_GRAM_TC_MAX_K = 43690;   // longest contraction whose int32 accumulators stay exact: 3 * 128^2 * k < 2^31
 bool lb_gram_tc_usable(int64_t n, int64_t F, bool primal);
 size_t lb_gram_tc_ws_bytes(int64_t n, int64_t F, int n_cand, int c_aug);
 bool lb_gram_tc_fuse_rhs(int64_t F, int n_classes);   // right-hand side as one-hot columns of the Gram's digit plane 0
@@ -168,6 +168,8 @@ size_t lb_refine_ws_bytes(int64_t F, int n_classes, int batch, int epochs);
 int lb_launch_refine(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, int64_t F, float h_scale, const int32_t* d_labels,
                      int c, const lbcnn_refine_t& cfg, float* d_W, float* d_loss, cudaStream_t st);
 int lb_launch_zero_i32(lbcnn_handle_s* h, int32_t* p, int64_t n, cudaStream_t st);
+int lb_launch_gather_best(lbcnn_handle_s* h, const int32_t* d_best, const int8_t* d_kernels, int64_t n_weights,
+                          const int32_t* d_bias, int64_t n_bias, int8_t* ker_out, int32_t* bias_out, cudaStream_t st);
 int lb_launch_finish(lbcnn_handle_s* h, const int32_t* d_correct, const int32_t* d_info, int64_t n_test, int n_cand,
                      float* d_acc, int32_t* d_best, const float* d_W_all, int64_t w_elems, float* d_W_best,
                      cudaStream_t st);

@@ -113,7 +113,8 @@ int lb_launch_refine(lbcnn_handle_s* h, void* ws, const float* d_H, int64_t n, i
   const unsigned gw = (unsigned)((nw + 255) / 256);
   const double hs = (double)h_scale;
   int rc;
-  rf_init_kernel<<<gw > 1 ? gw : 1, 256, 0, st>>>(d_W, nw, Wd, m, v, loss, cfg.epochs);
+  const unsigned gi = (unsigned)(((nw > cfg.epochs ? nw : cfg.epochs) + 255) / 256);   // also covers loss[0 .. epochs)
+  rf_init_kernel<<<gi > 1 ? gi : 1, 256, 0, st>>>(d_W, nw, Wd, m, v, loss, cfg.epochs);
   h->launches += 1;
   long long t = 0;
   for (int e = 0; e < cfg.epochs; ++e) {

@@ -153,7 +153,27 @@ __global__ void finish_kernel(const int32_t* __restrict__ correct, const int32_t
   }
 }
 
+// kernel set (and bias) of candidate best[0] copied to a slot of its own: a chunked dual-branch search re-fits its best
+// candidate after the last chunk, and the index exists on the device only
+__global__ void gather_best_kernel(const int32_t* __restrict__ best, const int8_t* __restrict__ ker, long long nw,
+                                   const int32_t* __restrict__ bias, long long nb, int8_t* __restrict__ ker_out,
+                                   int32_t* __restrict__ bias_out) {
+  const long long b = best[0];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nw) ker_out[t] = ker[b * nw + t];
+  if (bias && t < nb) bias_out[t] = bias[b * nb + t];
+}
+
 }  // namespace
+
+int lb_launch_gather_best(lbcnn_handle_s* h, const int32_t* d_best, const int8_t* d_kernels, int64_t n_weights,
+                          const int32_t* d_bias, int64_t n_bias, int8_t* ker_out, int32_t* bias_out, cudaStream_t st) {
+  const int64_t m = n_weights > n_bias ? n_weights : n_bias;
+  gather_best_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(d_best, d_kernels, n_weights, d_bias, n_bias, ker_out, bias_out);
+  h->launches += 1;
+  LB_CUDA_OK(cudaGetLastError());
+  return LBCNN_OK;
+}
 
 int lb_launch_score(lbcnn_handle_s* h, const float* d_H, int64_t n, int64_t F, float h_scale, const float* d_W,
                     int n_classes, const int32_t* d_labels, int n_cand, int32_t* d_pred, int32_t* d_correct,

@@ -432,6 +432,47 @@ def test_refine_output_layer_matches_oracle(handle, name, ntr, nte, epochs, batc
     assert (pred.cpu().numpy()[0] == po).mean() >= TOL_LABEL_AGREE
 
 
+def test_genetic_generator_nan_accuracy(handle):
+    """A NaN accuracy (0 / 0 from an empty test set upstream, or garbage passed in) ranks as minus infinity (R17): the
+    ranks stay a permutation, the elites are real candidates and the result equals the oracle's byte for byte."""
+    rng = np.random.default_rng(77)
+    K, nw = 40, 129
+    ker = (rng.integers(0, 2, size=(K, nw)) * 2 - 1).astype(np.int8)
+    acc = rng.integers(50, 60, size=K).astype(np.float32) / 100.0
+    acc[[3, 17, 18, 39]] = np.nan
+    acc[5] = -1.0
+    for elite in (K, 6):
+        ref, _, order = orc.evolve_candidates(ker, acc, elite, 10000, 4, 3)
+        assert order.tolist()[-5:] == [5, 3, 17, 18, 39]
+        nxt = handle.evolve_candidates(_dev(ker), _dev(acc), elite, 10000, 4, 3).cpu().numpy()
+        assert np.array_equal(nxt, ref)
+        nxt = handle.evolve_candidates_static(_dev(ker), _dev(acc), elite, 10000, 4, 3).cpu().numpy()
+        assert np.array_equal(nxt, ref)
+
+
+def test_refine_adam_worked_example_and_many_epochs(handle):
+    """(1) The hand-worked two Adam steps of tests/golden/worked_examples.txt [adam_two_steps] (R18) on the GPU: W after
+    step 2 = 0.19958968129158736 on the diagonal, reached across epochs and inside one epoch.  W comes back as fp32.
+    (2) More epochs than F * n_classes rounded up to a block (the loss accumulators beyond the weight count must start at
+    zero): 300 epochs on a 2 x 2 layer against the oracle, twice in the same workspace."""
+    w2 = 0.19958968129158736
+    want = np.array([[w2, -w2], [-w2, w2]])
+    H = torch.eye(2, device="cuda"); y = torch.tensor([0, 1], dtype=torch.int32, device="cuda"); W0 = torch.zeros((2, 2), device="cuda")
+    W, loss = handle.refine_output_layer(H, y, W0, epochs=2, batch=2, lr=0.1, seed=3)
+    assert np.allclose(W.cpu().numpy(), want, rtol=0, atol=2e-8)
+    assert np.allclose(loss.cpu().numpy(), [0.6931471805599453, 0.5981388729829197], rtol=0, atol=1e-7)
+    H4 = torch.cat([H, H]).contiguous(); y4 = torch.cat([y, y]).contiguous()
+    W, _ = handle.refine_output_layer(H4, y4, W0, epochs=1, batch=2, lr=0.1, seed=3)
+    assert np.allclose(W.cpu().numpy(), want, rtol=0, atol=2e-8)
+    rng = np.random.default_rng(9)
+    Hn = rng.normal(size=(33, 2)).astype(np.float32); yn = rng.integers(0, 2, size=33).astype(np.int32)
+    for rep in range(2):
+        Wg, lg = handle.refine_output_layer(_dev(Hn), _dev(yn), W0, epochs=300, batch=16, lr=1e-2, seed=rep)
+        Wo, lo = orc.refine_output_layer(Hn.astype(np.float64), yn, np.zeros((2, 2)), 300, 16, 1e-2, seed=rep)
+        assert np.allclose(lg.cpu().numpy(), lo, rtol=1e-5, atol=1e-7)
+        assert _fro(Wg.cpu().numpy().astype(np.float64), Wo) <= 1e-5
+
+
 def _search_both(handle, w, budget=None):
     trx, try_, tex, tey = synth.make_dataset(w)
     ker = synth.make_kernels(w)
@@ -594,6 +635,45 @@ def test_streamed_search_equals_resident(handle, name, ntr, nte, K, rows):
         assert torch.equal(a[k], b[k]), k
     assert (b["info"].cpu().numpy() == 0).all()
     handle.set_workspace(None)
+    if name != "vggface":      # the streamed result against the ORACLE, not only against the resident CUDA search
+        ref = orc.search(_orc_arch(w), trx, try_, tex, tey, w.n_classes, w.C, ker, feature_scale=w.feature_scale, keep=True)
+        _check_search(handle, w, {k: v.cpu().numpy() for k, v in b.items()}, ref)
+
+
+def test_streamed_search_beyond_the_int32_chunk_bound(handle):
+    """N_train above 43690 (the exact Gram's int32 bound per launch; the paper's own case is the full 60000 of MNIST,
+    PAPER.md:29, 104): LBCNN_OPT_STREAM_ROWS must still stream -- the bound is on the chunk, not on N -- and a request for
+    chunks longer than the bound is served with chunks of the bound.  Checked against the oracle; that it really streamed is
+    shown by the phase record (one Gram bracket per chunk, no separate right-hand side) and the int8 operation counter."""
+    w = _small("tiny_mnist", 45000, 700, 3)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w)
+    arch = lb.arch_of(w)
+    F = lb.feature_dim(arch)[0]
+    args = (arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    ref = orc.search(_orc_arch(w), trx, try_, tex, tey, w.n_classes, w.C, ker, feature_scale=w.feature_scale, keep=True)
+    resident_H = w.n_cand * w.n_train * F * 4
+    try:
+        for rows, chunks in ((20000, 3), (44000, 2)):       # 44000 > 43690: served as 43690 + 1310
+            handle.set_option(lb.OPT_STREAM_ROWS, rows)
+            small = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, handle=handle)[0]
+            if rows == 20000:
+                assert small < resident_H, (rows, small, resident_H)
+            handle.set_workspace(None)
+            handle.ensure_workspace(small)
+            handle.op_stats()
+            handle.set_profiling(True)
+            got = handle.search_candidates(*args)
+            ph = handle.phase_times()
+            handle.set_profiling(False)
+            # one Gram bracket per chunk of samples, no separate right-hand-side phase, and the int8 Gram counter moved:
+            # the streamed tensor-core plan ran, not the resident fp64 one
+            assert ph["gram"][1] == chunks and ph["rhs"][1] == 0, ph
+            assert handle.op_stats()["gram_int8_tmac"] > 0
+            _check_search(handle, w, {k: v.cpu().numpy() for k, v in got.items()}, ref)
+    finally:
+        handle.set_option(lb.OPT_STREAM_ROWS, 0)
+        handle.set_workspace(None)
 
 
 @pytest.mark.parametrize("name,ntr,nte,K", [("orl", 280, 120, 16), ("vggface", 700, 300, 3), ("paper_anchor", 300, 200, 2)])
@@ -619,6 +699,25 @@ def test_dual_branch_kernel_trick_equals_explicit_w(handle, name, ntr, nte, K):
     for k in ("acc", "correct", "info", "best"):
         assert torch.equal(a[k], b[k]), k
     assert _fro(a["W_best"].cpu().numpy().astype(np.float64), b["W_best"].cpu().numpy().astype(np.float64)) <= 1e-6
+
+
+@pytest.mark.parametrize("name,ntr,nte,K", [("orl", 280, 120, 16), ("vggface", 700, 300, 5)])
+def test_dual_branch_chunked_equals_unchunked(handle, name, ntr, nte, K):
+    """The decisions of a dual-branch search (correct[], acc, info, best / worst) must not depend on how much workspace the
+    caller gave: the kernel-trick scoring is taken chunk by chunk as well, and the best candidate -- whose chunk may be gone by
+    then -- is fitted once more on its own for W_best.  W_best then comes from the explicit W = H^T Z instead of the
+    factorisation's rows: equal up to the rounding order of fp64 sums.  Both runs against the oracle too."""
+    w = _small(name, ntr, nte, K)
+    arch = lb.arch_of(w)
+    full, mn = lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)
+    a, ref = _search_both(handle, w)
+    for budget in (mn + (full - mn) // 3, mn):          # a few candidates per chunk; one candidate per chunk
+        assert lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand, budget)[0] < full
+        b, _ = _search_both(handle, w, budget=budget)
+        for k in ("acc", "correct", "info", "best"):
+            assert np.array_equal(a[k], b[k]), (k, budget)
+        assert _fro(b["W_best"].astype(np.float64), a["W_best"].astype(np.float64)) <= 1e-6
+    _check_search(handle, w, b, ref)
 
 
 def test_search_chunked_equals_unchunked(handle):
