@@ -309,7 +309,7 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
             step(out)
             b.record()
         barrier()
-        return sum(a.elapsed_time(b) for a, b in evs)
+        return [a.elapsed_time(b) for a, b in evs]
 
     out = step()
     for _ in range(max(warmup - 2, 0)):
@@ -328,10 +328,10 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     barrier()
     # ---- timed region: device-resident inputs, per-phase events OFF ----
     n0 = h.launch_count()
-    ms = timed(steps)
+    ms_steps = timed(steps)
     launches = h.launch_count() - n0
     clocks = sampler.stop()
-    ms = replicas.max_over_ranks(ms, dev)
+    ms = replicas.max_over_ranks(sum(ms_steps), dev)
     # ---- second pass, per-phase CUDA events ON: where the time goes (not part of `value`) ----
     h.op_stats()                      # reset the device-side int8 operation counters
     h.set_profiling(True)
@@ -344,7 +344,7 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     if (info != 0).any() or not np.isfinite(acc).all():
         raise RuntimeError("fit failed for some candidate: info=%s" % info.tolist())
 
-    res = dict(w=w, K=K, F=F, ms=ms, launches=launches, clocks=clocks, phase_ms=phase_ms, stats=stats, acc=acc,
+    res = dict(w=w, K=K, F=F, ms=ms, ms_steps=sorted(ms_steps), launches=launches, clocks=clocks, phase_ms=phase_ms, stats=stats, acc=acc,
                best=int(out["best"][0].item()), l2_note=l2_note, data=(trx, try_, tex, tey), e2e=None)
     if with_e2e:
         # ---- e2e: host (pinned) buffers through lbcnn_search_candidates_host, copies inside the timed region ----
@@ -367,6 +367,26 @@ def _measure(lb, replicas, synth, torch, np, dist, name, steps, warmup, ws_gb, w
     return res
 
 
+def _cpu_baseline(np, w, data, K, acc, nc_override):
+    """the oracle as it stands on the host cores, on a bounded sample (about 10-30 s of host work) of workload `w`:
+    CPU_SAMPLE's (candidates, N_train, N_test); `acc` = the GPU's accuracies of the same candidates (compared at full N)."""
+    trx, try_, tex, tey = data
+    nc, ntr, nte = CPU_SAMPLE.get(w.name, (1, w.n_train, w.n_test))
+    if nc_override:
+        nc = nc_override
+    nc = min(nc, K)
+    full = (ntr >= w.n_train and nte >= w.n_test)
+    dt, r, threads = _oracle_sample(w, trx[:ntr], try_[:ntr], tex[:nte], tey[:nte], nc, first=0)
+    if full:
+        ok = bool(np.all(np.abs(r["acc"] - acc[:nc].astype(np.float64)) * 100.0 <= 0.2))
+        sample = ("first %d of %d candidates of the same workload at full N (%.1f s); accuracies agree with the "
+                  "GPU's within 0.2 pp: %s" % (nc, K, dt, ok))
+    else:
+        sample = ("first %d of %d candidates of the same workload on its first %d train / %d test samples "
+                  "(%.1f s; the full-N oracle run would take minutes per candidate)" % (nc, K, ntr, nte, dt))
+    return dict(value=nc / dt, unit=UNIT, cores=threads, kind="oracle", sample=sample)
+
+
 OPTIONS = []       # (option, value) pairs from --solver / --panel (measurement switches; default = the product path)
 
 DTYPE = ("int8 x int8 -> int32 tensor-core expander, Gram and Cholesky trailing updates (exact digit products), "
@@ -385,8 +405,10 @@ def _summary(res, steps, world, replicas, peaks):
     if roofline:
         roofline["kernel"] = dominant
     acc = res["acc"]
+    med = res["ms_steps"][len(res["ms_steps"]) // 2] if len(res["ms_steps"]) % 2 else \
+        0.5 * (res["ms_steps"][len(res["ms_steps"]) // 2 - 1] + res["ms_steps"][len(res["ms_steps"]) // 2])
     return dict(value=replicas.job_throughput(world, res["K"], steps, total_s), ms_per_step=res["ms"] / steps,
-                e2e=res["e2e"], gpu_launches=int(res["launches"]), clocks=res["clocks"], roofline=roofline, phases=roofs,
+                ms_per_step_median=med, e2e=res["e2e"], gpu_launches=int(res["launches"]), clocks=res["clocks"], roofline=roofline, phases=roofs,
                 accuracy=dict(best=float(acc.max()), worst=float(acc.min()), best_index=res["best"]),
                 config=_config(w, res["K"], res["l2_note"]))
 
@@ -507,12 +529,15 @@ def run_cuda(args):
     if not args.no_per_config and not args.n_cand:
         for name in ("tiny_mnist", "mnist", "gtsrb", "orl", "vggface"):
             if name == args.workload:
-                per_config[name] = {k: main[k] for k in ("value", "ms_per_step", "e2e", "gpu_launches", "clocks", "phases", "accuracy", "config")}
+                per_config[name] = {k: main[k] for k in ("value", "ms_per_step", "ms_per_step_median", "e2e", "gpu_launches", "clocks", "phases", "accuracy", "config")}
+                per_config[name]["steps"] = args.steps
                 continue
             r = _measure(*common, name, args.per_config_steps, 3, args.ws_gb, world, rank, local)
             sm = _summary(r, args.per_config_steps, world, replicas, peaks)
             sm["steps"] = args.per_config_steps
             del sm["roofline"]
+            if rank == 0 and world == 1 and not args.no_cpu_baseline:
+                sm["cpu_baseline"] = _cpu_baseline(np, r["w"], r["data"], r["K"], r["acc"], 0)
             per_config[name] = sm
 
     extras = None
@@ -533,22 +558,9 @@ def run_cuda(args):
     if extras:
         line["extras"] = extras
     if not args.no_cpu_baseline:
-        # bounded sample (about 10-30 s of host work): (candidates, N_train, N_test) of the same workload
-        trx, try_, tex, tey = res["data"]
-        nc, ntr, nte = CPU_SAMPLE.get(w.name, (1, w.n_train, w.n_test))
-        if args.ref_cands_baseline:
-            nc = args.ref_cands_baseline
-        nc = min(nc, K)
-        full = (ntr >= w.n_train and nte >= w.n_test)
-        dt, r, threads = _oracle_sample(w, trx[:ntr], try_[:ntr], tex[:nte], tey[:nte], nc, first=0)
-        if full:
-            ok = bool(np.all(np.abs(r["acc"] - acc[:nc].astype(np.float64)) * 100.0 <= 0.2))
-            sample = ("first %d of %d candidates of the same workload at full N (%.1f s); accuracies agree with the "
-                      "GPU's within 0.2 pp: %s" % (nc, K, dt, ok))
-        else:
-            sample = ("first %d of %d candidates of the same workload on its first %d train / %d test samples "
-                      "(%.1f s; the full-N oracle run would take minutes per candidate)" % (nc, K, ntr, nte, dt))
-        line["cpu_baseline"] = dict(value=nc / dt, unit=UNIT, cores=threads, kind="oracle", sample=sample)
+        line["cpu_baseline"] = _cpu_baseline(np, w, res["data"], K, acc, args.ref_cands_baseline)
+        if w.name in per_config:
+            per_config[w.name]["cpu_baseline"] = line["cpu_baseline"]
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -575,7 +587,7 @@ def main():
     ap.add_argument("--scorer", default="", choices=["", "auto", "fp64", "tensor"], help="LBCNN_OPT_SCORER (measurement)")
     ap.add_argument("--no-extras", action="store_true", help="skip the measurements of the SURVEY.md 8(f) rows")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (the other four workloads)")
-    ap.add_argument("--per-config-steps", type=int, default=3, help="timed steps for each per_config workload")
+    ap.add_argument("--per-config-steps", type=int, default=5, help="timed steps for each per_config workload")
     args = ap.parse_args()
     if args.warmup < 1 or args.steps < 1:
         ap.error("--steps and --warmup must be >= 1")

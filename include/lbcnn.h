@@ -105,6 +105,12 @@ int lbcnn_destroy(lbcnn_handle_t h);
  *                                about, takes the all-fp64 factorisation.  _FP64: all-fp64 everywhere.  _MIXED: tensor-core
  *                                updates whenever the system has a trailing update -- the caller vouches that the system is not
  *                                singular up to the ridge (cond * 2^-27 << 1)
+ *                                Failure mode of _AUTO / _MIXED: there is no automatic retry.  On a system that IS singular up to the
+ *                                ridge (a candidate whose last layer holds the same kernel twice, or nearly collinear features)
+ *                                the slice error can drive a pivot non-positive: the candidate is then flagged (d_info[k] > 0,
+ *                                acc -1, left out of best / worst), never returned wrong, where the all-fp64 factorisation would
+ *                                have succeeded.  To tell a precision breakdown from a truly indefinite system, run the flagged
+ *                                candidates again under LBCNN_SOLVER_FP64
  *   LBCNN_OPT_STREAM_ROWS        r > 0: streamed search ("limited GPU-RAM ... reduced fraction of the training
  *                                set"): the driver expands at most r samples at a time; the exact integer Gram and right-hand side
  *                                of the chunks add up (bit-identical to the unstreamed result), the test set is scored chunk by

@@ -720,6 +720,50 @@ def test_dual_branch_chunked_equals_unchunked(handle, name, ntr, nte, K):
     _check_search(handle, w, b, ref)
 
 
+def test_auto_solver_flags_a_duplicated_kernel_and_fp64_recovers(handle):
+    """Failure mode of the tensor-core Cholesky updates (LBCNN_SOLVER_AUTO from dimension 1024 on; ~2^-27 relative): a candidate
+    whose LAST layer holds the same kernel twice has two identical feature maps, the system is singular up to the ridge, and
+    the slice error may drive a pivot non-positive where the all-fp64 factorisation (and the oracle) succeeds.  Kernel sets
+    are an input, so such a candidate can arrive.  What is required:
+      - LBCNN_SOLVER_FP64: every candidate fits (info = 0) and matches the oracle;
+      - LBCNN_SOLVER_AUTO: never silently wrong -- a candidate either matches the oracle or is flagged (info > 0, acc = -1,
+        excluded from best / worst), and the healthy candidates are untouched by their neighbour's breakdown;
+      - the documented recipe works: the flagged candidate re-run alone under LBCNN_SOLVER_FP64 fits and matches."""
+    w = _small("gtsrb", 2600, 500, 3)
+    trx, try_, tex, tey = synth.make_dataset(w)
+    ker = synth.make_kernels(w).copy()
+    l2 = 16 * 3 * 9                                   # layer 2 starts here; each of its kernels has 16 * 9 = 144 taps
+    ker[1, l2 + 144:l2 + 288] = ker[1, l2:l2 + 144]   # candidate 1: layer-2 kernel 1 := kernel 0
+    arch = lb.arch_of(w)
+    args = lambda kk: (arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(kk))
+    ref = orc.search(_orc_arch(w), trx, try_, tex, tey, w.n_classes, w.C, ker, feature_scale=w.feature_scale, keep=True)
+    assert (ref["info"] == 0).all()
+    handle.set_workspace(None)
+    handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, w.n_cand)[0])
+    try:
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_FP64)
+        f = {k: v.cpu().numpy() for k, v in handle.search_candidates(*args(ker)).items()}
+        assert (f["info"] == 0).all()
+        assert (np.abs(f["acc"].astype(np.float64) - ref["acc"]) * 100.0 <= TOL_ACC_PP).all()
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_AUTO)
+        a = {k: v.cpu().numpy() for k, v in handle.search_candidates(*args(ker)).items()}
+        for k in range(w.n_cand):
+            if a["info"][k] == 0:
+                assert abs(float(a["acc"][k]) - ref["acc"][k]) * 100.0 <= TOL_ACC_PP, k
+            else:
+                assert k == 1 and a["info"][k] > 0 and a["acc"][k] == -1.0, (k, a["info"][k])
+        assert a["info"][0] == 0 and a["info"][2] == 0
+        assert int(a["best"][0]) != 1 or a["info"][1] == 0
+        if a["info"][1] != 0:                          # the recipe of include/lbcnn.h: re-run what was flagged in fp64
+            handle.set_option(lb.OPT_SOLVER, lb.SOLVER_FP64)
+            r = {k: v.cpu().numpy() for k, v in handle.search_candidates(*args(ker[1:2])).items()}
+            assert r["info"][0] == 0 and abs(float(r["acc"][0]) - ref["acc"][1]) * 100.0 <= TOL_ACC_PP
+        print("AUTO info on the duplicated-kernel candidate:", int(a["info"][1]))
+    finally:
+        handle.set_option(lb.OPT_SOLVER, lb.SOLVER_AUTO)
+        handle.set_workspace(None)
+
+
 def test_search_chunked_equals_unchunked(handle):
     w = _small("mnist", 400, 150, 7)
     arch = lb.arch_of(w)
