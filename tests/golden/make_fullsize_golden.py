@@ -30,7 +30,10 @@ from oracle import oracle as orc                      # noqa: E402
 from paper_2106_15350_b200 import synth               # noqa: E402
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-CANDS = {"gtsrb": [0], "vggface": [0]}
+# first, middle and last candidate of the launch bench.py times (128 / 32 candidates); W is kept for candidate 0 only
+# (8192 x 100 floats each: the others are compared through their labels and counts)
+CANDS = {"gtsrb": [0, 64, 127], "vggface": [0, 16, 31]}
+W_STORED = (0,)
 
 
 def input_key(trx, try_, tex, tey, ker_k, C, scale) -> np.ndarray:
@@ -61,11 +64,20 @@ def main(names):
         trx, try_, tex, tey = synth.make_dataset(w)
         ker = synth.make_kernels(w)
         out = {"cands": np.array(CANDS[name], dtype=np.int64)}
+        old = dict(np.load(path_of(name))) if os.path.exists(path_of(name)) else {}
         for k in CANDS[name]:
+            key = input_key(trx, try_, tex, tey, ker[k], w.C, float(np.float32(w.feature_scale)))
+            if ("key_%d" % k) in old and np.array_equal(old["key_%d" % k], key):      # stored for these very input bytes: keep
+                for f in ("W_%d", "pred_%d", "correct_%d", "margin_%d", "key_%d"):
+                    if (f % k) in old:
+                        out[f % k] = old[f % k]
+                print("%s candidate %d: kept (input key matches)" % (name, k), flush=True)
+                continue
             t0 = time.perf_counter()
             W, pred, corr, margin, info = oracle_candidate(w, trx, try_, tex, tey, ker[k])
             assert info == 0
-            out["W_%d" % k] = W.astype(np.float32)
+            if k in W_STORED:
+                out["W_%d" % k] = W.astype(np.float32)
             out["pred_%d" % k] = pred.astype(np.int16)
             out["correct_%d" % k] = np.array(corr, dtype=np.int64)
             out["margin_%d" % k] = margin.astype(np.float32)

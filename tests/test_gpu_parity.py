@@ -955,7 +955,7 @@ def test_full_size_expand_sampled(handle, name):
         assert np.array_equal(Hs[j].astype(np.int64), orc.expand(oa, trx[rows], ker[j])), (name, j)
 
 
-def _fullsize_reference(name, w, trx, try_, tex, tey, ker, k):
+def _fullsize_reference(name, w, trx, try_, tex, tey, ker, k, want_W=True):
     """the oracle's W / labels / margins of candidate k at full size: from tests/golden/fullsize_<name>.npz (written by
     tests/golden/make_fullsize_golden.py, which calls only oracle/) when its input key matches the bytes generated
     here, otherwise computed now by the oracle (minutes)."""
@@ -969,9 +969,9 @@ def _fullsize_reference(name, w, trx, try_, tex, tey, ker, k):
     path = mk.path_of(name)
     if os.path.exists(path):
         z = np.load(path)
-        if ("key_%d" % k) in z.files and np.array_equal(z["key_%d" % k], key):
-            return (z["W_%d" % k].astype(np.float64), z["pred_%d" % k].astype(np.int32), int(z["correct_%d" % k]),
-                    z["margin_%d" % k].astype(np.float64))
+        if ("key_%d" % k) in z.files and np.array_equal(z["key_%d" % k], key) and (("W_%d" % k) in z.files or not want_W):
+            Wz = z["W_%d" % k].astype(np.float64) if ("W_%d" % k) in z.files else None      # W is stored for candidate 0 only
+            return Wz, z["pred_%d" % k].astype(np.int32), int(z["correct_%d" % k]), z["margin_%d" % k].astype(np.float64)
     W, pred, corr, margin, info = mk.oracle_candidate(w, trx, try_, tex, tey, ker[k])
     assert info == 0
     return W, pred, corr, margin
@@ -1014,6 +1014,53 @@ def test_full_size_fit_score(handle, name):
     out = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker[:2]))
     assert int(out["correct"][0].item()) == int(corr[0]) and int(out["info"][0].item()) == 0
     handle.set_workspace(None)
+
+
+@pytest.mark.parametrize("name", ["gtsrb", "vggface"])
+def test_full_size_driver_at_full_candidate_count(handle, name):
+    """BASELINE.json configs[2] / configs[4] exactly as bench.py launches them: ALL 128 / 32 candidates at full N in one
+    lbcnn_search_candidates call with bench.py's 100 GB workspace budget (chunk planning at 75 / 61 GB, grid.z = the whole
+    batch, the band-major Gram tile order across candidates).  The first, the middle and the last candidate against the
+    oracle's stored full-size result (tests/golden/fullsize_<name>.npz, written by the oracle-only script beside it):
+    accuracy within 0.2 pp, and through the staged calls labels one by one; every candidate must fit (info = 0), the
+    accuracies must follow from the counts, best / worst must be the first maximum / minimum of the counts."""
+    import gc
+    w = synth.WORKLOADS[name]
+    data = synth.make_dataset(w)
+    trx, try_, tex, tey = data
+    ker = synth.make_kernels(w)
+    K = w.n_cand
+    arch = lb.arch_of(w)
+    handle.set_workspace(None)
+    gc.collect(); torch.cuda.empty_cache()
+    handle.ensure_workspace(lb.workspace_bytes(arch, w.n_train, w.n_test, w.n_classes, K, 100 << 30)[0])
+    out = handle.search_candidates(arch, _dev(trx), _dev(try_), _dev(tex), _dev(tey), w.n_classes, w.C, _dev(ker))
+    torch.cuda.synchronize()
+    got = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
+    handle.set_workspace(None)
+    del out
+    gc.collect(); torch.cuda.empty_cache()
+    assert (got["info"] == 0).all()
+    assert np.array_equal(got["acc"], (got["correct"].astype(np.float64) / w.n_test).astype(np.float32))
+    assert int(got["best"][0]) == int(np.argmax(got["correct"])) and int(got["best"][1]) == int(np.argmin(got["correct"]))
+    for k in (0, K // 2, K - 1):
+        Wo, po, co, margin = _fullsize_reference(name, w, trx, try_, tex, tey, ker, k, want_W=(k == 0))
+        assert co == int((po == tey).sum())
+        assert abs(int(got["correct"][k]) - co) / float(w.n_test) * 100.0 <= TOL_ACC_PP, (k, int(got["correct"][k]), co)
+        # labels one by one through the staged calls (same solver as the driver), tied to the driver by the equal count
+        try:
+            handle.set_option(lb.OPT_SOLVER, lb.SOLVER_MIXED)
+            W, pred, corr, info = _staged(handle, w, trx, try_, tex, tey, ker[k:k + 1])
+        finally:
+            handle.set_option(lb.OPT_SOLVER, lb.SOLVER_AUTO)
+        handle.set_workspace(None)
+        assert info[0] == 0 and int(corr[0]) == int(got["correct"][k]), ("driver and staged calls disagree", k)
+        differ = np.nonzero(pred[0] != po)[0]
+        assert 1.0 - len(differ) / float(w.n_test) >= TOL_LABEL_AGREE, (k, len(differ), margin[differ][:10])
+        if Wo is not None:
+            assert _fro(W[0], Wo) <= 1e-4
+            if int(got["best"][0]) == k:
+                assert _fro(got["W_best"].astype(np.float64), Wo) <= TOL_W_FRO
 
 
 # ---- exact integer Gram on the tensor cores (gram_tc.cu) -------------------------------------------------
