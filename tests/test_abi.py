@@ -36,7 +36,9 @@ def test_every_declared_symbol_is_exported():
 def test_version_and_status_strings():
     assert "sm_100a" in lb.version()
     assert lb.status_string(0) == "ok"
-    assert len({lb.status_string(i) for i in range(6)}) == 6
+    assert len({lb.status_string(i) for i in range(8)}) == 8
+    assert "built-in scratch" in lb.status_string(lb.ERR_STATIC_LIMIT)      # lbcnn_evolve_candidates_static's size refusal
+    assert lb.status_string(99) == "unknown status"
 
 
 def _dw_arch(h, w, c, mult):
